@@ -1,0 +1,500 @@
+/*
+ * wdmo.c -- CPU ORACLE for the split-step Schroedinger-Poisson + CIC particle step.
+ *
+ * TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and the
+ * cpu_baseline / --impl reference legs of bench.py may build, load or call this file.  It is
+ * plain, slow, float64 C written from the paper, shares no code with the CUDA path
+ * (paper_2606_25026_b200/csrc/) and is never tuned.
+ *
+ * What it follows (PAPER.md = /root/reference/PAPER.md at authoring time):
+ *   - kick-drift-kick split step, Eq. 16-18 and Algorithm 1 lines 5-16
+ *     (PAPER.md:247-267): (a) psi *= exp(-i Phi dt/(2 mu)), (b) psi = F^-1{exp(-i mu k^2 dt/2) F{psi}},
+ *     (c) Phi = F^-1{-4 pi G rho_k / k^2}, k = 0 mode zeroed (Eq. 23), (d) second half kick
+ *     with the NEW Phi.  mu = hbar/m; |psi|^2 is mass density (reading G6).
+ *   - grid x_i = -L/2 + i dx (Eq. 20) with dx = L/N (reading G1, periodic box).
+ *   - particles: "N-body particles contribute their gravitational potential to the grid ... the wave
+ *     dark matter gravitational acceleration is interpolated from the grid to particle positions"
+ *     (PAPER.md:314); realised, as BASELINE.json's north_star prescribes, by a cloud-in-cell deposit into
+ *     the Poisson source, a 2nd-order central-difference gradient (Eq. 21) gathered with
+ *     the same CIC weights, and a kick-drift-kick leapfrog sharing dt (readings G11-G16).
+ *   - the absorbing mask of Alg. 1 l.17-18 is NOT applied (reading G10; Eq. 22 is garbled).
+ *   - the 3-D DFT is separable; each 1-D transform is the textbook recursive radix-2
+ *     decimation-in-time FFT below; forward kernel e^{-ikx}, inverse carries 1/N per axis (reading G7).
+ *     A direct O(n^2) DFT is exported for the brute-force pin (tests/test_oracle_pins.py P5).
+ *
+ * Pins (tests/test_oracle_pins.py): P1 norm, P2 free Gaussian closed form, P3 plane wave,
+ * P4 single-mode Poisson, P5 direct DFT, P6 O(dt^2) energy error, P7 time reversal, P8 CIC
+ * momentum / mass / zero self force, P9 gather in a known field, P10 numpy.fft cross-check.
+ * The coupled psi+particle trajectory over many steps has no closed form: "parity unpinned"
+ * beyond P1, P7, P8 and second-order self-convergence.
+ *
+ * Threads: OpenMP over pencils / particles where the loop iterations are independent; the CIC
+ * deposit is serial (it is a scatter-add).  No blocking, fusion or reordering.
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef double complex cplx;
+
+enum { WDMO_OK = 0, WDMO_EINVAL = 1, WDMO_EUNSUPPORTED = 2, WDMO_ENOMEM = 3, WDMO_ESTATE = 5 };
+
+typedef struct wdmo_ctx {
+    int N;
+    double L, mu, G, dx;
+    size_t n;            /* N^3 */
+    cplx *psi;           /* N^3, C order (ix, iy, iz), iz contiguous */
+    cplx *work;          /* N^3 scratch */
+    double *rho, *phi;   /* N^3 */
+    long long np;
+    double *pos, *vel, *acc, *mass; /* np x 3, np */
+    int have_psi, stale;
+} wdmo_ctx;
+
+static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
+
+/* ---------------------------------------------------------------- 1-D transforms */
+
+/* Direct DFT: out[k] = sum_j in[j] exp(sign * 2 pi i j k / n).  O(n^2), any n. */
+static void dft_direct(const cplx *in, cplx *out, int n, int sign)
+{
+    for (int k = 0; k < n; ++k) {
+        cplx s = 0.0;
+        for (int j = 0; j < n; ++j) {
+            double a = sign * 2.0 * M_PI * (double)(((long long)j * k) % n) / (double)n;
+            s += in[j] * (cos(a) + I * sin(a));
+        }
+        out[k] = s;
+    }
+}
+
+/* Textbook recursive radix-2 decimation-in-time FFT.  tw[j] = exp(sign 2 pi i j / n_full);
+ * for a sub-transform of length n the twiddle w_n^k is tw[k * twstep], twstep = n_full / n. */
+static void fft_rec(const cplx *in, int stride, cplx *out, int n, const cplx *tw, int twstep)
+{
+    if (n == 1) { out[0] = in[0]; return; }
+    int h = n / 2;
+    fft_rec(in, 2 * stride, out, h, tw, 2 * twstep);              /* even samples */
+    fft_rec(in + stride, 2 * stride, out + h, h, tw, 2 * twstep); /* odd samples  */
+    for (int k = 0; k < h; ++k) {
+        cplx e = out[k], t = tw[k * twstep] * out[k + h];
+        out[k] = e + t;
+        out[k + h] = e - t;
+    }
+}
+
+static cplx *make_twiddles(int n, int sign)
+{
+    cplx *tw = (cplx *)malloc(sizeof(cplx) * (size_t)(n > 1 ? n : 1));
+    if (!tw) return NULL;
+    for (int j = 0; j < n; ++j) {
+        double a = sign * 2.0 * M_PI * (double)j / (double)n;
+        tw[j] = cos(a) + I * sin(a);
+    }
+    return tw;
+}
+
+/* sign = -1 forward (unnormalised), +1 inverse (times 1/n). */
+int wdmo_fft1d(int n, const double *in, double *out, int sign)
+{
+    if (!is_pow2(n) || !in || !out || (sign != 1 && sign != -1)) return WDMO_EINVAL;
+    cplx *tw = make_twiddles(n, sign);
+    if (!tw) return WDMO_ENOMEM;
+    fft_rec((const cplx *)in, 1, (cplx *)out, n, tw, 1);
+    if (sign == 1) for (int j = 0; j < n; ++j) ((cplx *)out)[j] /= (double)n;
+    free(tw);
+    return WDMO_OK;
+}
+
+int wdmo_dft1d_direct(int n, const double *in, double *out, int sign)
+{
+    if (n < 1 || !in || !out || (sign != 1 && sign != -1)) return WDMO_EINVAL;
+    dft_direct((const cplx *)in, (cplx *)out, n, sign);
+    if (sign == 1) for (int j = 0; j < n; ++j) ((cplx *)out)[j] /= (double)n;
+    return WDMO_OK;
+}
+
+/* ---------------------------------------------------------------- 3-D transforms */
+
+/* In-place separable 3-D DFT of a[N][N][N]: one 1-D transform along every pencil of each axis. */
+static int fft3_inplace(cplx *a, int N, int sign)
+{
+    cplx *tw = make_twiddles(N, sign);
+    if (!tw) return WDMO_ENOMEM;
+    size_t N2 = (size_t)N * N;
+    int fail = 0;
+    for (int axis = 2; axis >= 0; --axis) {
+        size_t st = axis == 2 ? 1 : (axis == 1 ? (size_t)N : N2);        /* stride along the axis */
+#pragma omp parallel
+        {
+            cplx *line = (cplx *)malloc(sizeof(cplx) * 2 * (size_t)N);
+            if (!line) {
+#pragma omp atomic write
+                fail = 1;
+            }
+#pragma omp for schedule(static)
+            for (long long p = 0; p < (long long)N2; ++p) {
+                if (!line) continue;
+                size_t u = (size_t)p / N, v = (size_t)p % N, base;     /* the two other indices */
+                if (axis == 2) base = u * N2 + v * N;                    /* (ix=u, iy=v, :)  */
+                else if (axis == 1) base = u * N2 + v;                   /* (ix=u, :, iz=v)  */
+                else base = u * N + v;                                   /* (:, iy=u, iz=v)  */
+                cplx *in = line, *out = line + N;
+                for (int j = 0; j < N; ++j) in[j] = a[base + j * st];
+                fft_rec(in, 1, out, N, tw, 1);
+                if (sign == 1) for (int j = 0; j < N; ++j) a[base + j * st] = out[j] / (double)N;
+                else for (int j = 0; j < N; ++j) a[base + j * st] = out[j];
+            }
+            free(line);
+        }
+    }
+    free(tw);
+    return fail ? WDMO_ENOMEM : WDMO_OK;
+}
+
+int wdmo_fft3(int N, const double *in, double *out, int sign)
+{
+    if (!is_pow2(N) || !in || !out || (sign != 1 && sign != -1)) return WDMO_EINVAL;
+    size_t n = (size_t)N * N * N;
+    if (in != out) memcpy(out, in, sizeof(cplx) * n);
+    return fft3_inplace((cplx *)out, N, sign);
+}
+
+/* Brute force: out[k] = sum_j in[j] exp(sign 2 pi i (j.k)/N), the plain triple sum.  O(N^6). */
+int wdmo_dft3_direct(int N, const double *in_, double *out_, int sign)
+{
+    if (N < 1 || N > 16 || !in_ || !out_ || (sign != 1 && sign != -1)) return WDMO_EINVAL;
+    const cplx *in = (const cplx *)in_;
+    cplx *out = (cplx *)out_;
+    for (int kx = 0; kx < N; ++kx) for (int ky = 0; ky < N; ++ky) for (int kz = 0; kz < N; ++kz) {
+        cplx s = 0.0;
+        for (int jx = 0; jx < N; ++jx) for (int jy = 0; jy < N; ++jy) for (int jz = 0; jz < N; ++jz) {
+            long long m = ((long long)jx * kx + (long long)jy * ky + (long long)jz * kz) % N;
+            double a = sign * 2.0 * M_PI * (double)m / (double)N;
+            s += in[((size_t)jx * N + jy) * N + jz] * (cos(a) + I * sin(a));
+        }
+        if (sign == 1) s /= (double)N * N * N;
+        out[((size_t)kx * N + ky) * N + kz] = s;
+    }
+    return WDMO_OK;
+}
+
+/* signed wavenumber k = 2 pi s(j) / L, s(j) = j for j < N/2 else j - N (reading G4) */
+static double wavenumber(int j, int N, double L)
+{
+    int s = j < N / 2 ? j : j - N;
+    if (N == 1) s = 0;
+    return 2.0 * M_PI * (double)s / L;
+}
+
+/* ---------------------------------------------------------------- Poisson (Eq. 18c, Eq. 23) */
+
+/* phi = Re F^-1{ -4 pi G rho_k / k^2 }, rho_k(k=0) dropped  ( == subtracting <rho>, reading G3 ). */
+static int poisson(const double *rho, double *phi, cplx *work, int N, double L, double G)
+{
+    size_t n = (size_t)N * N * N;
+    for (size_t i = 0; i < n; ++i) work[i] = rho[i];
+    int rc = fft3_inplace(work, N, -1);
+    if (rc) return rc;
+#pragma omp parallel for schedule(static)
+    for (int ix = 0; ix < N; ++ix) {
+        double kx = wavenumber(ix, N, L);
+        for (int iy = 0; iy < N; ++iy) {
+            double ky = wavenumber(iy, N, L);
+            for (int iz = 0; iz < N; ++iz) {
+                double kz = wavenumber(iz, N, L);
+                double k2 = kx * kx + ky * ky + kz * kz;
+                size_t i = ((size_t)ix * N + iy) * N + iz;
+                if (ix == 0 && iy == 0 && iz == 0) work[i] = 0.0;
+                else work[i] *= -4.0 * M_PI * G / k2;
+            }
+        }
+    }
+    rc = fft3_inplace(work, N, +1);
+    if (rc) return rc;
+    for (size_t i = 0; i < n; ++i) phi[i] = creal(work[i]);
+    return WDMO_OK;
+}
+
+int wdmo_poisson(int N, double L, double G, const double *rho, double *phi)
+{
+    if (!is_pow2(N) || L <= 0 || !rho || !phi) return WDMO_EINVAL;
+    cplx *work = (cplx *)malloc(sizeof(cplx) * (size_t)N * N * N);
+    if (!work) return WDMO_ENOMEM;
+    int rc = poisson(rho, phi, work, N, L, G);
+    free(work);
+    return rc;
+}
+
+/* ---------------------------------------------------------------- cloud-in-cell (readings G12, G13) */
+
+static int wrap_index(long long i, int N) { long long r = i % N; return (int)(r < 0 ? r + N : r); }
+
+/* rho[(i0 + corner) mod N] += m w / dx^3 for the 8 nodes around each particle; u = (x + L/2)/dx,
+ * i0 = floor(u), f = u - i0, w = prod_axis (f if corner bit else 1 - f).  Adds into rho. */
+static void cic_deposit(double *rho, int N, double L, long long np, const double *pos,
+                        const double *mass)
+{
+    double dx = L / N, inv_vol = 1.0 / (dx * dx * dx);
+    for (long long p = 0; p < np; ++p) {
+        long long i0[3]; double f[3];
+        for (int a = 0; a < 3; ++a) {
+            double u = (pos[3 * p + a] + 0.5 * L) / dx;
+            double fl = floor(u);
+            i0[a] = (long long)fl;
+            f[a] = u - fl;
+        }
+        for (int c = 0; c < 8; ++c) {
+            int bx = (c >> 2) & 1, by = (c >> 1) & 1, bz = c & 1;
+            double w = (bx ? f[0] : 1.0 - f[0]) * (by ? f[1] : 1.0 - f[1]) * (bz ? f[2] : 1.0 - f[2]);
+            size_t idx = ((size_t)wrap_index(i0[0] + bx, N) * N + wrap_index(i0[1] + by, N)) * N
+                         + wrap_index(i0[2] + bz, N);
+            rho[idx] += mass[p] * w * inv_vol;
+        }
+    }
+}
+
+/* g_axis[node] = -(phi[node + e_axis] - phi[node - e_axis]) / (2 dx)  (Eq. 21), then
+ * a_axis(x_p) = sum_corners w g_axis[(i0 + corner) mod N] with the deposit's weights. */
+static void cic_gather(const double *phi, int N, double L, long long np, const double *pos, double *acc)
+{
+    double dx = L / N;
+#pragma omp parallel for schedule(static)
+    for (long long p = 0; p < np; ++p) {
+        long long i0[3]; double f[3];
+        for (int a = 0; a < 3; ++a) {
+            double u = (pos[3 * p + a] + 0.5 * L) / dx;
+            double fl = floor(u);
+            i0[a] = (long long)fl;
+            f[a] = u - fl;
+        }
+        double ax = 0.0, ay = 0.0, az = 0.0;
+        for (int c = 0; c < 8; ++c) {
+            int bx = (c >> 2) & 1, by = (c >> 1) & 1, bz = c & 1;
+            double w = (bx ? f[0] : 1.0 - f[0]) * (by ? f[1] : 1.0 - f[1]) * (bz ? f[2] : 1.0 - f[2]);
+            int ix = wrap_index(i0[0] + bx, N), iy = wrap_index(i0[1] + by, N), iz = wrap_index(i0[2] + bz, N);
+#define PHI(a, b, c_) phi[((size_t)wrap_index((a), N) * N + wrap_index((b), N)) * N + wrap_index((c_), N)]
+            ax += w * -(PHI(ix + 1, iy, iz) - PHI(ix - 1, iy, iz)) / (2.0 * dx);
+            ay += w * -(PHI(ix, iy + 1, iz) - PHI(ix, iy - 1, iz)) / (2.0 * dx);
+            az += w * -(PHI(ix, iy, iz + 1) - PHI(ix, iy, iz - 1)) / (2.0 * dx);
+#undef PHI
+        }
+        acc[3 * p] = ax; acc[3 * p + 1] = ay; acc[3 * p + 2] = az;
+    }
+}
+
+int wdmo_cic_deposit(int N, double L, long long np, const double *pos, const double *mass, double *rho)
+{
+    if (N < 1 || L <= 0 || np < 0 || !rho || (np > 0 && (!pos || !mass))) return WDMO_EINVAL;
+    cic_deposit(rho, N, L, np, pos, mass);
+    return WDMO_OK;
+}
+
+int wdmo_cic_gather(int N, double L, const double *phi, long long np, const double *pos, double *acc)
+{
+    if (N < 1 || L <= 0 || np < 0 || !phi || (np > 0 && (!pos || !acc))) return WDMO_EINVAL;
+    cic_gather(phi, N, L, np, pos, acc);
+    return WDMO_OK;
+}
+
+/* ---------------------------------------------------------------- context */
+
+int wdmo_create(wdmo_ctx **out, int N, double L, double hbar_over_m, double G)
+{
+    if (!out) return WDMO_EINVAL;
+    *out = NULL;
+    if (!(L > 0) || !(hbar_over_m > 0) || !(G >= 0)) return WDMO_EINVAL;
+    if (!is_pow2(N) || N < 2 || N > 1024) return WDMO_EUNSUPPORTED;
+    wdmo_ctx *c = (wdmo_ctx *)calloc(1, sizeof(*c));
+    if (!c) return WDMO_ENOMEM;
+    c->N = N; c->L = L; c->mu = hbar_over_m; c->G = G; c->dx = L / N;
+    c->n = (size_t)N * N * N;
+    c->psi = (cplx *)malloc(sizeof(cplx) * c->n);
+    c->work = (cplx *)malloc(sizeof(cplx) * c->n);
+    c->rho = (double *)malloc(sizeof(double) * c->n);
+    c->phi = (double *)malloc(sizeof(double) * c->n);
+    if (!c->psi || !c->work || !c->rho || !c->phi) {
+        free(c->psi); free(c->work); free(c->rho); free(c->phi); free(c);
+        return WDMO_ENOMEM;
+    }
+    c->stale = 1;
+    *out = c;
+    return WDMO_OK;
+}
+
+int wdmo_destroy(wdmo_ctx *c)
+{
+    if (!c) return WDMO_OK;
+    free(c->psi); free(c->work); free(c->rho); free(c->phi);
+    free(c->pos); free(c->vel); free(c->acc); free(c->mass);
+    free(c);
+    return WDMO_OK;
+}
+
+int wdmo_set_psi(wdmo_ctx *c, const double *psi)
+{
+    if (!c || !psi) return WDMO_EINVAL;
+    memcpy(c->psi, psi, sizeof(cplx) * c->n);
+    c->have_psi = 1; c->stale = 1;
+    return WDMO_OK;
+}
+
+/* x <- x - L floor((x + L/2)/L): into [-L/2, L/2)  (reading G16) */
+static double wrap_pos(double x, double L)
+{
+    double y = x - L * floor((x + 0.5 * L) / L);
+    if (y >= 0.5 * L) y -= L;       /* guard the rounding case x + L/2 just below a multiple of L */
+    if (y < -0.5 * L) y += L;
+    return y;
+}
+
+int wdmo_set_particles(wdmo_ctx *c, long long np, const double *pos, const double *vel,
+                       const double *mass, double mass_scalar)
+{
+    if (!c || np < 0 || (np > 0 && (!pos || !vel))) return WDMO_EINVAL;
+    free(c->pos); free(c->vel); free(c->acc); free(c->mass);
+    c->pos = c->vel = c->acc = c->mass = NULL; c->np = 0;
+    if (np > 0) {
+        c->pos = (double *)malloc(sizeof(double) * 3 * (size_t)np);
+        c->vel = (double *)malloc(sizeof(double) * 3 * (size_t)np);
+        c->acc = (double *)calloc(3 * (size_t)np, sizeof(double));
+        c->mass = (double *)malloc(sizeof(double) * (size_t)np);
+        if (!c->pos || !c->vel || !c->acc || !c->mass) return WDMO_ENOMEM;
+        for (long long i = 0; i < 3 * np; ++i) { c->pos[i] = wrap_pos(pos[i], c->L); c->vel[i] = vel[i]; }
+        for (long long p = 0; p < np; ++p) c->mass[p] = mass ? mass[p] : mass_scalar;
+        c->np = np;
+    }
+    c->stale = 1;
+    return WDMO_OK;
+}
+
+/* rho = |psi|^2 + CIC(x);  Phi = Poisson(rho);  a = Gather(Phi, x)   (Alg. 1 l.12-15; G8, G22) */
+static int update_potential(wdmo_ctx *c)
+{
+    for (size_t i = 0; i < c->n; ++i) {
+        double re = creal(c->psi[i]), im = cimag(c->psi[i]);
+        c->rho[i] = re * re + im * im;
+    }
+    if (c->np > 0) cic_deposit(c->rho, c->N, c->L, c->np, c->pos, c->mass);
+    int rc = poisson(c->rho, c->phi, c->work, c->N, c->L, c->G);
+    if (rc) return rc;
+    if (c->np > 0) cic_gather(c->phi, c->N, c->L, c->np, c->pos, c->acc);
+    return WDMO_OK;
+}
+
+static int refresh(wdmo_ctx *c)
+{
+    if (!c->have_psi) return WDMO_ESTATE;
+    if (!c->stale) return WDMO_OK;
+    int rc = update_potential(c);
+    if (rc) return rc;
+    c->stale = 0;
+    return WDMO_OK;
+}
+
+/* psi *= exp(-i Phi h / mu), h = dt/2  (Eq. 18a/d; N^ = -i Phi) ; v += a h */
+static void half_kick(wdmo_ctx *c, double h)
+{
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < (long long)c->n; ++i) {
+        double th = -c->phi[i] * h / c->mu;
+        c->psi[i] *= cos(th) + I * sin(th);
+    }
+    for (long long i = 0; i < 3 * c->np; ++i) c->vel[i] += c->acc[i] * h;
+}
+
+/* psi = F^-1{ exp(-i mu k^2 dt/2) F{psi} }  (Eq. 18b) ;  x += v dt, wrapped */
+static int drift(wdmo_ctx *c, double dt)
+{
+    int N = c->N;
+    int rc = fft3_inplace(c->psi, N, -1);
+    if (rc) return rc;
+#pragma omp parallel for schedule(static)
+    for (int ix = 0; ix < N; ++ix) {
+        double kx = wavenumber(ix, N, c->L);
+        for (int iy = 0; iy < N; ++iy) {
+            double ky = wavenumber(iy, N, c->L);
+            for (int iz = 0; iz < N; ++iz) {
+                double kz = wavenumber(iz, N, c->L);
+                double th = -0.5 * c->mu * (kx * kx + ky * ky + kz * kz) * dt;
+                c->psi[((size_t)ix * N + iy) * N + iz] *= cos(th) + I * sin(th);
+            }
+        }
+    }
+    rc = fft3_inplace(c->psi, N, +1);
+    if (rc) return rc;
+    for (long long i = 0; i < 3 * c->np; ++i) c->pos[i] = wrap_pos(c->pos[i] + c->vel[i] * dt, c->L);
+    return WDMO_OK;
+}
+
+int wdmo_step(wdmo_ctx *c, int nsteps, double dt)
+{
+    if (!c || nsteps < 0) return WDMO_EINVAL;
+    int rc = refresh(c);
+    if (rc) return rc;
+    for (int s = 0; s < nsteps; ++s) {
+        half_kick(c, 0.5 * dt);                 /* (a) + particle half kick with a^n        */
+        rc = drift(c, dt);                      /* (b) + particle drift                      */
+        if (rc) return rc;
+        rc = update_potential(c);               /* (c) rho, Phi^{n+1}, a^{n+1}               */
+        if (rc) return rc;
+        half_kick(c, 0.5 * dt);                 /* (d) with the new Phi + closing half kick  */
+    }
+    return WDMO_OK;
+}
+
+int wdmo_get_psi(wdmo_ctx *c, double *out)
+{
+    if (!c || !out) return WDMO_EINVAL;
+    if (!c->have_psi) return WDMO_ESTATE;
+    memcpy(out, c->psi, sizeof(cplx) * c->n);
+    return WDMO_OK;
+}
+
+int wdmo_get_density(wdmo_ctx *c, double *out)
+{
+    if (!c || !out) return WDMO_EINVAL;
+    int rc = refresh(c);
+    if (rc) return rc;
+    memcpy(out, c->rho, sizeof(double) * c->n);
+    return WDMO_OK;
+}
+
+int wdmo_get_potential(wdmo_ctx *c, double *out)
+{
+    if (!c || !out) return WDMO_EINVAL;
+    int rc = refresh(c);
+    if (rc) return rc;
+    memcpy(out, c->phi, sizeof(double) * c->n);
+    return WDMO_OK;
+}
+
+int wdmo_get_particles(wdmo_ctx *c, double *pos, double *vel)
+{
+    if (!c) return WDMO_EINVAL;
+    if (pos) memcpy(pos, c->pos, sizeof(double) * 3 * (size_t)c->np);
+    if (vel) memcpy(vel, c->vel, sizeof(double) * 3 * (size_t)c->np);
+    return WDMO_OK;
+}
+
+int wdmo_get_accel(wdmo_ctx *c, double *acc)
+{
+    if (!c || !acc) return WDMO_EINVAL;
+    int rc = refresh(c);
+    if (rc) return rc;
+    memcpy(acc, c->acc, sizeof(double) * 3 * (size_t)c->np);
+    return WDMO_OK;
+}
+
+int wdmo_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

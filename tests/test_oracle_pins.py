@@ -1,0 +1,328 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these compares the oracle with itself by retyping its formula: each expected value is a
+closed form, an invariant, a brute-force sum, or a library routine used as a check OF the oracle.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import wdm_workloads as wl
+
+FOUR_PI = 4.0 * math.pi
+
+
+def grid(N, L=1.0):
+    x = -0.5 * L + (L / N) * np.arange(N)
+    return np.meshgrid(x, x, x, indexing="ij")
+
+
+def relerr(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(np.asarray(b).ravel()))
+
+
+def run(N, psi, nsteps, dt, L=1.0, mu=1.0, G=1.0 / FOUR_PI, particles=None):
+    o = oracle.Oracle(N, L, mu, G)
+    o.set_psi(psi)
+    if particles is not None:
+        o.set_particles(*particles)
+    o.step(nsteps, dt)
+    return o
+
+
+# ---------------------------------------------------------------- P5 / P10: the FFT itself
+
+@pytest.mark.parametrize("n", [2, 4, 8, 16, 64, 256, 1024])
+def test_p5_fft1d_vs_direct_dft(n):
+    rng = np.random.default_rng(n)
+    x = rng.normal(size=n) + 1j * rng.normal(size=n)
+    f = oracle.fft1d(x, -1)
+    d = oracle.dft1d_direct(x, -1)
+    assert relerr(f, d) < 1e-13
+    # the direct sum is itself the definition sum_j x_j e^{-2 pi i jk/n}: spot-check one bin by hand
+    k = n // 3
+    assert abs(d[k] - sum(x[j] * np.exp(-2j * np.pi * j * k / n) for j in range(n))) < 1e-10
+    # inverse carries 1/n and round-trips
+    assert relerr(oracle.fft1d(f, +1), x) < 1e-13
+
+
+def test_p5_fft3_vs_bruteforce_triple_sum_8cubed():
+    a = wl.random_field(8, "c128", 5)
+    assert relerr(oracle.fft3(a, -1), oracle.dft3_direct(a, -1)) < 1e-13
+    assert relerr(oracle.fft3(a, +1), oracle.dft3_direct(a, +1)) < 1e-13
+    # a delta at (1,2,3) transforms to the plane wave e^{-2 pi i (kx+2ky+3kz)/8}: fixes sign + axis order
+    d = np.zeros((8, 8, 8), complex); d[1, 2, 3] = 1.0
+    k = np.arange(8)
+    KX, KY, KZ = np.meshgrid(k, k, k, indexing="ij")
+    assert relerr(oracle.fft3(d, -1), np.exp(-2j * np.pi * (KX + 2 * KY + 3 * KZ) / 8)) < 1e-14
+
+
+@pytest.mark.parametrize("N", [16, 32, 64])
+def test_p10_fft3_vs_numpy(N):
+    a = wl.random_field(N, "c128", N)
+    assert relerr(oracle.fft3(a, -1), np.fft.fftn(a)) < 1e-13
+    assert relerr(oracle.fft3(a, +1), np.fft.ifftn(a)) < 1e-13
+
+
+# ---------------------------------------------------------------- P1: unitarity
+
+def test_p1_norm_conserved_config1():
+    w = wl.config1()
+    n0 = np.sum(np.abs(w.psi) ** 2) * w.dx ** 3
+    assert abs(n0 - 1.0) < 1e-12                      # G19: normalised input
+    o = run(w.N, w.psi, 10, w.dt)
+    n1 = np.sum(np.abs(o.psi()) ** 2) * w.dx ** 3
+    assert abs(n1 - n0) < 1e-13
+
+
+def test_p1_norm_conserved_strong_gravity():
+    N = 16
+    psi = wl.random_field(N, "c128", 1) + 3.0
+    o = run(N, psi, 20, 1e-3, G=50.0)
+    assert abs(np.sum(np.abs(o.psi()) ** 2) / np.sum(np.abs(psi) ** 2) - 1.0) < 1e-13
+
+
+# ---------------------------------------------------------------- P2: free Gaussian packet
+
+def gaussian_packet(X, Y, Z, sigma, k0, t, mu):
+    """psi(x,t) for psi(x,0) = (2 pi s^2)^(-3/4) exp(-|x|^2/4s^2 + i k0.x), free Schroedinger
+    i psi_t = -(mu/2) lap psi  (textbook spreading Gaussian)."""
+    tau = mu * t / (2.0 * sigma ** 2)
+    xc = [X - mu * k0[0] * t, Y - mu * k0[1] * t, Z - mu * k0[2] * t]
+    r2 = xc[0] ** 2 + xc[1] ** 2 + xc[2] ** 2
+    kk = float(np.dot(k0, k0))
+    phase = k0[0] * xc[0] + k0[1] * xc[1] + k0[2] * xc[2] + 0.5 * mu * kk * t
+    return (2 * np.pi * sigma ** 2) ** -0.75 * (1 + 1j * tau) ** -1.5 * np.exp(-r2 / (4 * sigma ** 2 * (1 + 1j * tau)) + 1j * phase)
+
+
+@pytest.mark.parametrize("nsteps", [1, 7])
+def test_p2_free_gaussian_closed_form(nsteps):
+    N, L, mu = 64, 1.0, 0.7
+    sigma = 0.04 * L
+    k0 = 2 * np.pi / L * np.array([3.0, -2.0, 1.0])
+    X, Y, Z = grid(N, L)
+    psi0 = gaussian_packet(X, Y, Z, sigma, k0, 0.0, mu)
+    T = 2.0 * sigma ** 2 / mu * 0.6            # tau = 0.6: width grows by sqrt(1.36)
+    o = run(N, psi0, nsteps, T / nsteps, L=L, mu=mu, G=0.0)
+    exact = gaussian_packet(X, Y, Z, sigma, k0, T, mu)
+    # spectral drift is exact for any dt: residual = periodic images + sampling only
+    assert relerr(o.psi(), exact) < 1e-9
+    # and the packet really moved and spread (guards a no-op)
+    assert relerr(psi0, exact) > 0.5
+
+
+def test_p2_sign_of_drift_phase():
+    """A wrong sign of the kinetic phase conjugates the evolution: check against the conjugate too."""
+    N, L, mu = 32, 1.0, 1.0
+    X, Y, Z = grid(N, L)
+    sigma = 0.08
+    k0 = 2 * np.pi * np.array([1.0, 0.0, 0.0])
+    T = 0.004
+    o = run(N, gaussian_packet(X, Y, Z, sigma, k0, 0.0, mu), 2, T / 2, G=0.0)
+    good = gaussian_packet(X, Y, Z, sigma, k0, T, mu)
+    bad = gaussian_packet(X, Y, Z, sigma, k0, -T, mu)
+    assert relerr(o.psi(), good) < 1e-3 < 0.1 < relerr(o.psi(), bad)   # 1e-3: periodic images of a sigma=0.08L packet
+
+
+# ---------------------------------------------------------------- P3: plane wave with gravity on
+
+def test_p3_plane_wave_exact():
+    N, L, mu = 16, 2.0, 1.3
+    X, Y, Z = grid(N, L)
+    n = np.array([2, -1, 3])
+    k = 2 * np.pi * n / L
+    A = 0.8 - 0.3j
+    psi0 = A * np.exp(1j * (k[0] * X + k[1] * Y + k[2] * Z))
+    dt, ns = 0.01, 9
+    o = run(N, psi0, ns, dt, L=L, mu=mu, G=3.0)
+    exact = psi0 * np.exp(-0.5j * mu * float(k @ k) * dt * ns)
+    assert relerr(o.psi(), exact) < 1e-13
+    assert np.max(np.abs(o.potential())) < 1e-12        # uniform density -> Phi = 0 (k=0 zeroed)
+    assert np.allclose(o.density(), abs(A) ** 2, rtol=1e-13)
+
+
+# ---------------------------------------------------------------- P4: single-mode Poisson
+
+def test_p4_single_mode_poisson_closed_form():
+    N, L, G = 32, 1.5, 0.37
+    X, Y, Z = grid(N, L)
+    n = np.array([1, 2, -3])
+    k = 2 * np.pi * n / L
+    rho0, rho1 = 5.0, 0.25
+    arg = k[0] * X + k[1] * Y + k[2] * Z
+    rho = rho0 + rho1 * np.cos(arg)
+    phi = oracle.poisson(rho, L, G)
+    exact = -4 * np.pi * G * rho1 * np.cos(arg) / float(k @ k)
+    assert relerr(phi, exact) < 1e-13
+    assert abs(phi.mean()) < 1e-15
+    # through the context as well: psi = sqrt(rho) gives the same potential
+    o = oracle.Oracle(N, L, 1.0, G); o.set_psi(np.sqrt(rho).astype(complex))
+    assert relerr(o.potential(), exact) < 1e-12
+
+
+def test_p4_poisson_discrete_laplacian_of_smooth_field():
+    """lap Phi = 4 pi G (rho - <rho>) checked spectrally-independent: 2nd-order FD Laplacian converges."""
+    L, G = 1.0, 1.0 / FOUR_PI
+    errs = []
+    for N in (16, 32):
+        X, Y, Z = grid(N, L)
+        rho = np.exp(np.cos(2 * np.pi * X) + np.sin(2 * np.pi * Y) * np.cos(2 * np.pi * Z))
+        phi = oracle.poisson(rho, L, G)
+        dx = L / N
+        lap = sum(np.roll(phi, 1, a) + np.roll(phi, -1, a) - 2 * phi for a in range(3)) / dx ** 2
+        errs.append(relerr(lap, FOUR_PI * G * (rho - rho.mean())))
+    assert errs[1] < errs[0] / 3.5 and errs[1] < 0.02
+
+
+# ---------------------------------------------------------------- P6: second-order energy error
+
+def total_energy(psi, phi, L, mu):
+    """E = T + W: T = (mu^2/2) sum_k k^2 |psi_k|^2 dV/N^3 (Parseval), W = (1/2) sum rho Phi dV."""
+    N = psi.shape[0]
+    dV = (L / N) ** 3
+    k = 2 * np.pi * np.fft.fftfreq(N, d=L / N)
+    K2 = k[:, None, None] ** 2 + k[None, :, None] ** 2 + k[None, None, :] ** 2
+    pk = np.fft.fftn(psi)
+    T = 0.5 * mu ** 2 * float(np.sum(K2 * np.abs(pk) ** 2)) * dV / N ** 3
+    W = 0.5 * float(np.sum(np.abs(psi) ** 2 * phi)) * dV
+    return T + W
+
+
+def test_p6_energy_error_is_second_order():
+    N, L, mu, G = 16, 1.0, 1.0, 200.0 / FOUR_PI
+    X, Y, Z = grid(N, L)
+    psi0 = (2.0 + np.exp(2j * np.pi * X) + 0.7 * np.exp(2j * np.pi * (Y - Z)) + 0.4 * np.cos(2 * np.pi * Z)).astype(complex)
+    Tend = 0.02
+    drifts = []
+    for ns in (8, 16, 32, 64):
+        o = oracle.Oracle(N, L, mu, G); o.set_psi(psi0)
+        e0 = total_energy(o.psi(), o.potential(), L, mu)
+        worst = 0.0
+        for _ in range(ns):
+            o.step(1, Tend / ns)
+            worst = max(worst, abs(total_energy(o.psi(), o.potential(), L, mu) - e0))
+        drifts.append(worst / abs(e0))
+    ratios = [drifts[i] / drifts[i + 1] for i in range(3)]
+    assert drifts[0] > 1e-9                      # gravity is actually doing something
+    assert all(3.6 < r < 4.4 for r in ratios), (drifts, ratios)
+
+
+def test_p6_solution_self_convergence_second_order():
+    N, L, G = 16, 1.0, 100.0 / FOUR_PI
+    psi0 = wl.small_coupled(N).psi
+    Tend = 0.004
+    sols = [run(N, psi0, ns, Tend / ns, G=G).psi() for ns in (4, 8, 16, 32)]
+    d = [np.linalg.norm(sols[i] - sols[i + 1]) for i in range(3)]
+    assert 3.6 < d[0] / d[1] < 4.4 and 3.6 < d[1] / d[2] < 4.4, d
+
+
+# ---------------------------------------------------------------- P7: time reversal (whole coupled step)
+
+def test_p7_time_reversal_with_particles():
+    w = wl.small_coupled(16)
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    o.set_psi(w.psi); o.set_particles(w.pos, w.vel, w.mass)
+    o.step(12, w.dt)
+    moved = relerr(o.psi(), w.psi)
+    o.step(12, -w.dt)
+    pos, vel = o.particles()
+    assert moved > 1e-3
+    assert relerr(o.psi(), w.psi) < 1e-12
+    d = pos - w.pos; d -= w.L * np.round(d / w.L)
+    assert np.max(np.abs(d)) < 1e-13 and np.max(np.abs(vel - w.vel)) < 1e-11
+
+
+# ---------------------------------------------------------------- P8: CIC deposit / gather pair
+
+def test_p8_cic_mass_node_and_weights():
+    N, L = 8, 2.0
+    dx = L / N
+    # a particle exactly on node (3,0,7) deposits m/dx^3 there and nothing elsewhere
+    pos = np.array([[-L / 2 + 3 * dx, -L / 2, -L / 2 + 7 * dx]])
+    rho = oracle.cic_deposit(N, L, pos, 2.5)
+    assert rho[3, 0, 7] == pytest.approx(2.5 / dx ** 3, rel=1e-14)
+    assert np.count_nonzero(rho) == 1
+    # a quarter of the way from node (7,7,7) towards (0,0,0) across the periodic face, per axis
+    pos = np.array([[L / 2 - 0.75 * dx] * 3])
+    rho = oracle.cic_deposit(N, L, pos, 1.0) * dx ** 3
+    assert rho[7, 7, 7] == pytest.approx(0.75 ** 3) and rho[0, 0, 0] == pytest.approx(0.25 ** 3)
+    assert rho[0, 7, 7] == pytest.approx(0.25 * 0.75 ** 2) and rho[7, 0, 0] == pytest.approx(0.75 * 0.25 ** 2)
+    assert rho.sum() == pytest.approx(1.0, rel=1e-14)
+    # total mass of a random cloud with individual masses
+    rng = np.random.default_rng(3)
+    p = rng.uniform(-L / 2, L / 2, size=(500, 3)); m = rng.uniform(0.1, 2.0, size=500)
+    assert oracle.cic_deposit(N, L, p, m).sum() * dx ** 3 == pytest.approx(m.sum(), rel=1e-13)
+
+
+def test_p8_zero_self_force_and_momentum_conservation():
+    N, L, G = 16, 1.0, 1.0
+    rng = np.random.default_rng(8)
+    o = oracle.Oracle(N, L, 1.0, G)
+    o.set_psi(np.zeros((N, N, N), complex))
+    # single particle: no self force
+    o.set_particles(rng.uniform(-0.5, 0.5, size=(1, 3)), np.zeros((1, 3)), 1.0)
+    assert np.max(np.abs(o.accel())) < 1e-12
+    # many particles: total momentum change vanishes
+    p = rng.uniform(-0.5, 0.5, size=(200, 3)); m = rng.uniform(0.5, 1.5, size=200)
+    o.set_particles(p, np.zeros((200, 3)), m)
+    a = o.accel()
+    assert np.max(np.abs(a)) > 1.0
+    assert np.max(np.abs((m[:, None] * a).sum(0))) < 1e-11 * np.abs(m[:, None] * a).sum()
+    # two particles attract each other (sign of gravity)
+    o.set_particles(np.array([[-0.1, 0.02, 0.0], [0.1, 0.0, 0.03]]), np.zeros((2, 3)), 1.0)
+    a = o.accel()
+    assert a[0, 0] > 0 > a[1, 0]
+
+
+# ---------------------------------------------------------------- P9: gather in a known field
+
+def test_p9_gather_closed_form():
+    N, L = 16, 1.0
+    dx = L / N
+    X, Y, Z = grid(N, L)
+    kk = 2 * np.pi * 2 / L
+    A = 0.3
+    phi = A * np.cos(kk * Y)                       # varies along axis 1 only
+    rng = np.random.default_rng(9)
+    pos = rng.uniform(-0.5, 0.5, size=(64, 3))
+    acc = oracle.cic_gather(phi, L, pos)
+    # node gradient of A cos(k y): -(phi[j+1]-phi[j-1])/(2dx) = A sin(k y_j) sin(k dx)/dx ; CIC = linear interp in y
+    u = (pos[:, 1] + L / 2) / dx
+    j0 = np.floor(u).astype(int); f = u - j0
+    y = -L / 2 + dx * np.arange(N + 1)
+    g = A * np.sin(kk * y) * np.sin(kk * dx) / dx
+    expect = (1 - f) * g[j0] + f * g[j0 + 1]
+    assert np.max(np.abs(acc[:, 1] - expect)) < 1e-13
+    assert np.max(np.abs(acc[:, 0])) < 1e-13 and np.max(np.abs(acc[:, 2])) < 1e-13
+
+
+def test_particle_leapfrog_free_streaming_and_wrap():
+    """G = 0: particles stream freely, x(t) = x0 + v t wrapped into [-L/2, L/2)."""
+    N, L = 8, 1.0
+    o = oracle.Oracle(N, L, 1.0, 0.0)
+    o.set_psi(np.ones((N, N, N), complex))
+    pos = np.array([[0.49, -0.49, 0.0]]); vel = np.array([[1.0, -2.0, 0.5]])
+    o.set_particles(pos, vel, 1.0)
+    o.step(10, 0.01)
+    p, v = o.particles()
+    assert np.allclose(p, [[0.59 - 1.0, -0.69 + 1.0, 0.05]], atol=1e-14)
+    assert np.allclose(v, vel)
+
+
+def test_kick_sign_and_half_step():
+    """Drift-free limit: for a k=0 wave function in a *given* potential the KDK step is a pure phase
+    exp(-i Phi dt/mu).  Use particles to impose Phi without touching |psi| (uniform)."""
+    N, L, mu, G = 8, 1.0, 2.0, 1.0
+    o = oracle.Oracle(N, L, mu, G)
+    o.set_psi(np.full((N, N, N), 1e-9, complex))        # negligible self-gravity, uniform
+    pos = np.array([[0.0, 0.0, 0.0]])
+    o.set_particles(pos, np.zeros((1, 3)), 3.0)          # static source (zero self force keeps it put)
+    phi = o.potential()
+    dt = 1e-4                                            # drift of a non-uniform phase is O(dt^2) here
+    o.step(1, dt)
+    ratio = o.psi() / 1e-9
+    assert relerr(ratio, np.exp(-1j * phi * dt / mu)) < 1e-5
+    assert np.max(np.abs(phi)) * dt / mu > 1e-3          # the phase is resolvable
+    assert phi[4, 4, 4] == phi.min() < 0                 # attractive well at the particle
