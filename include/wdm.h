@@ -1,0 +1,110 @@
+/*
+ * wdm.h -- C ABI of libwdm.so: the B200 (sm_100a) split-step Schroedinger-Poisson + CIC particle step.
+ *
+ * One context = one periodic N^3 box.  Every call returns a WDM_* code; no exception crosses the
+ * boundary.  Pointers named *_dev are DEVICE pointers (e.g. torch.Tensor.data_ptr()), pointers named
+ * *_host are HOST pointers (pinned memory makes the copies asynchronous).  The caller owns every
+ * buffer it passes; the library copies in/out on the context's stream and owns only its internal
+ * state.  PAPER.md below is the paper text (arxiv/paper_2606_25026); G<n> are the readings listed in
+ * DESIGN.md.
+ *
+ * Layout: grid arrays have shape (N, N, N) in C order, index (ix, iy, iz) <-> grid point
+ * x = -L/2 + ix*dx etc. with dx = L/N (Eq. 20; reading G1), iz contiguous.
+ * Complex values are interleaved (re, im).  For dtype WDM_C64 complex = 2 x float32 and every real
+ * array / particle array is float32; for WDM_C128 complex = 2 x float64 and reals are float64 (G23).
+ * Particle pos/vel are (n, 3) C order, columns x, y, z.
+ */
+#ifndef WDM_H
+#define WDM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wdm_ctx wdm_ctx; /* opaque, owned by the library */
+
+enum { WDM_C64 = 0, WDM_C128 = 1 };
+enum {
+    WDM_OK = 0,
+    WDM_EINVAL = 1,       /* null pointer, L <= 0, hbar_over_m <= 0, G < 0, n < 0, nsteps < 0, bad dtype */
+    WDM_EUNSUPPORTED = 2, /* N not a power of two or outside [8, 1024] (powers of two)  */
+    WDM_ENOMEM = 3,       /* device allocation failed / caller workspace too small                     */
+    WDM_ECUDA = 4,        /* a CUDA call failed; text in wdm_last_error                                */
+    WDM_ESTATE = 5        /* wdm_step / wdm_get_* before wdm_set_psi                                   */
+};
+
+/* Bytes of device workspace a context needs (psi, Phi, the Poisson half-spectrum, tables and, if
+ * max_particles > 0, the particle mesh and particle arrays).  Lets the caller take ALL device memory
+ * from its own allocator (PyTorch) and hand it to wdm_create_ws. */
+int wdm_workspace_bytes(int N, int dtype, long long max_particles, size_t *bytes_out);
+
+/* Create a context for the SPE  i psi_t = -(mu/2) lap psi + (1/mu) Phi psi,  lap Phi = 4 pi G rho,
+ * rho = |psi|^2 + particles, mu = hbar_over_m (Eq. 1-2 PAPER.md:47-58 with |psi|^2 the mass density,
+ * G6; Eq. 9-10 PAPER.md:96-103 when mu = 1).  wdm_create allocates with cudaMalloc on the current
+ * device; wdm_create_ws carves everything out of caller memory (256-byte aligned, at least
+ * wdm_workspace_bytes; must outlive the context).  *out is NULL on failure. */
+int wdm_create(wdm_ctx **out, int N, double L, double hbar_over_m, double G, int dtype);
+int wdm_create_ws(wdm_ctx **out, int N, double L, double hbar_over_m, double G, int dtype,
+                  long long max_particles, void *workspace_dev, size_t workspace_bytes);
+int wdm_destroy(wdm_ctx *ctx);
+
+/* All later work of this context is enqueued on `cuda_stream` (a cudaStream_t, e.g.
+ * torch.cuda.current_stream().cuda_stream; NULL = the legacy default stream). */
+int wdm_set_stream(wdm_ctx *ctx, void *cuda_stream);
+
+/* Copy in the wave function, N^3 interleaved complex of the context dtype.  Marks Phi stale (G8). */
+int wdm_set_psi(wdm_ctx *ctx, const void *psi_dev);
+int wdm_set_psi_host(wdm_ctx *ctx, const void *psi_host);
+
+/* Copy in n particles (n = 0 removes them).  Positions are wrapped into [-L/2, L/2) (G16).
+ * mass_dev: n reals, or NULL for the equal mass `mass_scalar`.  Particle mass enters the Poisson
+ * source through a cloud-in-cell deposit and particles feel the CIC-interpolated central-difference
+ * gradient of the shared potential (Eq. 21; G11-G13).  A context made
+ * by wdm_create_ws accepts at most its max_particles. */
+int wdm_set_particles(wdm_ctx *ctx, long long n, const void *pos_dev, const void *vel_dev,
+                      const void *mass_dev, double mass_scalar);
+int wdm_set_particles_host(wdm_ctx *ctx, long long n, const void *pos_host, const void *vel_host,
+                           const void *mass_host, double mass_scalar);
+
+/* Advance nsteps kick-drift-kick steps of size dt (Eq. 17-18; Alg. 1 l.5-16
+ * PAPER.md:247-267; particles: leapfrog KDK sharing dt, G14-G15).  nsteps >= 0; dt may be negative
+ * (time reversal).  If Phi is stale it is first recomputed from the current (psi, x); nsteps = 0 does
+ * only that.  On return (stream-ordered) psi, x, v are at the same time level and Phi / rho are the
+ * ones consistent with them.  Asynchronous: no host synchronisation. */
+int wdm_step(wdm_ctx *ctx, int nsteps, double dt);
+
+/* Whole user call with HOST buffers: copy psi in, wdm_step(nsteps, dt), copy psi out, synchronise. */
+int wdm_run_host(wdm_ctx *ctx, const void *psi_in_host, int nsteps, double dt, void *psi_out_host);
+
+/* Copy out (stream-ordered for *_dev; the *_host forms synchronise the stream before returning).
+ * density  : |psi|^2 + CIC particle mass density, the Poisson source before mean removal (G22)
+ * potential: zero-mean Phi (Eq. 23, k = 0 mode zeroed, G3)
+ * particles: pos (wrapped) and vel, either may be NULL; particles come back in the caller's order. */
+int wdm_get_psi(wdm_ctx *ctx, void *psi_out_dev);
+int wdm_get_density(wdm_ctx *ctx, void *rho_out_dev);
+int wdm_get_potential(wdm_ctx *ctx, void *phi_out_dev);
+int wdm_get_particles(wdm_ctx *ctx, void *pos_out_dev, void *vel_out_dev);
+int wdm_get_psi_host(wdm_ctx *ctx, void *psi_out_host);
+int wdm_get_density_host(wdm_ctx *ctx, void *rho_out_host);
+int wdm_get_potential_host(wdm_ctx *ctx, void *phi_out_host);
+int wdm_get_particles_host(wdm_ctx *ctx, void *pos_out_host, void *vel_out_host);
+
+/* Instrumentation.  wdm_launch_count: kernels launched by this context so far.  With profiling on,
+ * every kernel launch is bracketed by CUDA events on the context's stream;
+ * wdm_kernel_stats synchronises and returns, for slot i < *n_inout, the kernel name, the number of
+ * timed launches and their summed duration in ms, then resets the accumulators. */
+int wdm_launch_count(wdm_ctx *ctx, long long *count_out);
+int wdm_set_profiling(wdm_ctx *ctx, int on);
+int wdm_kernel_stats(wdm_ctx *ctx, int *n_inout, const char **names_out, long long *launches_out,
+                     double *ms_out);
+
+/* Text of the last error of this context (never NULL; valid until the next call on the context).
+ * wdm_last_error(NULL) reports the last failure of wdm_create*. */
+const char *wdm_last_error(const wdm_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WDM_H */

@@ -132,7 +132,11 @@ class Oracle:
             lib().wdmo_destroy(self._h)
             self._h = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
     def set_psi(self, psi):
         psi = _c128(psi)

@@ -1,0 +1,581 @@
+// wdm.cu -- host logic and C ABI of libwdm.so (see include/wdm.h for the contract).
+//
+// One wdm_step(nsteps, dt) enqueues, per step, on the context's stream:
+//   [particles: gather -grad Phi, kick, drift, wrap, deposit]            (wdm_particles.cu)
+//   psi sweep z  (kick on load: half kick at the first step, merged full kick afterwards; reading G21)
+//   psi sweep y
+//   psi sweep x + rho = |psi|^2 + rho_p + real-to-complex x-spectrum -> H
+//   H sweep y forward, H sweep z forward . Green . inverse, H sweep y inverse, x complex-to-real -> Phi
+// and once at the end the closing half kick.  Nothing synchronises with the host.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/wdm.h"
+#include "wdm_internal.hpp"
+#include "wdm_kernels.cuh"
+#include "wdm_particles.hpp"
+
+namespace wdm {
+
+#define X(n, ra, rb, rm, w, nt, minb) const SweepTable *sweep_table_0_##n();
+WDM_FACT_C64(X)
+#undef X
+#define X(n, ra, rb, rm, w, nt, minb) const SweepTable *sweep_table_1_##n();
+WDM_FACT_C128(X)
+#undef X
+
+const SweepTable *sweep_table(int dtype, int N)
+{
+#define X(n, ra, rb, rm, w, nt, minb) if (dtype == 0 && N == n) return sweep_table_0_##n();
+    WDM_FACT_C64(X)
+#undef X
+#define X(n, ra, rb, rm, w, nt, minb) if (dtype == 1 && N == n) return sweep_table_1_##n();
+    WDM_FACT_C128(X)
+#undef X
+    return nullptr;
+}
+
+// ---------------------------------------------------------------- elementwise kernels (not on the per-step path)
+
+template <typename T>
+__global__ void k_kick(cx<T> *psi, const T *phi, T coef, size_t n)
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        stv(psi + i, rotate_neg(ldv(psi + i), ldg(phi + i) * coef));
+}
+
+template <typename T>
+__global__ void k_density(const cx<T> *psi, const T *rho_p, T *out, size_t n)
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        cx<T> v = ldv(psi + i);
+        T r = v.x * v.x + v.y * v.y;
+        if (rho_p) r += rho_p[i];
+        out[i] = r;
+    }
+}
+
+enum Slot { S_PSI_Z, S_PSI_Y, S_PSI_X_RHO, S_H_Y_FWD, S_H_Z_GREEN, S_H_Y_INV, S_C2R, S_KICK, S_PART_PUSH,
+            S_PART_DEPOSIT, S_PART_SORT, S_MISC, S_COUNT };
+static const char *kSlotNames[S_COUNT] = {"psi_sweep_z_kick", "psi_sweep_y", "psi_sweep_x_rho_r2c", "poisson_y_fwd",
+                                          "poisson_z_green", "poisson_y_inv", "poisson_x_c2r", "kick_elementwise",
+                                          "particle_gather_kick_drift", "particle_cic_deposit", "particle_cell_sort",
+                                          "misc"};
+
+}  // namespace wdm
+
+using namespace wdm;
+
+struct wdm_ctx {
+    int N = 0, dtype = 0;
+    double L = 0, mu = 0, G = 0;
+    size_t n = 0, nH = 0;
+    const SweepTable *tab = nullptr;
+    cudaStream_t stream = nullptr;
+    // memory
+    bool owns = true;
+    unsigned char *ws = nullptr;
+    size_t ws_bytes = 0, ws_used = 0;
+    std::vector<void *> owned;
+    void *psi = nullptr, *phi = nullptr, *H = nullptr;
+    void *twA = nullptr, *twB = nullptr, *phase = nullptr, *ksq_pos = nullptr, *ksq_nat = nullptr;
+    unsigned short *pos_of_k = nullptr;
+    double phase_dt = 0;
+    bool phase_valid = false, have_psi = false, stale = true;
+    ParticleState part;
+    long long max_particles = -1;   // -1: unbounded (cudaMalloc on demand)
+    // instrumentation
+    long long launches = 0;
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev;    // pairs
+    std::vector<int> ev_slot;
+    size_t ev_used = 0;
+    double slot_ms[S_COUNT] = {0};
+    long long slot_n[S_COUNT] = {0};
+    std::string err;
+};
+
+static std::string g_create_err = "";
+
+static int fail(wdm_ctx *c, int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (c) c->err = buf;
+    else g_create_err = buf;
+    return code;
+}
+
+#define CU(c, call)                                                                                     \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess) return fail(c, WDM_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));     \
+    } while (0)
+
+static size_t csize(int dtype) { return dtype == WDM_C64 ? 8 : 16; }
+static size_t rsize(int dtype) { return dtype == WDM_C64 ? 4 : 8; }
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static size_t grid_bytes(int N, int dtype, long long max_particles)
+{
+    size_t n = (size_t)N * N * N, nH = (size_t)(N / 2 + 1) * N * N, c = csize(dtype), r = rsize(dtype);
+    size_t b = align_up(n * c) + align_up(n * r) + align_up(nH * c);
+    b += 3 * align_up((size_t)N * c) + 2 * align_up((size_t)N * r) + align_up((size_t)N * 2);
+    if (max_particles > 0) b += align_up(n * r) + particle_bytes(N, dtype, max_particles);
+    return b + 4096;
+}
+
+static int ctx_alloc(wdm_ctx *c, void **out, size_t bytes)
+{
+    bytes = align_up(bytes ? bytes : 1);
+    if (c->owns) {
+        void *p = nullptr;
+        cudaError_t e = cudaMalloc(&p, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(c, WDM_ENOMEM, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)); }
+        c->owned.push_back(p);
+        *out = p;
+    } else {
+        if (c->ws_used + bytes > c->ws_bytes) return fail(c, WDM_ENOMEM, "workspace too small: need %zu more bytes", c->ws_used + bytes - c->ws_bytes);
+        *out = c->ws + c->ws_used;
+        c->ws_used += bytes;
+    }
+    return WDM_OK;
+}
+
+// ---------------------------------------------------------------- instrumentation
+
+static int prof_flush(wdm_ctx *c)
+{
+    if (c->ev_used == 0) return WDM_OK;
+    CU(c, cudaStreamSynchronize(c->stream));
+    for (size_t i = 0; i < c->ev_used; ++i) {
+        float ms = 0;
+        CU(c, cudaEventElapsedTime(&ms, c->ev[2 * i], c->ev[2 * i + 1]));
+        c->slot_ms[c->ev_slot[i]] += ms;
+        c->slot_n[c->ev_slot[i]] += 1;
+    }
+    c->ev_used = 0;
+    return WDM_OK;
+}
+
+struct Timed {
+    wdm_ctx *c;
+    int slot;
+    bool on;
+    size_t idx = 0;
+    Timed(wdm_ctx *c_, int slot_) : c(c_), slot(slot_), on(c_->profiling)
+    {
+        c->launches++;
+        if (!on) return;
+        if (c->ev_used * 2 >= c->ev.size()) {
+            if (c->ev.size() >= 2 * 8192) { prof_flush(c); }
+            else {
+                cudaEvent_t a, b;
+                cudaEventCreate(&a); cudaEventCreate(&b);
+                c->ev.push_back(a); c->ev.push_back(b); c->ev_slot.push_back(0);
+            }
+        }
+        idx = c->ev_used++;
+        c->ev_slot[idx] = slot;
+        cudaEventRecord(c->ev[2 * idx], c->stream);
+    }
+    ~Timed() { if (on) cudaEventRecord(c->ev[2 * idx + 1], c->stream); }
+};
+
+// ---------------------------------------------------------------- tables
+
+template <typename T>
+static int upload_tables(wdm_ctx *c)
+{
+    Tables<T> t = build_tables<T>(c->tab->fact, c->L);
+    CU(c, cudaMemcpyAsync(c->twA, t.twA.data(), t.twA.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->twB, t.twB.data(), t.twB.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->ksq_pos, t.ksq_pos.data(), t.ksq_pos.size() * sizeof(T), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->ksq_nat, t.ksq_nat.data(), t.ksq_nat.size() * sizeof(T), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->pos_of_k, t.pos_of_k.data(), t.pos_of_k.size() * 2, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));   // host vectors die here
+    return WDM_OK;
+}
+
+template <typename T>
+static int ensure_phase(wdm_ctx *c, double dt)
+{
+    if (c->phase_valid && c->phase_dt == dt) return WDM_OK;
+    std::vector<cx<T>> ph = build_phase<T>(c->tab->fact, c->L, c->mu, dt);
+    CU(c, cudaMemcpyAsync(c->phase, ph.data(), ph.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    c->phase_dt = dt;
+    c->phase_valid = true;
+    return WDM_OK;
+}
+
+template <typename T>
+static SweepParams<T> base_params(wdm_ctx *c)
+{
+    SweepParams<T> p{};
+    const int N = c->N;
+    p.twA = (const cx<T> *)c->twA;
+    p.twB = (const cx<T> *)c->twB;
+    p.phase = (const cx<T> *)c->phase;
+    p.pos_of_k = c->pos_of_k;
+    p.ksq_pos = (const T *)c->ksq_pos;
+    p.ksq_nat = (const T *)c->ksq_nat;
+    p.green = (T)(-4.0 * M_PI * c->G / ((double)N * N * N));
+    p.tilesInner = N / c->tab->fact.W;
+    p.H = (cx<T> *)c->H;
+    p.phi = (const T *)c->phi;
+    p.phi_out = (T *)c->phi;
+    p.rho_p = c->part.n > 0 ? (const T *)c->part.rho_p : nullptr;
+    return p;
+}
+
+// ---------------------------------------------------------------- the step
+
+// rho (from the current psi and particle mesh) -> Phi.  drift: also do the x-axis part of Eq. 18(b).
+template <typename T>
+static int density_poisson(wdm_ctx *c, bool drift)
+{
+    const long long N = c->N;
+    {
+        SweepParams<T> p = base_params<T>(c);
+        p.data = (cx<T> *)c->psi; p.rowStride = N * N; p.outerStride = N;
+        Timed t(c, S_PSI_X_RHO);
+        CU(c, c->tab->psi_x_rho(&p, drift ? 1 : 0, c->stream));
+    }
+    SweepParams<T> p = base_params<T>(c);
+    p.data = (cx<T> *)c->H; p.rowStride = N; p.outerStride = N * N;
+    { Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
+    { Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
+    { Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
+    p.rowStride = N * N; p.outerStride = N;
+    { Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, c->stream)); }
+    return WDM_OK;
+}
+
+template <typename T>
+static int particles_deposit(wdm_ctx *c)
+{
+    if (c->part.n == 0) return WDM_OK;
+    { Timed t(c, S_MISC); CU(c, cudaMemsetAsync(c->part.rho_p, 0, c->n * sizeof(T), c->stream)); }
+    Timed t(c, S_PART_DEPOSIT);
+    CU(c, particle_deposit(c->part, c->N, c->L, c->dtype, c->stream));
+    return WDM_OK;
+}
+
+template <typename T>
+static int refresh(wdm_ctx *c)
+{
+    if (!c->have_psi) return fail(c, WDM_ESTATE, "wdm_set_psi has not been called");
+    if (!c->stale) return WDM_OK;
+    if (c->G > 0) {
+        int rc = particles_deposit<T>(c);
+        if (rc) return rc;
+        rc = density_poisson<T>(c, false);
+        if (rc) return rc;
+    } else {
+        Timed t(c, S_MISC);
+        CU(c, cudaMemsetAsync(c->phi, 0, c->n * sizeof(T), c->stream));
+    }
+    c->stale = false;
+    return WDM_OK;
+}
+
+template <typename T>
+static int step_impl(wdm_ctx *c, int nsteps, double dt)
+{
+    int rc = refresh<T>(c);
+    if (rc || nsteps == 0) return rc;
+    rc = ensure_phase<T>(c, dt);
+    if (rc) return rc;
+    const long long N = c->N;
+    const bool grav = c->G > 0;
+    for (int s = 0; s < nsteps; ++s) {
+        const double kdt = (s == 0 ? 0.5 : 1.0) * dt;     // merged closing + opening half kicks (G21)
+        if (c->part.n > 0) {
+            // v += a(Phi^n, x^n) kdt ; x += v dt ; wrap ; then deposit x^{n+1}  (readings G14-G16)
+            { Timed t(c, S_PART_PUSH); CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, grav ? kdt : 0.0, dt, c->stream)); }
+            if (grav) { rc = particles_deposit<T>(c); if (rc) return rc; }
+        }
+        {
+            SweepParams<T> p = base_params<T>(c);
+            p.data = (cx<T> *)c->psi;
+            p.kick = (T)(kdt / c->mu);
+            Timed t(c, S_PSI_Z);
+            CU(c, c->tab->psi_z(&p, grav ? 1 : 0, c->stream));
+        }
+        {
+            SweepParams<T> p = base_params<T>(c);
+            p.data = (cx<T> *)c->psi; p.rowStride = N; p.outerStride = N * N;
+            Timed t(c, S_PSI_Y);
+            CU(c, c->tab->psi_strided(&p, c->stream));
+        }
+        if (grav) {
+            rc = density_poisson<T>(c, true);
+            if (rc) return rc;
+        } else {
+            SweepParams<T> p = base_params<T>(c);
+            p.data = (cx<T> *)c->psi; p.rowStride = N * N; p.outerStride = N;
+            Timed t(c, S_PSI_Y);
+            CU(c, c->tab->psi_strided(&p, c->stream));
+        }
+    }
+    if (grav) {
+        {
+            Timed t(c, S_KICK);
+            k_kick<T><<<148 * 8, 256, 0, c->stream>>>((cx<T> *)c->psi, (const T *)c->phi, (T)(0.5 * dt / c->mu), c->n);
+            CU(c, cudaGetLastError());
+        }
+        if (c->part.n > 0) {
+            Timed t(c, S_PART_PUSH);
+            CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, 0.5 * dt, 0.0, c->stream));
+        }
+    }
+    return WDM_OK;
+}
+
+// ---------------------------------------------------------------- C ABI
+
+static int check_args(int N, double L, double mu, double G, int dtype)
+{
+    if (!(L > 0) || !(mu > 0) || !(G >= 0)) return fail(nullptr, WDM_EINVAL, "need L > 0, hbar_over_m > 0, G >= 0");
+    if (dtype != WDM_C64 && dtype != WDM_C128) return fail(nullptr, WDM_EINVAL, "dtype must be WDM_C64 or WDM_C128");
+    if (N < 8 || N > 1024 || (N & (N - 1))) return fail(nullptr, WDM_EUNSUPPORTED, "N must be a power of two in [8, 1024], got %d", N);
+    return WDM_OK;
+}
+
+extern "C" int wdm_workspace_bytes(int N, int dtype, long long max_particles, size_t *bytes_out)
+{
+    if (!bytes_out || max_particles < 0) return fail(nullptr, WDM_EINVAL, "null output or negative max_particles");
+    int rc = check_args(N, 1.0, 1.0, 0.0, dtype);
+    if (rc) return rc;
+    *bytes_out = grid_bytes(N, dtype, max_particles);
+    return WDM_OK;
+}
+
+static int create_common(wdm_ctx **out, int N, double L, double mu, double G, int dtype, long long max_particles,
+                         void *ws, size_t ws_bytes, bool owns)
+{
+    if (!out) return fail(nullptr, WDM_EINVAL, "null output pointer");
+    *out = nullptr;
+    int rc = check_args(N, L, mu, G, dtype);
+    if (rc) return rc;
+    wdm_ctx *c = new wdm_ctx();
+    c->N = N; c->dtype = dtype; c->L = L; c->mu = mu; c->G = G;
+    c->n = (size_t)N * N * N; c->nH = (size_t)(N / 2 + 1) * N * N;
+    c->owns = owns; c->ws = (unsigned char *)ws; c->ws_bytes = ws_bytes;
+    c->max_particles = owns ? -1 : max_particles;
+    c->tab = sweep_table(dtype, N);
+    auto bail = [&](int code) {
+        g_create_err = c->err;
+        for (void *p : c->owned) cudaFree(p);
+        delete c;
+        return code;
+    };
+    if (!c->tab) return bail(fail(c, WDM_EUNSUPPORTED, "no kernels built for N = %d", N));
+    if (!owns) {
+        size_t mis = (size_t)((uintptr_t)ws & 255);
+        if (!ws) return bail(fail(c, WDM_EINVAL, "null workspace"));
+        if (mis) { c->ws += 256 - mis; c->ws_bytes -= (256 - mis) < ws_bytes ? (256 - mis) : ws_bytes; }
+        if (ws_bytes < grid_bytes(N, dtype, max_particles)) return bail(fail(c, WDM_ENOMEM, "workspace of %zu bytes < required %zu", ws_bytes, grid_bytes(N, dtype, max_particles)));
+    }
+    cudaError_t e = c->tab->init();
+    if (e != cudaSuccess) return bail(fail(c, WDM_ECUDA, "kernel attribute setup: %s", cudaGetErrorString(e)));
+    size_t cs = csize(dtype), rs = rsize(dtype);
+    if ((rc = ctx_alloc(c, &c->psi, c->n * cs)) || (rc = ctx_alloc(c, &c->phi, c->n * rs)) ||
+        (rc = ctx_alloc(c, &c->H, c->nH * cs)) || (rc = ctx_alloc(c, &c->twA, N * cs)) ||
+        (rc = ctx_alloc(c, &c->twB, N * cs)) || (rc = ctx_alloc(c, &c->phase, N * cs)) ||
+        (rc = ctx_alloc(c, &c->ksq_pos, N * rs)) || (rc = ctx_alloc(c, &c->ksq_nat, N * rs)) ||
+        (rc = ctx_alloc(c, (void **)&c->pos_of_k, N * 2)))
+        return bail(rc);
+    rc = dtype == WDM_C64 ? upload_tables<float>(c) : upload_tables<double>(c);
+    if (rc) return bail(rc);
+    if (!owns && max_particles > 0) {
+        void *rho_p = nullptr, *pm = nullptr;
+        if ((rc = ctx_alloc(c, &rho_p, c->n * rs)) || (rc = ctx_alloc(c, &pm, particle_bytes(N, dtype, max_particles)))) return bail(rc);
+        particle_bind(c->part, N, dtype, max_particles, rho_p, pm);
+    }
+    *out = c;
+    return WDM_OK;
+}
+
+extern "C" int wdm_create(wdm_ctx **out, int N, double L, double hbar_over_m, double G, int dtype)
+{
+    return create_common(out, N, L, hbar_over_m, G, dtype, 0, nullptr, 0, true);
+}
+
+extern "C" int wdm_create_ws(wdm_ctx **out, int N, double L, double hbar_over_m, double G, int dtype,
+                             long long max_particles, void *workspace_dev, size_t workspace_bytes)
+{
+    if (max_particles < 0) return fail(nullptr, WDM_EINVAL, "negative max_particles");
+    return create_common(out, N, L, hbar_over_m, G, dtype, max_particles, workspace_dev, workspace_bytes, false);
+}
+
+extern "C" int wdm_destroy(wdm_ctx *c)
+{
+    if (!c) return WDM_OK;
+    cudaStreamSynchronize(c->stream);
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    for (void *p : c->owned) cudaFree(p);
+    delete c;
+    return WDM_OK;
+}
+
+extern "C" int wdm_set_stream(wdm_ctx *c, void *s)
+{
+    if (!c) return WDM_EINVAL;
+    int rc = prof_flush(c);
+    if (rc) return rc;
+    c->stream = (cudaStream_t)s;
+    return WDM_OK;
+}
+
+static int set_psi(wdm_ctx *c, const void *psi, cudaMemcpyKind kind)
+{
+    if (!c) return WDM_EINVAL;
+    if (!psi) return fail(c, WDM_EINVAL, "null psi");
+    CU(c, cudaMemcpyAsync(c->psi, psi, c->n * csize(c->dtype), kind, c->stream));
+    c->have_psi = true;
+    c->stale = true;
+    return WDM_OK;
+}
+extern "C" int wdm_set_psi(wdm_ctx *c, const void *p) { return set_psi(c, p, cudaMemcpyDeviceToDevice); }
+extern "C" int wdm_set_psi_host(wdm_ctx *c, const void *p) { return set_psi(c, p, cudaMemcpyHostToDevice); }
+
+static int set_particles(wdm_ctx *c, long long n, const void *pos, const void *vel, const void *mass, double ms,
+                         cudaMemcpyKind kind)
+{
+    if (!c) return WDM_EINVAL;
+    if (n < 0 || (n > 0 && (!pos || !vel))) return fail(c, WDM_EINVAL, "bad particle arguments");
+    if (c->max_particles >= 0 && n > c->max_particles) return fail(c, WDM_ENOMEM, "%lld particles > max_particles %lld of the workspace", n, c->max_particles);
+    if (c->owns && n > c->part.capacity) {
+        size_t rs = rsize(c->dtype);
+        void *rho_p = c->part.rho_p, *pm = nullptr;
+        int rc;
+        if (!rho_p && (rc = ctx_alloc(c, &rho_p, c->n * rs))) return rc;
+        if ((rc = ctx_alloc(c, &pm, particle_bytes(c->N, c->dtype, n)))) return rc;   // older pool stays until destroy
+        particle_bind(c->part, c->N, c->dtype, n, rho_p, pm);
+    }
+    c->launches += 3;
+    cudaError_t e = particle_set(c->part, c->N, c->L, c->dtype, n, pos, vel, mass, ms, kind == cudaMemcpyHostToDevice, c->stream);
+    if (e != cudaSuccess) return fail(c, WDM_ECUDA, "particle_set: %s", cudaGetErrorString(e));
+    c->stale = true;
+    return WDM_OK;
+}
+extern "C" int wdm_set_particles(wdm_ctx *c, long long n, const void *pos, const void *vel, const void *mass, double ms)
+{
+    return set_particles(c, n, pos, vel, mass, ms, cudaMemcpyDeviceToDevice);
+}
+extern "C" int wdm_set_particles_host(wdm_ctx *c, long long n, const void *pos, const void *vel, const void *mass, double ms)
+{
+    return set_particles(c, n, pos, vel, mass, ms, cudaMemcpyHostToDevice);
+}
+
+extern "C" int wdm_step(wdm_ctx *c, int nsteps, double dt)
+{
+    if (!c) return WDM_EINVAL;
+    if (nsteps < 0 || dt != dt) return fail(c, WDM_EINVAL, "nsteps must be >= 0 and dt finite");
+    return c->dtype == WDM_C64 ? step_impl<float>(c, nsteps, dt) : step_impl<double>(c, nsteps, dt);
+}
+
+static int do_refresh(wdm_ctx *c) { return c->dtype == WDM_C64 ? refresh<float>(c) : refresh<double>(c); }
+
+static int get_grid(wdm_ctx *c, void *out, int what, cudaMemcpyKind kind)
+{
+    if (!c) return WDM_EINVAL;
+    if (!out) return fail(c, WDM_EINVAL, "null output");
+    if (!c->have_psi) return fail(c, WDM_ESTATE, "wdm_set_psi has not been called");
+    if (what == 0) {
+        CU(c, cudaMemcpyAsync(out, c->psi, c->n * csize(c->dtype), kind, c->stream));
+    } else {
+        int rc = do_refresh(c);
+        if (rc) return rc;
+        if (what == 1) {
+            CU(c, cudaMemcpyAsync(out, c->phi, c->n * rsize(c->dtype), kind, c->stream));
+        } else {
+            // density is not kept (its spectrum is overwritten by the Poisson solve): recompute, via H as scratch
+            void *dst = kind == cudaMemcpyDeviceToDevice ? out : c->H;
+            const void *rp = c->part.n > 0 && c->G > 0 ? c->part.rho_p : nullptr;
+            if (rp == nullptr && c->part.n > 0) {   // G = 0 never deposits: do it now
+                int r2 = c->dtype == WDM_C64 ? particles_deposit<float>(c) : particles_deposit<double>(c);
+                if (r2) return r2;
+                rp = c->part.rho_p;
+            }
+            {
+                Timed t(c, S_MISC);
+                if (c->dtype == WDM_C64) k_density<float><<<148 * 8, 256, 0, c->stream>>>((const cx<float> *)c->psi, (const float *)rp, (float *)dst, c->n);
+                else k_density<double><<<148 * 8, 256, 0, c->stream>>>((const cx<double> *)c->psi, (const double *)rp, (double *)dst, c->n);
+                CU(c, cudaGetLastError());
+            }
+            if (dst != out) CU(c, cudaMemcpyAsync(out, dst, c->n * rsize(c->dtype), kind, c->stream));
+        }
+    }
+    if (kind == cudaMemcpyDeviceToHost) CU(c, cudaStreamSynchronize(c->stream));
+    return WDM_OK;
+}
+extern "C" int wdm_get_psi(wdm_ctx *c, void *o) { return get_grid(c, o, 0, cudaMemcpyDeviceToDevice); }
+extern "C" int wdm_get_potential(wdm_ctx *c, void *o) { return get_grid(c, o, 1, cudaMemcpyDeviceToDevice); }
+extern "C" int wdm_get_density(wdm_ctx *c, void *o) { return get_grid(c, o, 2, cudaMemcpyDeviceToDevice); }
+extern "C" int wdm_get_psi_host(wdm_ctx *c, void *o) { return get_grid(c, o, 0, cudaMemcpyDeviceToHost); }
+extern "C" int wdm_get_potential_host(wdm_ctx *c, void *o) { return get_grid(c, o, 1, cudaMemcpyDeviceToHost); }
+extern "C" int wdm_get_density_host(wdm_ctx *c, void *o) { return get_grid(c, o, 2, cudaMemcpyDeviceToHost); }
+
+static int get_particles(wdm_ctx *c, void *pos, void *vel, bool host)
+{
+    if (!c) return WDM_EINVAL;
+    if (c->part.n > 0) {
+        c->launches += 1;
+        cudaError_t e = particle_get(c->part, c->dtype, pos, vel, host, c->stream);
+        if (e != cudaSuccess) return fail(c, WDM_ECUDA, "particle_get: %s", cudaGetErrorString(e));
+    }
+    if (host) CU(c, cudaStreamSynchronize(c->stream));
+    return WDM_OK;
+}
+extern "C" int wdm_get_particles(wdm_ctx *c, void *pos, void *vel) { return get_particles(c, pos, vel, false); }
+extern "C" int wdm_get_particles_host(wdm_ctx *c, void *pos, void *vel) { return get_particles(c, pos, vel, true); }
+
+extern "C" int wdm_run_host(wdm_ctx *c, const void *psi_in, int nsteps, double dt, void *psi_out)
+{
+    int rc = wdm_set_psi_host(c, psi_in);
+    if (rc) return rc;
+    if ((rc = wdm_step(c, nsteps, dt))) return rc;
+    return wdm_get_psi_host(c, psi_out);
+}
+
+extern "C" int wdm_launch_count(wdm_ctx *c, long long *out)
+{
+    if (!c || !out) return WDM_EINVAL;
+    *out = c->launches;
+    return WDM_OK;
+}
+
+extern "C" int wdm_set_profiling(wdm_ctx *c, int on)
+{
+    if (!c) return WDM_EINVAL;
+    int rc = prof_flush(c);
+    c->profiling = on != 0;
+    return rc;
+}
+
+extern "C" int wdm_kernel_stats(wdm_ctx *c, int *n_inout, const char **names, long long *launches, double *ms)
+{
+    if (!c || !n_inout) return WDM_EINVAL;
+    int rc = prof_flush(c);
+    if (rc) return rc;
+    int cap = *n_inout;
+    *n_inout = S_COUNT;
+    for (int i = 0; i < S_COUNT && i < cap; ++i) {
+        if (names) names[i] = kSlotNames[i];
+        if (launches) launches[i] = c->slot_n[i];
+        if (ms) ms[i] = c->slot_ms[i];
+    }
+    for (int i = 0; i < S_COUNT; ++i) { c->slot_n[i] = 0; c->slot_ms[i] = 0; }
+    return WDM_OK;
+}
+
+extern "C" const char *wdm_last_error(const wdm_ctx *c) { return c ? c->err.c_str() : g_create_err.c_str(); }

@@ -1,0 +1,35 @@
+// wdm_particles.hpp -- N-body particles coupled through the shared potential:
+// cloud-in-cell deposit into the Poisson source, CIC gather of the central-difference gradient
+// (Eq. 21), kick-drift-kick leapfrog with the wave field's dt (readings G11-G16).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstddef>
+
+namespace wdm {
+
+struct ParticleState {
+    long long n = 0, capacity = 0;
+    void *rho_p = nullptr;                   // N^3 reals: particle mass density on the mesh
+    void *pos = nullptr, *vel = nullptr;     // (n,3) reals, kept sorted by mesh tile
+    void *pos2 = nullptr, *vel2 = nullptr;   // sort double buffers
+    void *mass = nullptr, *mass2 = nullptr;  // n reals (per-particle masses) -- unused when has_mass == false
+    int *orig = nullptr, *orig2 = nullptr;   // caller's index of each sorted particle
+    int *key = nullptr;                      // tile key per particle
+    int *bin = nullptr;                      // (ntiles + 1) counters / offsets, then a cursor copy
+    bool has_mass = false;
+    double mass_scalar = 0.0;
+    int steps_since_sort = 0;
+};
+
+size_t particle_bytes(int N, int dtype, long long capacity);
+void particle_bind(ParticleState &ps, int N, int dtype, long long capacity, void *rho_p, void *pool);
+cudaError_t particle_set(ParticleState &ps, int N, double L, int dtype, long long n, const void *pos, const void *vel,
+                         const void *mass, double mass_scalar, bool from_host, cudaStream_t s);
+// v += a(phi, x) * kick_dt ; x += v * drift_dt ; wrap into [-L/2, L/2)
+cudaError_t particle_push(ParticleState &ps, int N, double L, int dtype, const void *phi, double kick_dt,
+                          double drift_dt, cudaStream_t s);
+// rho_p += CIC(x) (the caller zeroes rho_p)
+cudaError_t particle_deposit(ParticleState &ps, int N, double L, int dtype, cudaStream_t s);
+cudaError_t particle_get(ParticleState &ps, int dtype, void *pos_out, void *vel_out, bool to_host, cudaStream_t s);
+
+}  // namespace wdm
