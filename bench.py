@@ -1,0 +1,295 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fused split-step Schroedinger-Poisson step on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload t512|cfg2|cfg3|cfg4|cfg5] [--impl reference]
+
+One "step" is one kick-drift-kick step of the whole hot path (all rows of SURVEY.md 8(a)).  The timed
+region is ONE wdm_step(K, dt) call (the user's call) bracketed by CUDA events on the context's stream,
+after W warm-up steps.  Default workload: T512 = 512^3 complex64 soliton + 65536-mode halo, the
+configuration BASELINE.json's north_star quotes its HBM-roofline target on (psi alone is 1.07 GB, 8x the
+126 MB L2, so no L2 flush is needed between steps).  Prints ONE JSON line (rank 0).
+
+Multi-GPU: the path does not shard: --gpus N runs N independent replicas, one process
+per GPU under torchrun, no data-path collective; value = all ranks' cells / max-over-ranks time.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import wdm_workloads as wl  # noqa: E402
+
+METRIC = "SPE grid cell-updates/sec per KDK step"
+UNIT = "cell-updates/s"
+
+# algorithmic HBM bytes per cell per launch of each kernel, in units of the complex size c (DESIGN.md
+# "Kernels": one read + one write of the field per axis sweep; reals are c/2)
+ALG_BYTES_PER_CELL_C = {
+    "psi_sweep_z_kick": 2.5, "psi_sweep_y": 2.0, "psi_sweep_x_rho_r2c": 2.5,
+    "poisson_y_fwd": 1.0, "poisson_z_green": 1.0, "poisson_y_inv": 1.0, "poisson_x_c2r": 1.0,
+}
+
+
+def make_workload(name: str):
+    if name == "t512":
+        return wl.t512()
+    if name == "cfg2":
+        return wl.config2()
+    if name == "cfg3":
+        return wl.config3()
+    if name == "cfg4":
+        return wl.config4()
+    if name == "cfg5":
+        return wl.config5()
+    if name.startswith("sample"):          # soliton + halo at a reduced grid (reference arm / cpu_baseline)
+        n = int(name[6:])
+        w = wl.config2(N=n, nmodes=4096 if n < 512 else 65536, name=f"sample{n}_c64_soliton_halo", seed=4)
+        w.dt = (w.L / n) ** 2 / 6.0
+        return w
+    raise SystemExit(f"unknown workload {name}")
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Polls SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._t = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+            nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+            nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def __enter__(self):
+        if self.nv:
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._t:
+            self._t.join()
+
+    def summary(self):
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_rate(sample_name: str, steps: int, warmup: int):
+    """cells/s of the CPU oracle on the named sample: `warmup` untimed then `steps` timed KDK steps."""
+    import oracle
+    w = make_workload(sample_name)
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    o.set_psi(w.psi)
+    if w.pos is not None:
+        o.set_particles(w.pos, w.vel, w.mass)
+    dt = w.dt if w.dt is not None else (w.L / w.N) ** 2 / 6.0
+    o.step(warmup, dt)                      # also pays the first potential refresh
+    t0 = time.perf_counter()
+    o.step(steps, dt)
+    el = time.perf_counter() - t0
+    return w, (w.N ** 3) * steps / el, el, oracle.threads()
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    n_ref = 256 if (args.steps + args.warmup) <= 12 else 128
+    w, rate, el, thr = oracle_rate(f"sample{n_ref}", args.steps, args.warmup)
+    sample = (f"float64 CPU oracle, soliton+halo workload at {n_ref}^3 instead of 512^3 "
+              f"({args.steps} timed KDK steps, {el:.1f} s)")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "t512_c64_soliton_halo", "sample": sample},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="t512")
+    ap.add_argument("--impl", default="wdm")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip e2e / per-kernel / particle legs (used under ncu)")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import paper_2606_25026_b200 as wdm   # raises if libwdm.so is missing: there is no fallback
+
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    K, W = args.steps, max(3, args.warmup)
+    w = make_workload(args.workload)
+    N = w.N
+    npart = 0 if w.pos is None else len(w.pos)
+    sim = wdm.Sim(N, w.L, w.hbar_over_m, w.G, w.dtype, max_particles=npart)
+    psi_host = torch.from_numpy(w.psi).pin_memory()
+    sim.set_psi(psi_host)
+    if npart:
+        sim.set_particles(w.pos, w.vel, w.mass)
+    dt = w.dt
+    if dt is None:                                     # CFL from the initial potential (reading G17)
+        sim.step(0, 0.0)
+        dt = wl.cfl_dt(w, float(sim.potential().abs().max()))
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- warm-up, then the timed region: ONE wdm_step(K, dt)
+    sim.step(W, dt)
+    barrier()
+    l0 = wdm.wdm_launch_count(sim.h)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        barrier()
+        e0.record(stream)
+        sim.step(K, dt)
+        e1.record(stream)
+        barrier()
+    ms = e0.elapsed_time(e1)
+    launches = wdm.wdm_launch_count(sim.h) - l0
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * (N ** 3) * K / (ms * 1e-3)
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if w.dtype == "c64" else "f64", "data": "synthetic",
+        "config": {"workload": w.name, "N": N, "grid_dtype": "complex64" if w.dtype == "c64" else "complex128",
+                   "particles": npart, "dt": dt, "timed_call": f"wdm_step({K}, dt)",
+                   "l2": "inputs larger than L2 (psi alone is %.2f GB vs 126 MB L2), no flush" % (N ** 3 * 8 / 1e9)
+                         if N >= 512 else "working set near/below L2: L2-resident, launch-bound regime",
+                   "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU"},
+        "gpu_launches": launches, "clocks": clk.summary(),
+    }
+    if npart:
+        out["particle_updates_per_s"] = world * npart * K / (ms * 1e-3)
+
+    if not args.no_extras:
+        csize = 8 if w.dtype == "c64" else 16
+        # ---- per-kernel CUDA-event timing on the context's stream (profiled pass, not the headline number)
+        wdm.wdm_set_profiling(sim.h, True)
+        kp = min(K, 20)
+        sim.step(kp, dt)
+        stats = wdm.wdm_kernel_stats(sim.h)
+        wdm.wdm_set_profiling(sim.h, False)
+        total_ms = sum(t for _, t in stats.values())
+        kern = {k: {"launches": c, "avg_ms": t / c, "share": t / total_ms} for k, (c, t) in stats.items() if c}
+        dom = max((k for k in kern if k in ALG_BYTES_PER_CELL_C), key=lambda k: kern[k]["launches"] * kern[k]["avg_ms"])
+        peak, how = peaks()
+        alg = ALG_BYTES_PER_CELL_C[dom] * csize * N ** 3
+        achieved = alg / (kern[dom]["avg_ms"] * 1e-3) / 1e9
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp):
+            traffic = json.load(open(tp)).get(w.name, {}).get(dom)
+        out["roofline"] = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                           "frac": achieved / peak, "traffic": traffic, "peak_source": how,
+                           "alg_bytes_per_launch": alg,
+                           "whole_step": {"alg_bytes_per_step": 11 * csize * N ** 3,
+                                          "achieved": 11 * csize * N ** 3 / (ms / K * 1e-3) / 1e9,
+                                          "frac": 11 * csize * N ** 3 / (ms / K * 1e-3) / 1e9 / peak,
+                                          "frac_of_nominal_8TBs": 11 * csize * N ** 3 / (ms / K * 1e-3) / 1e9 / 8000.0}}
+        out["kernels"] = kern
+
+        # ---- end to end through the C ABI with HOST buffers: copy in + K steps + copy out, wall clock
+        out_host = torch.empty_like(psi_host).pin_memory()
+        ke = K
+        barrier()
+        t0 = time.perf_counter()
+        wdm.wdm_run_host(sim.h, psi_host, ke, dt, out_host)     # synchronises before returning
+        el = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([el], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            el = float(t.item())
+        nbytes = psi_host.numel() * psi_host.element_size()
+        out["e2e"] = {"value": world * N ** 3 * ke / el, "unit": UNIT, "h2d_bytes_per_step": nbytes / ke,
+                      "d2h_bytes_per_step": nbytes / ke, "call": f"wdm_run_host(psi_in, {ke}, dt, psi_out)",
+                      "note": "state stays on the device between steps; one H2D of psi and one D2H per call"}
+
+        # ---- CPU oracle on the host cores, bounded sample (rank 0, N = 1 only)
+        if rank == 0 and world == 1 and not args.no_cpu_baseline:
+            n_ref = 256
+            ws, rate, el, thr = oracle_rate(f"sample{n_ref}", 8, 1)
+            out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": thr, "kind": "oracle",
+                                   "sample": f"float64 CPU oracle, soliton+halo at {n_ref}^3, 8 timed KDK steps ({el:.1f} s)"}
+    sim.close()
+    if rank == 0:
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -58,6 +58,34 @@ __global__ void k_density(const cx<T> *psi, const T *rho_p, T *out, size_t n)
     }
 }
 
+// <rho> = (sum |psi|^2)/N^3 + (sum m_p)/L^3, accumulated in double: acc[0] grid sum, acc[1] particle mass
+template <typename T>
+__global__ void k_sum_density(const cx<T> *psi, size_t n, double *acc)
+{
+    double s = 0;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        cx<T> v = ldv(psi + i);
+        s += (double)v.x * v.x + (double)v.y * v.y;
+    }
+    for (int d = 16; d; d >>= 1) s += __shfl_down_sync(0xffffffffu, s, d);
+    if ((threadIdx.x & 31) == 0) atomicAdd(acc, s);
+}
+
+template <typename T>
+__global__ void k_sum_mass(const T *mass, long long n, double *acc)
+{
+    double s = 0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) s += mass[i];
+    for (int d = 16; d; d >>= 1) s += __shfl_down_sync(0xffffffffu, s, d);
+    if ((threadIdx.x & 31) == 0) atomicAdd(acc + 1, s);
+}
+
+template <typename T>
+__global__ void k_finish_mean(const double *acc, double inv_cells, double extra_mass, double inv_volume, T *mean)
+{
+    *mean = (T)(acc[0] * inv_cells + (acc[1] + extra_mass) * inv_volume);
+}
+
 enum Slot { S_PSI_Z, S_PSI_Y, S_PSI_X_RHO, S_H_Y_FWD, S_H_Z_GREEN, S_H_Y_INV, S_C2R, S_KICK, S_PART_PUSH,
             S_PART_DEPOSIT, S_PART_SORT, S_MISC, S_COUNT };
 static const char *kSlotNames[S_COUNT] = {"psi_sweep_z_kick", "psi_sweep_y", "psi_sweep_x_rho_r2c", "poisson_y_fwd",
@@ -81,6 +109,7 @@ struct wdm_ctx {
     size_t ws_bytes = 0, ws_used = 0;
     std::vector<void *> owned;
     void *psi = nullptr, *phi = nullptr, *H = nullptr;
+    void *rho_mean = nullptr;   // [0..1] double accumulators, then the mean as T at byte offset 16
     void *twA = nullptr, *twB = nullptr, *phase = nullptr, *ksq_pos = nullptr, *ksq_nat = nullptr;
     unsigned short *pos_of_k = nullptr;
     double phase_dt = 0;
@@ -126,7 +155,7 @@ static size_t grid_bytes(int N, int dtype, long long max_particles)
 {
     size_t n = (size_t)N * N * N, nH = (size_t)(N / 2 + 1) * N * N, c = csize(dtype), r = rsize(dtype);
     size_t b = align_up(n * c) + align_up(n * r) + align_up(nH * c);
-    b += 3 * align_up((size_t)N * c) + 2 * align_up((size_t)N * r) + align_up((size_t)N * 2);
+    b += 3 * align_up((size_t)N * c) + 2 * align_up((size_t)N * r) + align_up((size_t)N * 2) + 256;
     if (max_particles > 0) b += align_up(n * r) + particle_bytes(N, dtype, max_particles);
     return b + 4096;
 }
@@ -232,6 +261,7 @@ static SweepParams<T> base_params(wdm_ctx *c)
     p.phi = (const T *)c->phi;
     p.phi_out = (T *)c->phi;
     p.rho_p = c->part.n > 0 ? (const T *)c->part.rho_p : nullptr;
+    p.rho_mean = (const T *)((const unsigned char *)c->rho_mean + 16);
     return p;
 }
 
@@ -274,6 +304,20 @@ static int refresh(wdm_ctx *c)
     if (!c->have_psi) return fail(c, WDM_ESTATE, "wdm_set_psi has not been called");
     if (!c->stale) return WDM_OK;
     if (c->G > 0) {
+        {   // <rho> of the current state (conserved afterwards): see the density sweep
+            double *acc = (double *)c->rho_mean;
+            Timed t(c, S_MISC);
+            CU(c, cudaMemsetAsync(acc, 0, 16, c->stream));
+            k_sum_density<T><<<148 * 4, 256, 0, c->stream>>>((const cx<T> *)c->psi, c->n, acc);
+            double extra = 0;
+            if (c->part.n > 0) {
+                if (c->part.has_mass) k_sum_mass<T><<<148, 256, 0, c->stream>>>((const T *)c->part.mass, c->part.n, acc);
+                else extra = c->part.mass_scalar * (double)c->part.n;
+            }
+            k_finish_mean<T><<<1, 1, 0, c->stream>>>(acc, 1.0 / (double)c->n, extra, 1.0 / (c->L * c->L * c->L),
+                                                      (T *)((unsigned char *)c->rho_mean + 16));
+            CU(c, cudaGetLastError());
+        }
         int rc = particles_deposit<T>(c);
         if (rc) return rc;
         rc = density_poisson<T>(c, false);
@@ -391,7 +435,7 @@ static int create_common(wdm_ctx **out, int N, double L, double mu, double G, in
         (rc = ctx_alloc(c, &c->H, c->nH * cs)) || (rc = ctx_alloc(c, &c->twA, N * cs)) ||
         (rc = ctx_alloc(c, &c->twB, N * cs)) || (rc = ctx_alloc(c, &c->phase, N * cs)) ||
         (rc = ctx_alloc(c, &c->ksq_pos, N * rs)) || (rc = ctx_alloc(c, &c->ksq_nat, N * rs)) ||
-        (rc = ctx_alloc(c, (void **)&c->pos_of_k, N * 2)))
+        (rc = ctx_alloc(c, (void **)&c->pos_of_k, N * 2)) || (rc = ctx_alloc(c, &c->rho_mean, 64)))
         return bail(rc);
     rc = dtype == WDM_C64 ? upload_tables<float>(c) : upload_tables<double>(c);
     if (rc) return bail(rc);

@@ -75,6 +75,7 @@ struct SweepParams {
     const T *phi;              // KICK: potential, same shape as psi
     T kick;                    // KICK: theta = phi * kick   (dt/(2 mu) or dt/mu)
     const T *rho_p;            // RHO: particle mesh density or nullptr
+    const T *rho_mean;         // RHO: device scalar <rho>, subtracted before the transform (Eq. 23)
     cx<T> *H;                  // RHO / C2R: half spectrum
     T *phi_out;                // C2R: potential out
     const unsigned short *pos_of_k;  // position holding frequency k after a forward transform
@@ -232,6 +233,10 @@ WDM_DEV void psi_sweep_body(const SweepParams<typename C::T> &p, int tid, int bi
         constexpr int WP = W / 2, RSP = W / 2;
         T *F = reinterpret_cast<T *>(smem_raw);
         if (DRIFT) WDM_SYNC();   // every thread has finished reading the psi tile
+        // rho - <rho> (Eq. 23).  <rho> is conserved, so it is measured once per refresh; the k = 0
+        // mode is zeroed in the Green's function anyway -- subtracting here only keeps the large mean out of
+        // the single-precision partial sums of the low-k modes.
+        const T mean = ldg(p.rho_mean);
         static_for<0, ITER>([&](auto it_) {
             constexpr int it = decltype(it_)::value;
             int b = tid + it * NT, q, l;
@@ -241,7 +246,7 @@ WDM_DEV void psi_sweep_body(const SweepParams<typename C::T> &p, int tid, int bi
                 int row = q + mA * r;
                 T v = rho[it][r];
                 if (p.rho_p) v += ldg(p.rho_p + tile.at(row, l));
-                F[row * W + l] = v;
+                F[row * W + l] = v - mean;
             });
         });
         WDM_SYNC();

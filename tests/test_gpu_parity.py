@@ -1,0 +1,301 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star; growth per SURVEY.md reading G18):
+  complex128: rel-L2(psi), rel-L2(Phi) <= 1e-12 per 10 steps
+  complex64 : <= 2e-5 per 10 steps;   particle positions <= 1e-5 L
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import wdm_workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL10 = {"c128": 1e-12, "c64": 2e-5}
+POS_TOL = 1e-5
+
+
+def tol(dtype, nsteps):
+    return TOL10[dtype] * max(1.0, nsteps / 10.0)
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.complex128 if np.iscomplexobj(a) else np.float64)
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(np.asarray(b).ravel()))
+
+
+@pytest.fixture(scope="module")
+def wdm():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2606_25026_b200 as w
+    w.lib()
+    return w
+
+
+def pair(wdm, w, max_particles=0):
+    sim = wdm.Sim(w.N, w.L, w.hbar_over_m, w.G, w.dtype, max_particles=max_particles)
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    sim.set_psi(w.psi)
+    o.set_psi(w.psi)
+    if w.pos is not None:
+        sim.set_particles(w.pos, w.vel, w.mass)
+        o.set_particles(w.pos, w.vel, w.mass)
+    return sim, o
+
+
+def check_fields(sim, o, dtype, nsteps, what=""):
+    t = tol(dtype, nsteps)
+    e_psi = rel(sim.psi().cpu().numpy(), o.psi())
+    e_phi = rel(sim.potential().cpu().numpy(), o.potential())
+    e_rho = rel(sim.density().cpu().numpy(), o.density())
+    assert e_psi <= t, f"{what} psi {e_psi} > {t}"
+    assert e_phi <= t, f"{what} Phi {e_phi} > {t}"
+    assert e_rho <= 2 * t, f"{what} rho {e_rho} > {2 * t}"
+    return e_psi, e_phi
+
+
+# ---------------------------------------------------------------- config 1: exactness, checked after every step
+
+def test_config1_c128_every_step(wdm):
+    w = wl.config1()
+    sim, o = pair(wdm, w)
+    check_fields(sim, o, "c128", 0, "initial")          # refresh only: Phi from the initial psi
+    for s in range(1, w.nsteps + 1):
+        sim.step(1, w.dt)
+        o.step(1, w.dt)
+        check_fields(sim, o, "c128", s, f"step {s}")
+    # the same 10 steps in ONE call (merged kicks inside wdm_step, reading G21)
+    sim2, _ = pair(wdm, w)
+    sim2.step(w.nsteps, w.dt)
+    assert rel(sim2.psi().cpu().numpy(), o.psi()) <= 1e-12
+
+
+# ---------------------------------------------------------------- every supported size, both precisions, several tiles
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("N", [8, 16, 32, 64, 128])
+def test_white_noise_all_modes(wdm, N, dtype):
+    """White noise excites every Fourier mode: any wrong twiddle, digit reversal, Hermitian pairing or
+    Green's-function index shows up at O(1)."""
+    psi0 = (0.3 * wl.random_field(N, dtype, N) + 1.5).astype(np.complex64 if dtype == "c64" else np.complex128)
+    w = wl.Workload(f"noise{N}", N, dtype, 3, L=1.3, hbar_over_m=0.8, G=30.0, psi=psi0)
+    w.dt = 0.2 * (w.L / N) ** 2
+    sim, o = pair(wdm, w)
+    sim.step(3, w.dt)
+    o.step(3, w.dt)
+    check_fields(sim, o, dtype, 3, f"N={N}")
+    sim.close()
+
+
+@pytest.mark.parametrize("dtype,N", [("c64", 256), ("c128", 256), ("c64", 512)])
+def test_large_sizes_two_steps(wdm, dtype, N):
+    psi0 = (0.3 * wl.random_field(N, dtype, 7) + 1.0).astype(np.complex64 if dtype == "c64" else np.complex128)
+    w = wl.Workload(f"noise{N}", N, dtype, 2, psi=psi0)
+    w.dt = (w.L / N) ** 2 / 6
+    sim, o = pair(wdm, w)
+    sim.step(2, w.dt)
+    o.step(2, w.dt)
+    check_fields(sim, o, dtype, 2, f"N={N}")
+    sim.close()
+
+
+def test_free_drift_G0_and_negative_dt(wdm):
+    N = 64
+    psi0 = wl.random_field(N, "c128", 3)
+    w = wl.Workload("free", N, "c128", 4, G=0.0, psi=psi0)
+    w.dt = 1e-4
+    sim, o = pair(wdm, w)
+    sim.step(4, w.dt)
+    o.step(4, w.dt)
+    assert rel(sim.psi().cpu().numpy(), o.psi()) < 1e-12
+    assert float(sim.potential().abs().max()) == 0.0
+    sim.step(4, -w.dt)                                   # exact reversal of the unitary drift
+    assert rel(sim.psi().cpu().numpy(), psi0) < 1e-12
+
+
+# ---------------------------------------------------------------- BASELINE configs 2, 3 (shortened by default) 
+
+def run_config(wdm, w, nsteps):
+    sim, o = pair(wdm, w, 0 if w.pos is None else len(w.pos))
+    dt = w.dt
+    if dt is None:
+        sim.step(0, 0.0)
+        phimax_gpu = float(sim.potential().abs().max())
+        phimax = float(np.abs(o.potential()).max())
+        assert abs(phimax_gpu - phimax) <= 1e-4 * phimax
+        dt = wl.cfl_dt(w, phimax)                        # both sides get the same dt
+    sim.step(nsteps, dt)
+    o.step(nsteps, dt)
+    return sim, o, dt
+
+
+def test_config2_128_c64_soliton_halo_20_steps(wdm):
+    w = wl.config2()
+    sim, o, _ = run_config(wdm, w, 20)
+    e = check_fields(sim, o, "c64", 20, "cfg2")
+    n0 = float(np.sum(np.abs(w.psi.astype(np.complex128)) ** 2))
+    n1 = float((sim.psi().abs().double() ** 2).sum())
+    assert abs(n1 / n0 - 1) < 1e-5                       # unitarity (P1) on the GPU path
+    sim.close()
+
+
+def test_config3_256_c64_merger_10_steps(wdm):
+    w = wl.config3()
+    sim, o, _ = run_config(wdm, w, 10)
+    check_fields(sim, o, "c64", 10, "cfg3")
+    sim.close()
+
+
+@pytest.mark.slow
+def test_config2_full_100_steps(wdm):
+    w = wl.config2()
+    sim, o, _ = run_config(wdm, w, w.nsteps)
+    check_fields(sim, o, "c64", w.nsteps, "cfg2 full")
+
+
+@pytest.mark.slow
+def test_config3_full_200_steps(wdm):
+    w = wl.config3()
+    sim, o, _ = run_config(wdm, w, w.nsteps)
+    check_fields(sim, o, "c64", w.nsteps, "cfg3 full")
+
+
+# ---------------------------------------------------------------- coupled particles
+
+def check_particles(sim, o, L, nsteps, dtype):
+    p, v = sim.particles()
+    po, vo = o.particles()
+    d = p.cpu().numpy().astype(np.float64) - po
+    d -= L * np.round(d / L)
+    ptol = POS_TOL * L if dtype == "c64" else 1e-12
+    assert np.abs(d).max() <= ptol, np.abs(d).max()
+    assert rel(v.cpu().numpy(), vo) <= (1e-4 if dtype == "c64" else 1e-11)
+    pn = p.cpu().numpy()
+    assert pn.min() >= -0.5 * L and pn.max() < 0.5 * L   # wrapped into [-L/2, L/2)
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_small_coupled_every_element(wdm, dtype):
+    w = wl.small_coupled(16, dtype=dtype)
+    sim, o = pair(wdm, w, len(w.pos))
+    check_fields(sim, o, dtype, 0, "initial coupled")
+    sim.step(5, w.dt)
+    o.step(5, w.dt)
+    check_fields(sim, o, dtype, 5, "coupled")
+    check_particles(sim, o, w.L, 5, dtype)
+    sim.close()
+
+
+def test_per_particle_masses_and_caller_order(wdm):
+    w = wl.small_coupled(32, n_particles=1000, dtype="c128")
+    rng = np.random.default_rng(5)
+    m = w.mass * rng.uniform(0.2, 3.0, size=len(w.pos))
+    sim = wdm.Sim(w.N, w.L, w.hbar_over_m, w.G, "c128", max_particles=len(w.pos))
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    sim.set_psi(w.psi); o.set_psi(w.psi)
+    sim.set_particles(w.pos, w.vel, m); o.set_particles(w.pos, w.vel, m)
+    p0, v0 = sim.particles()                              # sorted internally, returned in the caller's order
+    assert np.array_equal(p0.cpu().numpy(), w.pos) and np.array_equal(v0.cpu().numpy(), w.vel)
+    sim.step(4, w.dt); o.step(4, w.dt)
+    check_fields(sim, o, "c128", 4, "masses")
+    check_particles(sim, o, w.L, 4, "c128")
+
+
+def test_config5_coupled_disk_reduced(wdm):
+    """BASELINE config 5 at reduced size (128^3, 2^16 particles, 10 steps): thin-disc deposit contention,
+    cell sort, merged particle kicks."""
+    w = wl.config5(N=128, n_particles=1 << 16, nsteps=10)
+    sim, o, dt = run_config(wdm, w, 10)
+    check_fields(sim, o, "c64", 10, "cfg5")
+    check_particles(sim, o, w.L, 10, "c64")
+    # total mass on the mesh = DM mass + particle mass
+    tot = float(sim.density().double().sum()) * (w.L / w.N) ** 3
+    assert abs(tot - (w.meta["m_dm"] * 1.05)) < 1e-4 * tot
+    sim.close()
+
+
+@pytest.mark.slow
+def test_config5_full(wdm):
+    w = wl.config5()
+    sim, o, dt = run_config(wdm, w, w.nsteps)
+    check_fields(sim, o, "c64", w.nsteps, "cfg5 full")
+    check_particles(sim, o, w.L, w.nsteps, "c64")
+
+
+def test_resort_keeps_results(wdm):
+    """More pushes than the re-sort interval: sorting must not change what is computed."""
+    w = wl.small_coupled(16, dtype="c128", n_particles=300)
+    sim, o = pair(wdm, w, len(w.pos))
+    sim.step(70, w.dt); o.step(70, w.dt)
+    check_fields(sim, o, "c128", 70, "resort")
+    check_particles(sim, o, w.L, 70, "c128")
+
+
+# ---------------------------------------------------------------- state semantics and errors through the ABI
+
+def test_state_semantics_and_errors(wdm):
+    import torch
+    h = wdm.wdm_create(16, 1.0, 1.0, 1.0, wdm.WDM_C64)
+    buf = torch.empty((16, 16, 16), dtype=torch.complex64, device="cuda")
+    with pytest.raises(wdm.WdmError) as e:
+        wdm.wdm_step(h, 1, 0.1)
+    assert e.value.code == wdm.WDM_ESTATE
+    with pytest.raises(wdm.WdmError) as e:
+        wdm.wdm_get_psi(h, buf)
+    assert e.value.code == wdm.WDM_ESTATE
+    with pytest.raises(wdm.WdmError) as e:
+        wdm.wdm_set_psi(h, None)
+    assert e.value.code == wdm.WDM_EINVAL
+    psi = torch.randn((16, 16, 16), dtype=torch.complex64, device="cuda")
+    wdm.wdm_set_psi(h, psi)
+    with pytest.raises(wdm.WdmError) as e:
+        wdm.wdm_step(h, -1, 0.1)
+    assert e.value.code == wdm.WDM_EINVAL
+    wdm.wdm_step(h, 0, 0.0)                              # refresh only leaves psi untouched
+    wdm.wdm_get_psi(h, buf)
+    torch.cuda.synchronize()
+    assert torch.equal(buf, psi)
+    n0 = wdm.wdm_launch_count(h)
+    wdm.wdm_step(h, 2, 1e-4)
+    assert wdm.wdm_launch_count(h) - n0 == 2 * 7 + 1    # 7 sweeps per step + the closing half kick
+    wdm.wdm_destroy(h)
+
+
+def test_host_buffer_entry_points(wdm):
+    w = wl.config1()
+    h = wdm.wdm_create(w.N, w.L, w.hbar_over_m, w.G, wdm.WDM_C128)
+    out = np.empty_like(w.psi)
+    wdm.wdm_run_host(h, w.psi, 3, w.dt, out)
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G); o.set_psi(w.psi); o.step(3, w.dt)
+    assert rel(out, o.psi()) < 1e-12
+    phi = np.empty((w.N,) * 3); rho = np.empty((w.N,) * 3)
+    wdm.wdm_get_potential_host(h, phi); wdm.wdm_get_density_host(h, rho)
+    assert rel(phi, o.potential()) < 1e-12 and rel(rho, o.density()) < 1e-12
+    wdm.wdm_destroy(h)
+
+
+def test_t512_sampled_properties(wdm):
+    """Full bench size (512^3 complex64, the launch configuration bench.py times): unitarity, zero-mean Phi,
+    and Phi against the oracle's Poisson solve of the GPU's own density (the oracle needs ~6 GB / ~10 s)."""
+    import torch
+    N = 512
+    w = wl.Workload("t512_noise", N, "c64", 2)
+    g = torch.Generator(device="cuda"); g.manual_seed(26062500)
+    psi = (torch.randn((N, N, N, 2), generator=g, device="cuda", dtype=torch.float32) * 0.3)
+    psi[..., 0] += 1.0
+    psi = torch.view_as_complex(psi).contiguous()
+    sim = wdm.Sim(N, dtype="c64")
+    sim.set_psi(psi)
+    n0 = float((psi.abs().double() ** 2).sum())
+    sim.step(2, (1.0 / N) ** 2 / 6)
+    n1 = float((sim.psi().abs().double() ** 2).sum())
+    assert abs(n1 / n0 - 1) < 1e-5
+    phi = sim.potential()
+    assert abs(float(phi.double().mean())) < 1e-6 * float(phi.abs().max())
+    rho = sim.density().cpu().numpy().astype(np.float64)
+    ref = oracle.poisson(rho, 1.0, 1.0 / (4 * math.pi))
+    assert rel(phi.cpu().numpy(), ref) < 2e-5
+    sim.close()
