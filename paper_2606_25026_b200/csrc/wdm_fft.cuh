@@ -150,12 +150,11 @@ WDM_HD void dit_inv(cx<T> (&v)[R])
 // tw[s * m] = omega_M^{q s}  (tables are stored s-major so that lanes with consecutive q read
 // consecutive words).
 
-// DIF level: rows rowbase + m*r -> butterfly -> twiddle -> rows rowbase + m*s (natural digit order)
-template <int R, typename T, class LD, class ST>
-WDM_HD void fwd_level(int rowbase, int m, const cx<T> *tw, LD &&ld, ST &&st)
+// DIF level: rows rowbase + m*r -> butterfly -> twiddle -> rows rowbase + m*s (natural digit order).
+// The _regs form takes the R inputs already in registers (so the caller can issue all loads first).
+template <int R, typename T, class ST>
+WDM_HD void fwd_level_regs(cx<T> (&v)[R], int rowbase, int m, const cx<T> *tw, ST &&st)
 {
-    cx<T> v[R];
-    static_for<0, R>([&](auto r) { v[decltype(r)::value] = ld(rowbase + m * decltype(r)::value); });
     dif_fwd<R>(v);
     static_for<0, R>([&](auto s_) {
         constexpr int s = decltype(s_)::value;
@@ -163,6 +162,14 @@ WDM_HD void fwd_level(int rowbase, int m, const cx<T> *tw, LD &&ld, ST &&st)
         if constexpr (s > 0) y = cmul(y, tw[s * m]);
         st(rowbase + m * s, y);
     });
+}
+
+template <int R, typename T, class LD, class ST>
+WDM_HD void fwd_level(int rowbase, int m, const cx<T> *tw, LD &&ld, ST &&st)
+{
+    cx<T> v[R];
+    static_for<0, R>([&](auto r) { v[decltype(r)::value] = ld(rowbase + m * decltype(r)::value); });
+    fwd_level_regs<R, T>(v, rowbase, m, tw, st);
 }
 
 // adjoint of fwd_level; the _regs form leaves the R outputs (rows rowbase + m*r) in v

@@ -175,12 +175,18 @@ WDM_DEV void psi_sweep_body(const SweepParams<typename C::T> &p, int tid, int bi
     };
 
     if constexpr (DRIFT) {
-        // level A forward: global -> registers -> shared
+        // level A forward: global -> registers -> shared (all loads of a butterfly are issued before any use)
         for (int b = tid; b < mA * W; b += NT) {
             int q, l;
             split<AX, mA, W>(b, q, l);
-            fwd_level<RA, T>(q, mA, p.twA + q, [&](int row) { return load_psi(row, l); },
-                             [&](int row, cx<T> v) { S[row * RS + l] = v; });
+            cx<T> v[RA];
+            static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = ldv(psi + tile.at(q + mA * r, l)); });
+            if constexpr (KICK) {
+                T th[RA];
+                static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; th[r] = ldg(p.phi + tile.at(q + mA * r, l)); });
+                static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], th[r] * p.kick); });
+            }
+            fwd_level_regs<RA, T>(v, q, mA, p.twA + q, [&](int row, cx<T> y) { S[row * RS + l] = y; });
         }
         WDM_SYNC();
         smem_fwd_B<C, W, RS, T>(S, p.twB, tid);
@@ -356,17 +362,35 @@ WDM_DEV void c2r_body(const SweepParams<typename C::T> &p, int tid, int bid, uns
     constexpr int WP = W / 2, RSP = W / 2;
     cx<T> *Sp = reinterpret_cast<cx<T> *>(smem_raw);
     const Tile<C, AX_STRIDED> tile(p, bid);
-    // Z_k = A_k + i B_k,  Z_{N-k} = conj(A_k) + i conj(B_k)
-    for (int b = tid; b < (N / 2 + 1) * WP; b += NT) {
-        int l = b % WP, k = b / WP;
-        cx<T> A, B;
-        ld2(p.H + tile.at(k, 2 * l), A, B);
+    // Z_k = A_k + i B_k,  Z_{N-k} = conj(A_k) + i conj(B_k).  Loads are issued in unrolled batches.
+    auto place = [&](int k, int l, cx<T> A, cx<T> B) {
         int pk = ldg(p.pos_of_k + k);
         Sp[pk * RSP + l] = mk<T>(A.x - B.y, A.y + B.x);
         if (k > 0 && k < N / 2) {
             int pn = ldg(p.pos_of_k + (N - k));
             Sp[pn * RSP + l] = mk<T>(A.x + B.y, B.x - A.y);
         }
+    };
+    constexpr int ITEMS = (N / 2) * WP;              // rows k < N/2
+    constexpr int UN = ITEMS % (NT * 8) == 0 ? 8 : (ITEMS % (NT * 4) == 0 ? 4 : (ITEMS % (NT * 2) == 0 ? 2 : 1));
+    static_assert(ITEMS % NT == 0 || ITEMS < NT, "pack loop");
+    for (int b0 = tid; b0 < ITEMS; b0 += NT * UN) {
+        cx<T> A[UN], B[UN];
+        static_for<0, UN>([&](auto u_) {
+            constexpr int u = decltype(u_)::value;
+            int b = b0 + u * NT;
+            if (ITEMS >= NT || b < ITEMS) ld2(p.H + tile.at(b / WP, 2 * (b % WP)), A[u], B[u]);
+        });
+        static_for<0, UN>([&](auto u_) {
+            constexpr int u = decltype(u_)::value;
+            int b = b0 + u * NT;
+            if (ITEMS >= NT || b < ITEMS) place(b / WP, b % WP, A[u], B[u]);
+        });
+    }
+    if (tid < WP) {
+        cx<T> A, B;
+        ld2(p.H + tile.at(N / 2, 2 * tid), A, B);
+        place(N / 2, tid, A, B);
     }
     WDM_SYNC();
     for (int b = tid; b < (N / RM) * WP; b += NT) {
