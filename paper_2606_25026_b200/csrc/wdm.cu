@@ -20,19 +20,19 @@
 
 namespace wdm {
 
-#define X(n, ra, rb, rm, w, nt, minb) const SweepTable *sweep_table_0_##n();
+#define X(n, ra, rb, rm, w, nt, ng, minb) const SweepTable *sweep_table_0_##n();
 WDM_FACT_C64(X)
 #undef X
-#define X(n, ra, rb, rm, w, nt, minb) const SweepTable *sweep_table_1_##n();
+#define X(n, ra, rb, rm, w, nt, ng, minb) const SweepTable *sweep_table_1_##n();
 WDM_FACT_C128(X)
 #undef X
 
 const SweepTable *sweep_table(int dtype, int N)
 {
-#define X(n, ra, rb, rm, w, nt, minb) if (dtype == 0 && N == n) return sweep_table_0_##n();
+#define X(n, ra, rb, rm, w, nt, ng, minb) if (dtype == 0 && N == n) return sweep_table_0_##n();
     WDM_FACT_C64(X)
 #undef X
-#define X(n, ra, rb, rm, w, nt, minb) if (dtype == 1 && N == n) return sweep_table_1_##n();
+#define X(n, ra, rb, rm, w, nt, ng, minb) if (dtype == 1 && N == n) return sweep_table_1_##n();
     WDM_FACT_C128(X)
 #undef X
     return nullptr;

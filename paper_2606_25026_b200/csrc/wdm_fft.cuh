@@ -228,11 +228,12 @@ WDM_HD void mid_inv(int rowbase, LD &&ld, ST &&st)
 
 // ---------------------------------------------------------------- factorisation of a line
 
-// N = RA * RB * RM (RB = 1: two levels).  W lines per tile, NT threads per CTA.
-template <typename T_, int N_, int RA_, int RB_, int RM_, int W_, int NT_, int MINB_>
+// N = RA * RB * RM (RB = 1: two levels).  W lines per tile, NT threads per compute group, NG groups per CTA
+// (NG + 1 tile buffers), MINB resident CTAs per SM.
+template <typename T_, int N_, int RA_, int RB_, int RM_, int W_, int NT_, int NG_, int MINB_>
 struct LineCfg {
     using T = T_;
-    static constexpr int N = N_, RA = RA_, RB = RB_, RM = RM_, W = W_, NT = NT_, MINB = MINB_;
+    static constexpr int N = N_, RA = RA_, RB = RB_, RM = RM_, W = W_, NT = NT_, NG = NG_, MINB = MINB_;
     static constexpr int mA = N / RA;          // level A: block N, stride mA
     static constexpr int MB = N / RA;          // level B: block MB, stride mB
     static constexpr int mB = MB / RB;

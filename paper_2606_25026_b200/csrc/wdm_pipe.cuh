@@ -1,0 +1,478 @@
+// wdm_pipe.cuh -- persistent, software-pipelined form of the axis sweeps (sm_100a).
+//
+// One CTA per SM walks tiles t = blockIdx.x, blockIdx.x + gridDim.x, ...  The CTA is NG "compute groups" of
+// C::NT threads; tile j of the CTA is transformed by group j % NG inside shared-memory buffer j % (NG+1).
+// A tile is brought in by asynchronous copies (cp.async / LDGSTS -- no registers, no issue slots while in
+// flight) that signal an mbarrier, and the group that has just finished reading a buffer immediately
+// refills it with the tile NG+1 positions ahead, so every load has more than one whole tile-compute time of
+// lead and HBM latency never reaches the math.  Results leave through plain (fire-and-forget) global stores.
+//
+//   full[b]  mbarrier, count = C::NT: every thread of the issuing group attaches its copies with
+//            cp.async.mbarrier.arrive.noinc; the consuming group waits on the phase parity (j / NBUF) & 1.
+//   group barrier: bar.sync (1 + group), C::NT -- the other group is never stalled by it.
+#pragma once
+
+#include "wdm_kernels.cuh"
+
+namespace wdm {
+
+// ---------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, int parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WDM_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WDM_DONE;\n"
+        "bra WDM_WAIT;\n"
+        "WDM_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void cp_async_arrive(uint64_t *bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void *dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void *dst, const void *src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_elem(cx<float> *dst, const cx<float> *src) { cp_async8(dst, src); }
+__device__ __forceinline__ void cp_async_elem(cx<double> *dst, const cx<double> *src) { cp_async16(dst, src); }
+__device__ __forceinline__ void group_sync(int group, int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "r"(nthreads) : "memory");
+}
+
+// ---------------------------------------------------------------- the pipeline driver
+// K provides:  using C;  TILE_BYTES;  AUX;  struct Pre;  issue(p, tile, buf, gt);  prefetch(p, tile, gt, pre);
+//              compute(p, tabs, tile, next_tile, buf, gt, grp, pre)
+
+// Lookup tables of the sweep.  A persistent CTA copies them into shared memory ONCE (they are read by every
+// butterfly of every tile: from global memory each read is an L1 round trip on the long scoreboard).
+template <typename T>
+struct Tabs {
+    const cx<T> *twA, *twB, *phase;
+    const T *ksq_pos;
+};
+enum { AUX_NONE = 0, AUX_PHASE = 1, AUX_KSQ = 2 };
+constexpr size_t kMaxSmem = 227 * 1024;
+
+template <class K>
+struct PipeSmem {
+    using C = typename K::C;
+    using T = typename C::T;
+    static constexpr size_t CTRL = (size_t)(C::NG + 1) * K::TILE_BYTES;          // mbarriers + issued[]
+    static constexpr size_t TWA = CTRL + 64;
+    static constexpr size_t TWA_BYTES = (size_t)C::N * sizeof(cx<T>);
+    static constexpr size_t TWB_BYTES = C::RB > 1 ? (size_t)C::MB * sizeof(cx<T>) : 0;
+    static constexpr size_t AUX_BYTES = K::AUX == AUX_PHASE ? (size_t)C::N * sizeof(cx<T>) : (K::AUX == AUX_KSQ ? (size_t)C::N * sizeof(T) : 0);
+    static constexpr bool TW_IN_SMEM = TWA + TWA_BYTES + TWB_BYTES <= kMaxSmem;
+    static constexpr size_t AUX_OFF = TWA + (TW_IN_SMEM ? TWA_BYTES + TWB_BYTES : 0);
+    static constexpr bool AUX_IN_SMEM = K::AUX != AUX_NONE && AUX_OFF + AUX_BYTES <= kMaxSmem;
+    static constexpr size_t TOTAL = AUX_OFF + (AUX_IN_SMEM ? AUX_BYTES : 0);
+};
+
+template <class K>
+__device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p, int ntiles, unsigned char *smem)
+{
+    using C = typename K::C;
+    constexpr int NTG = C::NT, NG = C::NG, NBUF = NG + 1;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)NBUF * K::TILE_BYTES);
+    // issued[b] = number of fills of buffer b started so far.  A parity wait can only tell the current phase
+    // from the one before it, so a consumer that has run ahead first makes sure the fill it needs has been
+    // STARTED (which implies the previous phase completed) before waiting on the parity.
+    volatile int *issued = reinterpret_cast<volatile int *>(full + NBUF);
+    const int tid = threadIdx.x, grp = tid / NTG, gt = tid - grp * NTG;
+    const int bid = blockIdx.x, stride = gridDim.x;
+    const int J = (ntiles - bid + stride - 1) / stride;        // tiles of this CTA: bid + j*stride
+    if (tid == 0)
+        for (int b = 0; b < NBUF; ++b) { mbar_init(full + b, NTG); issued[b] = (b < J) ? 1 : 0; }
+    using SM = PipeSmem<K>;
+    using T = typename C::T;
+    Tabs<T> tb{p.twA, p.twB, p.phase, p.ksq_pos};
+    if constexpr (SM::TW_IN_SMEM) {
+        cx<T> *a = reinterpret_cast<cx<T> *>(smem + SM::TWA);
+        for (int i = tid; i < C::N; i += NTG * NG) a[i] = p.twA[i];
+        tb.twA = a;
+        if constexpr (C::RB > 1) {
+            cx<T> *b2 = a + C::N;
+            for (int i = tid; i < C::MB; i += NTG * NG) b2[i] = p.twB[i];
+            tb.twB = b2;
+        }
+    }
+    if constexpr (SM::AUX_IN_SMEM && K::AUX == AUX_PHASE) {
+        cx<T> *a = reinterpret_cast<cx<T> *>(smem + SM::AUX_OFF);
+        for (int i = tid; i < C::N; i += NTG * NG) a[i] = p.phase[i];
+        tb.phase = a;
+    }
+    if constexpr (SM::AUX_IN_SMEM && K::AUX == AUX_KSQ) {
+        T *a = reinterpret_cast<T *>(smem + SM::AUX_OFF);
+        for (int i = tid; i < C::N; i += NTG * NG) a[i] = p.ksq_pos[i];
+        tb.ksq_pos = a;
+    }
+    __syncthreads();
+    for (int j = 0; j < NBUF && j < J; ++j)
+        if (j % NG == grp) {
+            K::issue(p, bid + j * stride, smem + (size_t)j * K::TILE_BYTES, gt);
+            cp_async_arrive(full + j);
+        }
+    typename K::Pre pre;
+    if (grp < J) K::prefetch(p, bid + grp * stride, gt, pre);
+    for (int j = grp; j < J; j += NG) {
+        const int b = j % NBUF;
+        unsigned char *buf = smem + (size_t)b * K::TILE_BYTES;
+        while (issued[b] < j / NBUF + 1) __nanosleep(64);
+        mbar_wait(full + b, (j / NBUF) & 1);
+        const int jn = j + NG;
+        K::compute(p, tb, bid + j * stride, jn < J ? bid + jn * stride : -1, buf, gt, grp, pre);
+        group_sync(grp, NTG);                                   // every read of this buffer is done
+        if (j + NBUF < J) {
+            if (gt == 0) issued[b] = (j + NBUF) / NBUF + 1;
+            K::issue(p, bid + (j + NBUF) * stride, buf, gt);
+            cp_async_arrive(full + b);
+        }
+    }
+}
+
+// ---------------------------------------------------------------- shared building blocks
+
+// asynchronous tile load.  Strided tiles: row j is W contiguous elements (16-byte chunks, a warp covers
+// whole 128-byte rows).  Contiguous tiles: W pencils, transposed on the fly into the padded [row][line]
+// layout (one element per copy; lanes walk along a pencil, so global reads are coalesced and the shared
+// stores hit distinct banks because the row stride W+1 is odd).
+template <class C, int AX, int ROWS>
+__device__ __forceinline__ void issue_tile(cx<typename C::T> *S, const cx<typename C::T> *src, const Tile<C, AX> &tile, int gt)
+{
+    using T = typename C::T;
+    constexpr int RS = Tile<C, AX>::RS, W = C::W, NTG = C::NT;
+    if constexpr (AX == AX_STRIDED) {
+        constexpr int EPC = 16 / (int)sizeof(cx<T>);            // elements per 16-byte chunk
+        constexpr int CH = W / EPC;                             // chunks per row
+        static_assert(W % EPC == 0, "row must be a whole number of 16-byte chunks");
+#pragma unroll 4
+        for (int c = gt; c < ROWS * CH; c += NTG) {
+            int row = c / CH, part = (c - row * CH) * EPC;
+            cp_async16(S + row * RS + part, src + tile.at(row, part));
+        }
+    } else {
+#pragma unroll 4
+        for (int e = gt; e < ROWS * W; e += NTG) {
+            int row = e % ROWS, l = e / ROWS;
+            cp_async_elem(S + row * RS + l, src + tile.at(row, l));
+        }
+    }
+}
+
+// level B stages with the group barrier
+template <class C, int W, int RS, typename T>
+__device__ __forceinline__ void g_fwd_B(cx<T> *S, const cx<T> *twB, int gt, int grp)
+{
+    if constexpr (C::RB > 1) {
+        constexpr int NB = C::N / C::RB;
+        for (int b = gt; b < NB * W; b += C::NT) {
+            int l = b % W, g = b / W, blk = g / C::mB, q = g - blk * C::mB;
+            fwd_level<C::RB, T>(blk * C::MB + q, C::mB, twB + q, [&](int row) { return S[row * RS + l]; },
+                                [&](int row, cx<T> v) { S[row * RS + l] = v; });
+        }
+        group_sync(grp, C::NT);
+    }
+}
+template <class C, int W, int RS, typename T>
+__device__ __forceinline__ void g_inv_B(cx<T> *S, const cx<T> *twB, int gt, int grp)
+{
+    if constexpr (C::RB > 1) {
+        constexpr int NB = C::N / C::RB;
+        for (int b = gt; b < NB * W; b += C::NT) {
+            int l = b % W, g = b / W, blk = g / C::mB, q = g - blk * C::mB;
+            inv_level<C::RB, T>(blk * C::MB + q, C::mB, twB + q, [&](int row) { return S[row * RS + l]; },
+                                [&](int row, cx<T> v) { S[row * RS + l] = v; });
+        }
+        group_sync(grp, C::NT);
+    }
+}
+
+struct NoPre {};
+
+constexpr size_t align128(size_t x) { return (x + 127) & ~(size_t)127; }
+
+// ---------------------------------------------------------------- psi sweep
+// DRIFT: FFT . per-axis kinetic phase . inverse FFT (Eq. 18(b)).  KICK: psi *= exp(-i Phi kick) as the tile
+// leaves shared memory for the first butterfly (Eq. 18(a),(d)); the Phi values of the NEXT tile are fetched
+// into registers before the current tile's last stage.  RHO (x axis): rho - <rho> = |psi2|^2 (+ rho_p) - <rho>
+// formed from the outgoing registers, packed real-to-complex FFT along x in the same buffer -> H.
+template <class C_, int AX, bool KICK, bool RHO, bool DRIFT>
+struct PsiK {
+    using C = C_;
+    using T = typename C::T;
+    using TL = Tile<C, AX>;
+    static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA, RS = TL::RS;
+    static constexpr int ITER = (mA * W) / NTG;
+    static_assert((mA * W) % NTG == 0, "whole number of level-A butterflies per thread");
+    static_assert(!RHO || AX == AX_STRIDED, "the density sweep runs along a strided axis");
+    static constexpr size_t TILE_BYTES = align128((size_t)N * RS * sizeof(cx<T>));
+    static constexpr int AUX = DRIFT ? AUX_PHASE : AUX_NONE;
+    struct Pre { T th[KICK ? ITER : 1][KICK ? RA : 1]; };
+
+    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
+    {
+        const TL tile(p, t);
+        issue_tile<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, tile, gt);
+    }
+    static __device__ __forceinline__ void prefetch(const SweepParams<T> &p, int t, int gt, Pre &pre)
+    {
+        if constexpr (KICK) {
+            const TL tile(p, t);
+            static_for<0, ITER>([&](auto it_) {
+                constexpr int it = decltype(it_)::value;
+                int q, l;
+                split<AX, mA, W>(gt + it * NTG, q, l);
+                static_for<0, RA>([&](auto r_) {
+                    constexpr int r = decltype(r_)::value;
+                    pre.th[it][r] = ldg(p.phi + tile.at(q + mA * r, l));
+                });
+            });
+        }
+    }
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, int tnext, unsigned char *buf, int gt,
+                                                   int grp, Pre &pre)
+    {
+        cx<T> *S = reinterpret_cast<cx<T> *>(buf);
+        const TL tile(p, t);
+        cx<T> *psi = p.data;
+        T rho[RHO ? ITER : 1][RHO ? RA : 1];
+        if constexpr (DRIFT) {
+            static_for<0, ITER>([&](auto it_) {
+                constexpr int it = decltype(it_)::value;
+                int q, l;
+                split<AX, mA, W>(gt + it * NTG, q, l);
+                cx<T> v[RA];
+                static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = S[(q + mA * r) * RS + l]; });
+                if constexpr (KICK)
+                    static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], pre.th[it][r] * p.kick); });
+                fwd_level_regs<RA, T>(v, q, mA, tb.twA + q, [&](int row, cx<T> y) { S[row * RS + l] = y; });
+            });
+            group_sync(grp, NTG);
+            g_fwd_B<C, W, RS, T>(S, tb.twB, gt, grp);
+            for (int b = gt; b < (N / RM) * W; b += NTG) {
+                int l = b % W, g = b / W;
+                mid_both<RM, T>(g * RM, [&](int row) { return S[row * RS + l]; },
+                                [&](int row, cx<T> v) { S[row * RS + l] = v; },
+                                [&](int pos, cx<T> v) { return cmul(v, tb.phase[pos]); });
+            }
+            group_sync(grp, NTG);
+            g_inv_B<C, W, RS, T>(S, tb.twB, gt, grp);
+            if (KICK && tnext >= 0) prefetch(p, tnext, gt, pre);
+            static_for<0, ITER>([&](auto it_) {
+                constexpr int it = decltype(it_)::value;
+                int q, l;
+                split<AX, mA, W>(gt + it * NTG, q, l);
+                cx<T> v[RA];
+                inv_level_regs<RA, T>(q, mA, tb.twA + q, [&](int row) { return S[row * RS + l]; }, v);
+                static_for<0, RA>([&](auto r_) {
+                    constexpr int r = decltype(r_)::value;
+                    stv(psi + tile.at(q + mA * r, l), v[r]);
+                    if constexpr (RHO) rho[it][r] = v[r].x * v[r].x + v[r].y * v[r].y;
+                });
+            });
+        } else if constexpr (RHO) {
+            static_for<0, ITER>([&](auto it_) {
+                constexpr int it = decltype(it_)::value;
+                int q, l;
+                split<AX, mA, W>(gt + it * NTG, q, l);
+                static_for<0, RA>([&](auto r_) {
+                    constexpr int r = decltype(r_)::value;
+                    cx<T> v = S[(q + mA * r) * RS + l];
+                    rho[it][r] = v.x * v.x + v.y * v.y;
+                });
+            });
+        }
+        if constexpr (RHO) {
+            // rho tile as N rows x W reals == N rows x W/2 packed complex lines (lines 2l', 2l'+1)
+            constexpr int WP = W / 2, RSP = W / 2;
+            T *F = reinterpret_cast<T *>(buf);
+            group_sync(grp, NTG);                       // every thread has finished reading the psi tile
+            // rho - <rho> (Eq. 23).  <rho> is conserved, so it is measured once per refresh; k = 0 is
+            // zeroed in the Green's function anyway -- subtracting here only keeps the large mean out of the
+            // single-precision partial sums of the low-k modes.
+            const T mean = ldg(p.rho_mean);
+            static_for<0, ITER>([&](auto it_) {
+                constexpr int it = decltype(it_)::value;
+                int q, l;
+                split<AX, mA, W>(gt + it * NTG, q, l);
+                static_for<0, RA>([&](auto r_) {
+                    constexpr int r = decltype(r_)::value;
+                    int row = q + mA * r;
+                    T v = rho[it][r];
+                    if (p.rho_p) v += ldg(p.rho_p + tile.at(row, l));
+                    F[row * W + l] = v - mean;
+                });
+            });
+            group_sync(grp, NTG);
+            cx<T> *Sp = reinterpret_cast<cx<T> *>(buf);
+            for (int b = gt; b < mA * WP; b += NTG) {
+                int l = b % WP, q = b / WP;
+                fwd_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; },
+                                 [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
+            }
+            group_sync(grp, NTG);
+            g_fwd_B<C, WP, RSP, T>(Sp, tb.twB, gt, grp);
+            for (int b = gt; b < (N / RM) * WP; b += NTG) {
+                int l = b % WP, g = b / WP;
+                mid_fwd<RM, T>(g * RM, [&](int row) { return Sp[row * RSP + l]; },
+                               [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
+            }
+            group_sync(grp, NTG);
+            // Hermitian split of Z = FFT(a + i b):  A_k = (Z_k + conj Z_{N-k})/2,  B_k = (Z_k - conj Z_{N-k})/(2i)
+            for (int b = gt; b < (N / 2 + 1) * WP; b += NTG) {
+                int l = b % WP, k = b / WP;
+                int pk = ldg(p.pos_of_k + k), pn = ldg(p.pos_of_k + ((N - k) & (N - 1)));
+                cx<T> zk = Sp[pk * RSP + l], zn = Sp[pn * RSP + l];
+                const T h = (T)0.5;
+                cx<T> A = mk<T>((zk.x + zn.x) * h, (zk.y - zn.y) * h);
+                cx<T> B = mk<T>((zk.y + zn.y) * h, (zn.x - zk.x) * h);
+                st2(p.H + tile.at(k, 2 * l), A, B);
+            }
+        }
+    }
+};
+
+// ---------------------------------------------------------------- Poisson sweeps on the half spectrum
+template <class C_, int MODE>
+struct HK {
+    using C = C_;
+    using T = typename C::T;
+    static constexpr int AX = (MODE == H_Z_GREEN) ? AX_CONTIG : AX_STRIDED;
+    using TL = Tile<C, AX>;
+    static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA, RS = TL::RS;
+    static constexpr size_t TILE_BYTES = align128((size_t)N * RS * sizeof(cx<T>));
+    static constexpr int AUX = MODE == H_Z_GREEN ? AUX_KSQ : AUX_NONE;
+    using Pre = NoPre;
+    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
+    {
+        const TL tile(p, t);
+        issue_tile<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, tile, gt);
+    }
+    static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, int, unsigned char *buf, int gt, int grp, Pre &)
+    {
+        cx<T> *S = reinterpret_cast<cx<T> *>(buf);
+        const TL tile(p, t);
+        cx<T> *H = p.data;
+        auto ldS = [&](int l) { return [S, l](int row) { return S[row * RS + l]; }; };
+        auto stS = [&](int l) { return [S, l](int row, cx<T> v) { S[row * RS + l] = v; }; };
+        if constexpr (MODE == H_Y_FWD || MODE == H_Z_GREEN) {
+            for (int b = gt; b < mA * W; b += NTG) {
+                int q, l;
+                split<AX, mA, W>(b, q, l);
+                fwd_level<RA, T>(q, mA, tb.twA + q, ldS(l), stS(l));
+            }
+            group_sync(grp, NTG);
+            g_fwd_B<C, W, RS, T>(S, tb.twB, gt, grp);
+        }
+        if constexpr (MODE == H_Y_FWD) {
+            for (int b = gt; b < (N / RM) * W; b += NTG) {
+                int l = b % W, g = b / W;
+                mid_fwd<RM, T>(g * RM, ldS(l), [&](int row, cx<T> v) { stv(H + tile.at(row, l), v); });
+            }
+        }
+        if constexpr (MODE == H_Z_GREEN) {
+            // pencil l of this tile is (kx, y position) = divmod(t*W + l, N); the y axis is in position order
+            for (int b = gt; b < (N / RM) * W; b += NTG) {
+                int l = b % W, g = b / W;
+                int pen = t * W + l, kx = pen / N, ypos = pen - kx * N;
+                T kxy = ldg(p.ksq_nat + kx) + tb.ksq_pos[ypos];
+                bool zero_line = (kx == 0 && ypos == 0);
+                mid_both<RM, T>(g * RM, ldS(l), stS(l), [&](int pos, cx<T> v) {
+                    T k2 = kxy + tb.ksq_pos[pos];
+                    T gr = (zero_line && pos == 0) ? (T)0 : p.green / k2;
+                    return cscale(v, gr);
+                });
+            }
+            group_sync(grp, NTG);
+            g_inv_B<C, W, RS, T>(S, tb.twB, gt, grp);
+        }
+        if constexpr (MODE == H_Y_INV) {
+            for (int b = gt; b < (N / RM) * W; b += NTG) {
+                int l = b % W, g = b / W;
+                mid_inv<RM, T>(g * RM, ldS(l), stS(l));
+            }
+            group_sync(grp, NTG);
+            g_inv_B<C, W, RS, T>(S, tb.twB, gt, grp);
+        }
+        if constexpr (MODE == H_Y_INV || MODE == H_Z_GREEN) {
+            for (int b = gt; b < mA * W; b += NTG) {
+                int q, l;
+                split<AX, mA, W>(b, q, l);
+                inv_level<RA, T>(q, mA, tb.twA + q, ldS(l), [&](int row, cx<T> v) { stv(H + tile.at(row, l), v); });
+            }
+        }
+    }
+};
+
+// complex-to-real inverse along x: H[kx <= N/2][y][z] -> Phi[x][y][z]; lines (2l', 2l'+1) share one FFT.
+// Buffer = [packed tile: N rows x W/2 complex][raw tile: N/2+1 rows x W complex, filled by the async copies].
+template <class C_>
+struct C2RK {
+    using C = C_;
+    using T = typename C::T;
+    using TL = Tile<C, AX_STRIDED>;
+    static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA;
+    static constexpr int WP = W / 2, RSP = W / 2;
+    static constexpr size_t PACKED_BYTES = align128((size_t)N * RSP * sizeof(cx<T>));
+    static constexpr size_t TILE_BYTES = PACKED_BYTES + align128((size_t)(N / 2 + 1) * W * sizeof(cx<T>));
+    static constexpr int AUX = AUX_NONE;
+    using Pre = NoPre;
+    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
+    {
+        const TL tile(p, t);
+        issue_tile<C, AX_STRIDED, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf + PACKED_BYTES), p.H, tile, gt);
+    }
+    static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, int, unsigned char *buf, int gt, int grp, Pre &)
+    {
+        cx<T> *Sp = reinterpret_cast<cx<T> *>(buf);
+        const cx<T> *R = reinterpret_cast<const cx<T> *>(buf + PACKED_BYTES);
+        const TL tile(p, t);
+        // Z_k = A_k + i B_k,  Z_{N-k} = conj(A_k) + i conj(B_k)
+        for (int b = gt; b < (N / 2 + 1) * WP; b += NTG) {
+            int l = b % WP, k = b / WP;
+            cx<T> A = R[k * W + 2 * l], B = R[k * W + 2 * l + 1];
+            int pk = ldg(p.pos_of_k + k);
+            Sp[pk * RSP + l] = mk<T>(A.x - B.y, A.y + B.x);
+            if (k > 0 && k < N / 2) {
+                int pn = ldg(p.pos_of_k + (N - k));
+                Sp[pn * RSP + l] = mk<T>(A.x + B.y, B.x - A.y);
+            }
+        }
+        group_sync(grp, NTG);
+        for (int b = gt; b < (N / RM) * WP; b += NTG) {
+            int l = b % WP, g = b / WP;
+            mid_inv<RM, T>(g * RM, [&](int row) { return Sp[row * RSP + l]; },
+                           [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
+        }
+        group_sync(grp, NTG);
+        g_inv_B<C, WP, RSP, T>(Sp, tb.twB, gt, grp);
+        for (int b = gt; b < mA * WP; b += NTG) {
+            int l = b % WP, q = b / WP;
+            inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; },
+                             [&](int row, cx<T> v) {
+                                 // Re -> line 2l', Im -> line 2l'+1: one (re, im) pair is two adjacent reals of Phi
+                                 stv(reinterpret_cast<cx<T> *>(p.phi_out + tile.at(row, 2 * l)), v);
+                             });
+        }
+    }
+};
+
+}  // namespace wdm

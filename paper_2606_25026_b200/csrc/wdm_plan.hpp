@@ -11,35 +11,37 @@
 namespace wdm {
 
 struct Fact {
-    int N, RA, RB, RM, W, NT, MINB;
+    int N, RA, RB, RM, W, NT, NG, MINB;
 };
 
-// One factorisation per (N, dtype); must match the LineCfg instantiated in wdm_sweeps.cu.
+// One factorisation per (N, dtype): X(N, RA, RB, RM, W, NT, NG, MINB); wdm_sweeps.cu instantiates the same rows.
 // complex64 : two levels, radix <= 32 (a radix-32 butterfly is 64 registers of data).
 // complex128: radix <= 16 (a radix-16 butterfly is already 64 registers), three levels for N >= 512.
-#define WDM_FACT_C64(X)        \
-    X(8, 2, 1, 4, 8, 32, 8)    \
-    X(16, 4, 1, 4, 16, 64, 8)  \
-    X(32, 4, 1, 8, 16, 128, 4) \
-    X(64, 8, 1, 8, 16, 128, 4) \
-    X(128, 8, 1, 16, 16, 128, 4) \
-    X(256, 16, 1, 16, 16, 256, 2) \
-    X(512, 16, 1, 32, 16, 256, 2) \
-    X(1024, 32, 1, 32, 8, 256, 2)
-#define WDM_FACT_C128(X)       \
-    X(8, 2, 1, 4, 8, 32, 8)    \
-    X(16, 4, 1, 4, 8, 32, 8)   \
-    X(32, 4, 1, 8, 8, 64, 4)   \
-    X(64, 8, 1, 8, 8, 64, 4)   \
-    X(128, 8, 1, 16, 8, 64, 4) \
-    X(256, 16, 1, 16, 8, 128, 2) \
-    X(512, 8, 8, 8, 8, 256, 2) \
-    X(1024, 8, 8, 16, 8, 256, 1)
+// W lines per tile (128-byte rows where shared memory allows), NT threads per compute group, NG groups and
+// NG + 1 tile buffers per CTA, MINB CTAs per SM.
+#define WDM_FACT_C64(X)             \
+    X(8, 2, 1, 4, 8, 32, 2, 4)      \
+    X(16, 4, 1, 4, 16, 64, 2, 4)    \
+    X(32, 4, 1, 8, 16, 128, 2, 4)   \
+    X(64, 8, 1, 8, 16, 128, 2, 4)   \
+    X(128, 8, 1, 16, 16, 128, 2, 2) \
+    X(256, 16, 1, 16, 16, 256, 2, 1) \
+    X(512, 16, 1, 32, 16, 256, 2, 1) \
+    X(1024, 32, 1, 32, 8, 256, 2, 1)
+#define WDM_FACT_C128(X)            \
+    X(8, 2, 1, 4, 8, 32, 2, 4)      \
+    X(16, 4, 1, 4, 8, 32, 2, 4)     \
+    X(32, 4, 1, 8, 8, 64, 2, 4)     \
+    X(64, 8, 1, 8, 8, 64, 2, 2)     \
+    X(128, 8, 1, 16, 8, 64, 2, 2)   \
+    X(256, 16, 1, 16, 8, 128, 2, 1) \
+    X(512, 8, 8, 8, 8, 256, 2, 1)   \
+    X(1024, 8, 8, 16, 4, 256, 1, 1)
 
 inline bool find_fact(int N, int dtype, Fact &f)
 {
-#define X(n, ra, rb, rm, w, nt, minb) \
-    if (N == n) { f = Fact{n, ra, rb, rm, w, nt, minb}; return true; }
+#define X(n, ra, rb, rm, w, nt, ng, minb) \
+    if (N == n) { f = Fact{n, ra, rb, rm, w, nt, ng, minb}; return true; }
     if (dtype == 0) { WDM_FACT_C64(X) }
     else { WDM_FACT_C128(X) }
 #undef X
