@@ -13,8 +13,8 @@
 // lives at smem[j * RS + l]; a half-warp always touches one whole row, so any butterfly stride is free
 // of bank conflicts.
 //
-// The same source compiles for the host (thread-per-std::thread emulation used while developing), hence
-// the WDM_HD / WDM_SYNC macros; the product only ever runs the sm_100a build.
+// The arithmetic here is plain C++ (WDM_HD = __host__ __device__), so the host-side plan code can share the
+// digit-reversal helpers; the product only ever runs the sm_100a build.
 #pragma once
 
 #include <stdint.h>
@@ -206,6 +206,21 @@ WDM_HD void mid_both(int rowbase, LD &&ld, ST &&st, MUL &&mul)
     });
     dit_inv<R>(v);
     static_for<0, R>([&](auto r) { st(rowbase + decltype(r)::value, v[decltype(r)::value]); });
+}
+
+// same, the R consecutive rows moved as pairs (16-byte shared-memory vectors for complex64)
+template <int R, typename T, class LD2, class ST2, class MUL>
+WDM_HD void mid_both2(int rowbase, LD2 &&ld2, ST2 &&st2, MUL &&mul)
+{
+    cx<T> v[R];
+    static_for<0, R / 2>([&](auto i_) { constexpr int i = decltype(i_)::value; ld2(rowbase + 2 * i, v[2 * i], v[2 * i + 1]); });
+    dif_fwd<R>(v);
+    static_for<0, R>([&](auto j_) {
+        constexpr int j = decltype(j_)::value;
+        v[j] = mul(rowbase + brev(j, R), v[j]);
+    });
+    dit_inv<R>(v);
+    static_for<0, R / 2>([&](auto i_) { constexpr int i = decltype(i_)::value; st2(rowbase + 2 * i, v[2 * i], v[2 * i + 1]); });
 }
 
 template <int R, typename T, class LD, class ST>

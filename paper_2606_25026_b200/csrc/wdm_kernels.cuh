@@ -8,25 +8,17 @@
 //   Poisson sweeps (4 per step) on the half-spectrum H[kx <= N/2][y][z]: y forward, z forward . Green . inverse
 //       (Eq. 18(c), Eq. 23: -4 pi G / k^2, k = 0 zeroed), y inverse, x complex-to-real -> Phi.
 //
-// Each body is written per thread (tid) and per tile (bid) with WDM_SYNC() as the CTA barrier.
+// This header holds what every sweep shares: parameters, tile addressing and memory-access helpers.  The
+// kernels themselves (persistent, software-pipelined) are in wdm_pipe.cuh.
 #pragma once
 
 #include "wdm_fft.cuh"
 
-#if defined(__CUDACC__)
 #define WDM_DEV __device__ __forceinline__
-#define WDM_SYNC() __syncthreads()
-#else
-#include <cmath>
-#define WDM_DEV inline __attribute__((always_inline))
-void wdm_host_sync();
-#define WDM_SYNC() wdm_host_sync()
-#endif
 
 namespace wdm {
 
 // ---------------------------------------------------------------- global memory access helpers
-#if defined(__CUDACC__)
 WDM_DEV cx<float> ldg(const cx<float> *p) { float2 t = __ldg(reinterpret_cast<const float2 *>(p)); return mk<float>(t.x, t.y); }
 WDM_DEV cx<double> ldg(const cx<double> *p) { double2 t = __ldg(reinterpret_cast<const double2 *>(p)); return mk<double>(t.x, t.y); }
 WDM_DEV float ldg(const float *p) { return __ldg(p); }
@@ -40,25 +32,27 @@ WDM_DEV void ld2(const cx<float> *p, cx<float> &a, cx<float> &b) { float4 t = *r
 WDM_DEV void st2(cx<float> *p, cx<float> a, cx<float> b) { *reinterpret_cast<float4 *>(p) = make_float4(a.x, a.y, b.x, b.y); }
 WDM_DEV void ld2(const cx<double> *p, cx<double> &a, cx<double> &b) { a = ldv(p); b = ldv(p + 1); }
 WDM_DEV void st2(cx<double> *p, cx<double> a, cx<double> b) { stv(p, a); stv(p + 1, b); }
-WDM_DEV void sincos_t(float x, float *s, float *c) { sincosf(x, s, c); }
-WDM_DEV void sincos_t(double x, double *s, double *c) { sincos(x, s, c); }
-#else
-template <typename U> WDM_DEV U ldg(const U *p) { return *p; }
-template <typename U> WDM_DEV U ldv(const U *p) { return *p; }
-template <typename U> WDM_DEV void stv(U *p, U v) { *p = v; }
-template <typename U> WDM_DEV void ld2(const U *p, U &a, U &b) { a = p[0]; b = p[1]; }
-template <typename U> WDM_DEV void st2(U *p, U a, U b) { p[0] = a; p[1] = b; }
-WDM_DEV void sincos_t(float x, float *s, float *c) { *s = std::sin(x); *c = std::cos(x); }
-WDM_DEV void sincos_t(double x, double *s, double *c) { *s = std::sin(x); *c = std::cos(x); }
-#endif
 
-// psi * exp(-i theta)
-template <typename T>
-WDM_DEV cx<T> rotate_neg(cx<T> v, T theta)
+// psi * exp(-i theta).  |theta| = |Phi| dt/(2 mu) is far below 1 under the CFL limit (Eq. 26),
+// so the single-precision path takes the Taylor branch (truncation error < 1e-11 for |theta| < 1/4, below
+// float rounding) and falls back to sincosf only for large phases.
+WDM_DEV cx<float> rotate_neg(cx<float> v, float th)
 {
-    T s, c;
-    sincos_t(theta, &s, &c);
-    return mk<T>(v.x * c + v.y * s, v.y * c - v.x * s);
+    float s, c;
+    if (fabsf(th) < 0.25f) {
+        float t2 = th * th;
+        s = th * fmaf(t2, fmaf(t2, fmaf(t2, -1.0f / 5040.0f, 1.0f / 120.0f), -1.0f / 6.0f), 1.0f);
+        c = fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, 1.0f / 40320.0f, -1.0f / 720.0f), 1.0f / 24.0f), -0.5f), 1.0f);
+    } else {
+        sincosf(th, &s, &c);
+    }
+    return mk<float>(v.x * c + v.y * s, v.y * c - v.x * s);
+}
+WDM_DEV cx<double> rotate_neg(cx<double> v, double th)
+{
+    double s, c;
+    sincos(th, &s, &c);
+    return mk<double>(v.x * c + v.y * s, v.y * c - v.x * s);
 }
 
 // ---------------------------------------------------------------- parameters
@@ -86,9 +80,26 @@ struct SweepParams {
 
 enum { AX_STRIDED = 0, AX_CONTIG = 1 };
 
+// Shared-memory layout of a tile (row = position along the transformed axis, l = line).
+//   strided axis   : [row][l], row stride W  -- a half-warp (complex64) reads one whole 128-byte row, so a
+//                    butterfly of any stride is free of bank conflicts; filled by 16-byte async copies.
+//   contiguous axis: [l][row], line stride N + 16 bytes -- filled by 16-byte async copies straight along
+//                    each pencil; level A walks rows with consecutive lanes, the middle level reads its R
+//                    consecutive rows as 16-byte vectors with lanes on different lines (the odd line
+//                    stride in 16-byte units spreads them over all banks).
+template <class C, int AX>
+struct Lay {
+    using T = typename C::T;
+    static constexpr int PAD = 16 / (int)sizeof(cx<T>);
+    static constexpr int LS = C::N + PAD;
+    static constexpr int RS = C::W;
+    static constexpr size_t ELEMS = AX == AX_CONTIG ? (size_t)C::W * LS : (size_t)C::N * RS;
+    static constexpr bool VEC2 = AX == AX_CONTIG && sizeof(T) == 4;
+    static WDM_DEV int idx(int row, int l) { return AX == AX_CONTIG ? l * LS + row : row * RS + l; }
+};
+
 template <class C, int AX>
 struct Tile {
-    static constexpr int RS = (AX == AX_CONTIG) ? C::W + 1 : C::W;   // smem row stride (elements)
     long long base, rstride, lstride;
     template <typename T>
     WDM_DEV Tile(const SweepParams<T> &p, int bid)
@@ -116,298 +127,6 @@ WDM_DEV void split(int b, int &g, int &l)
     else { g = b % NB; l = b / NB; }
 }
 
-// ---------------------------------------------------------------- in-shared-memory stages (lines fastest)
-
-template <class C, int W, int RS, typename T>
-WDM_DEV void smem_fwd_B(cx<T> *S, const cx<T> *twB, int tid)
-{
-    if constexpr (C::RB > 1) {
-        constexpr int NB = C::N / C::RB;
-        for (int b = tid; b < NB * W; b += C::NT) {
-            int l = b % W, g = b / W, blk = g / C::mB, q = g - blk * C::mB;
-            fwd_level<C::RB, T>(blk * C::MB + q, C::mB, twB + q,
-                                [&](int row) { return S[row * RS + l]; },
-                                [&](int row, cx<T> v) { S[row * RS + l] = v; });
-        }
-        WDM_SYNC();
-    }
-}
-
-template <class C, int W, int RS, typename T>
-WDM_DEV void smem_inv_B(cx<T> *S, const cx<T> *twB, int tid)
-{
-    if constexpr (C::RB > 1) {
-        constexpr int NB = C::N / C::RB;
-        for (int b = tid; b < NB * W; b += C::NT) {
-            int l = b % W, g = b / W, blk = g / C::mB, q = g - blk * C::mB;
-            inv_level<C::RB, T>(blk * C::MB + q, C::mB, twB + q,
-                                [&](int row) { return S[row * RS + l]; },
-                                [&](int row, cx<T> v) { S[row * RS + l] = v; });
-        }
-        WDM_SYNC();
-    }
-}
-
-// ---------------------------------------------------------------- psi sweep
-// DRIFT: FFT . phase . inverse FFT along the axis.  KICK: psi *= exp(-i phi kick) on load.
-// RHO (strided x axis only): rho = |psi|^2 (+rho_p) -> packed real-to-complex FFT along x -> H.
-
-template <class C, int AX, bool KICK, bool RHO, bool DRIFT>
-WDM_DEV void psi_sweep_body(const SweepParams<typename C::T> &p, int tid, int bid, unsigned char *smem_raw)
-{
-    using T = typename C::T;
-    constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NT = C::NT, mA = C::mA;
-    using TL = Tile<C, AX>;
-    constexpr int RS = TL::RS;
-    static_assert(!RHO || AX == AX_STRIDED, "the density sweep runs along a strided axis");
-    static_assert((mA * W) % NT == 0 || !RHO, "density sweep needs a whole number of butterflies per thread");
-    cx<T> *S = reinterpret_cast<cx<T> *>(smem_raw);
-    const TL tile(p, bid);
-    cx<T> *psi = p.data;
-    constexpr int ITER = RHO ? (mA * W) / NT : 1;
-    T rho[ITER][RA];
-
-    auto load_psi = [&](int row, int l) {
-        long long a = tile.at(row, l);
-        cx<T> v = ldv(psi + a);
-        if (KICK) v = rotate_neg(v, ldg(p.phi + a) * p.kick);
-        return v;
-    };
-
-    if constexpr (DRIFT) {
-        // level A forward: global -> registers -> shared (all loads of a butterfly are issued before any use)
-        for (int b = tid; b < mA * W; b += NT) {
-            int q, l;
-            split<AX, mA, W>(b, q, l);
-            cx<T> v[RA];
-            static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = ldv(psi + tile.at(q + mA * r, l)); });
-            if constexpr (KICK) {
-                T th[RA];
-                static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; th[r] = ldg(p.phi + tile.at(q + mA * r, l)); });
-                static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], th[r] * p.kick); });
-            }
-            fwd_level_regs<RA, T>(v, q, mA, p.twA + q, [&](int row, cx<T> y) { S[row * RS + l] = y; });
-        }
-        WDM_SYNC();
-        smem_fwd_B<C, W, RS, T>(S, p.twB, tid);
-        // middle level: forward . kinetic phase . inverse
-        for (int b = tid; b < (N / RM) * W; b += NT) {
-            int l = b % W, g = b / W;
-            mid_both<RM, T>(g * RM, [&](int row) { return S[row * RS + l]; },
-                            [&](int row, cx<T> v) { S[row * RS + l] = v; },
-                            [&](int pos, cx<T> v) { return cmul(v, ldg(p.phase + pos)); });
-        }
-        WDM_SYNC();
-        smem_inv_B<C, W, RS, T>(S, p.twB, tid);
-        // level A inverse: shared -> registers -> global
-        if constexpr (RHO) {
-            static_for<0, ITER>([&](auto it_) {
-                constexpr int it = decltype(it_)::value;
-                int b = tid + it * NT, q, l;
-                split<AX, mA, W>(b, q, l);
-                cx<T> v[RA];
-                inv_level_regs<RA, T>(q, mA, p.twA + q, [&](int row) { return S[row * RS + l]; }, v);
-                static_for<0, RA>([&](auto r_) {
-                    constexpr int r = decltype(r_)::value;
-                    stv(psi + tile.at(q + mA * r, l), v[r]);
-                    rho[it][r] = v[r].x * v[r].x + v[r].y * v[r].y;
-                });
-            });
-        } else {
-            for (int b = tid; b < mA * W; b += NT) {
-                int q, l;
-                split<AX, mA, W>(b, q, l);
-                inv_level<RA, T>(q, mA, p.twA + q, [&](int row) { return S[row * RS + l]; },
-                                 [&](int row, cx<T> v) { stv(psi + tile.at(row, l), v); });
-            }
-        }
-    } else if constexpr (RHO) {
-        static_for<0, ITER>([&](auto it_) {
-            constexpr int it = decltype(it_)::value;
-            int b = tid + it * NT, q, l;
-            split<AX, mA, W>(b, q, l);
-            static_for<0, RA>([&](auto r_) {
-                constexpr int r = decltype(r_)::value;
-                cx<T> v = load_psi(q + mA * r, l);
-                rho[it][r] = v.x * v.x + v.y * v.y;
-            });
-        });
-    }
-
-    if constexpr (RHO) {
-        // rho tile as N rows x W reals == N rows x W/2 packed complex lines (lines 2l', 2l'+1)
-        constexpr int WP = W / 2, RSP = W / 2;
-        T *F = reinterpret_cast<T *>(smem_raw);
-        if (DRIFT) WDM_SYNC();   // every thread has finished reading the psi tile
-        // rho - <rho> (Eq. 23).  <rho> is conserved, so it is measured once per refresh; the k = 0
-        // mode is zeroed in the Green's function anyway -- subtracting here only keeps the large mean out of
-        // the single-precision partial sums of the low-k modes.
-        const T mean = ldg(p.rho_mean);
-        static_for<0, ITER>([&](auto it_) {
-            constexpr int it = decltype(it_)::value;
-            int b = tid + it * NT, q, l;
-            split<AX, mA, W>(b, q, l);
-            static_for<0, RA>([&](auto r_) {
-                constexpr int r = decltype(r_)::value;
-                int row = q + mA * r;
-                T v = rho[it][r];
-                if (p.rho_p) v += ldg(p.rho_p + tile.at(row, l));
-                F[row * W + l] = v - mean;
-            });
-        });
-        WDM_SYNC();
-        cx<T> *Sp = reinterpret_cast<cx<T> *>(smem_raw);
-        for (int b = tid; b < mA * WP; b += NT) {
-            int l = b % WP, q = b / WP;
-            fwd_level<RA, T>(q, mA, p.twA + q, [&](int row) { return Sp[row * RSP + l]; },
-                             [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
-        }
-        WDM_SYNC();
-        smem_fwd_B<C, WP, RSP, T>(Sp, p.twB, tid);
-        for (int b = tid; b < (N / RM) * WP; b += NT) {
-            int l = b % WP, g = b / WP;
-            mid_fwd<RM, T>(g * RM, [&](int row) { return Sp[row * RSP + l]; },
-                           [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
-        }
-        WDM_SYNC();
-        // Hermitian split of Z = FFT(a + i b):  A_k = (Z_k + conj Z_{N-k})/2,  B_k = (Z_k - conj Z_{N-k})/(2i)
-        for (int b = tid; b < (N / 2 + 1) * WP; b += NT) {
-            int l = b % WP, k = b / WP;
-            int pk = ldg(p.pos_of_k + k), pn = ldg(p.pos_of_k + ((N - k) & (N - 1)));
-            cx<T> zk = Sp[pk * RSP + l], zn = Sp[pn * RSP + l];
-            const T h = (T)0.5;
-            cx<T> A = mk<T>((zk.x + zn.x) * h, (zk.y - zn.y) * h);
-            cx<T> B = mk<T>((zk.y + zn.y) * h, (zn.x - zk.x) * h);
-            st2(p.H + tile.at(k, 2 * l), A, B);
-        }
-    }
-}
-
-// ---------------------------------------------------------------- Poisson sweeps on the half spectrum
-
 enum { H_Y_FWD = 0, H_Z_GREEN = 1, H_Y_INV = 2 };
-
-template <class C, int MODE>
-WDM_DEV void h_sweep_body(const SweepParams<typename C::T> &p, int tid, int bid, unsigned char *smem_raw)
-{
-    using T = typename C::T;
-    constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NT = C::NT, mA = C::mA;
-    constexpr int AX = (MODE == H_Z_GREEN) ? AX_CONTIG : AX_STRIDED;
-    using TL = Tile<C, AX>;
-    constexpr int RS = TL::RS;
-    cx<T> *S = reinterpret_cast<cx<T> *>(smem_raw);
-    const TL tile(p, bid);
-    cx<T> *H = p.data;
-
-    if constexpr (MODE == H_Y_FWD || MODE == H_Z_GREEN) {
-        for (int b = tid; b < mA * W; b += NT) {
-            int q, l;
-            split<AX, mA, W>(b, q, l);
-            fwd_level<RA, T>(q, mA, p.twA + q, [&](int row) { return ldv(H + tile.at(row, l)); },
-                             [&](int row, cx<T> v) { S[row * RS + l] = v; });
-        }
-        WDM_SYNC();
-        smem_fwd_B<C, W, RS, T>(S, p.twB, tid);
-    }
-    if constexpr (MODE == H_Y_FWD) {
-        for (int b = tid; b < (N / RM) * W; b += NT) {
-            int l = b % W, g = b / W;
-            mid_fwd<RM, T>(g * RM, [&](int row) { return S[row * RS + l]; },
-                           [&](int row, cx<T> v) { stv(H + tile.at(row, l), v); });
-        }
-    }
-    if constexpr (MODE == H_Z_GREEN) {
-        // pencil l of this tile is (kx, y position) = divmod(bid*W + l, N); the y axis is in position order
-        for (int b = tid; b < (N / RM) * W; b += NT) {
-            int l = b % W, g = b / W;
-            int pen = bid * W + l, kx = pen / N, ypos = pen - kx * N;
-            T kxy = ldg(p.ksq_nat + kx) + ldg(p.ksq_pos + ypos);
-            bool zero_line = (kx == 0 && ypos == 0);
-            mid_both<RM, T>(g * RM, [&](int row) { return S[row * RS + l]; },
-                            [&](int row, cx<T> v) { S[row * RS + l] = v; },
-                            [&](int pos, cx<T> v) {
-                                T k2 = kxy + ldg(p.ksq_pos + pos);
-                                T gr = (zero_line && pos == 0) ? (T)0 : p.green / k2;
-                                return cscale(v, gr);
-                            });
-        }
-        WDM_SYNC();
-        smem_inv_B<C, W, RS, T>(S, p.twB, tid);
-    }
-    if constexpr (MODE == H_Y_INV) {
-        for (int b = tid; b < (N / RM) * W; b += NT) {
-            int l = b % W, g = b / W;
-            mid_inv<RM, T>(g * RM, [&](int row) { return ldv(H + tile.at(row, l)); },
-                           [&](int row, cx<T> v) { S[row * RS + l] = v; });
-        }
-        WDM_SYNC();
-        smem_inv_B<C, W, RS, T>(S, p.twB, tid);
-    }
-    if constexpr (MODE == H_Y_INV || MODE == H_Z_GREEN) {
-        for (int b = tid; b < mA * W; b += NT) {
-            int q, l;
-            split<AX, mA, W>(b, q, l);
-            inv_level<RA, T>(q, mA, p.twA + q, [&](int row) { return S[row * RS + l]; },
-                             [&](int row, cx<T> v) { stv(H + tile.at(row, l), v); });
-        }
-    }
-}
-
-// complex-to-real inverse along x: H[kx <= N/2][y][z] -> Phi[x][y][z]; lines (2l', 2l'+1) share one FFT
-template <class C>
-WDM_DEV void c2r_body(const SweepParams<typename C::T> &p, int tid, int bid, unsigned char *smem_raw)
-{
-    using T = typename C::T;
-    constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NT = C::NT, mA = C::mA;
-    constexpr int WP = W / 2, RSP = W / 2;
-    cx<T> *Sp = reinterpret_cast<cx<T> *>(smem_raw);
-    const Tile<C, AX_STRIDED> tile(p, bid);
-    // Z_k = A_k + i B_k,  Z_{N-k} = conj(A_k) + i conj(B_k).  Loads are issued in unrolled batches.
-    auto place = [&](int k, int l, cx<T> A, cx<T> B) {
-        int pk = ldg(p.pos_of_k + k);
-        Sp[pk * RSP + l] = mk<T>(A.x - B.y, A.y + B.x);
-        if (k > 0 && k < N / 2) {
-            int pn = ldg(p.pos_of_k + (N - k));
-            Sp[pn * RSP + l] = mk<T>(A.x + B.y, B.x - A.y);
-        }
-    };
-    constexpr int ITEMS = (N / 2) * WP;              // rows k < N/2
-    constexpr int UN = ITEMS % (NT * 8) == 0 ? 8 : (ITEMS % (NT * 4) == 0 ? 4 : (ITEMS % (NT * 2) == 0 ? 2 : 1));
-    static_assert(ITEMS % NT == 0 || ITEMS < NT, "pack loop");
-    for (int b0 = tid; b0 < ITEMS; b0 += NT * UN) {
-        cx<T> A[UN], B[UN];
-        static_for<0, UN>([&](auto u_) {
-            constexpr int u = decltype(u_)::value;
-            int b = b0 + u * NT;
-            if (ITEMS >= NT || b < ITEMS) ld2(p.H + tile.at(b / WP, 2 * (b % WP)), A[u], B[u]);
-        });
-        static_for<0, UN>([&](auto u_) {
-            constexpr int u = decltype(u_)::value;
-            int b = b0 + u * NT;
-            if (ITEMS >= NT || b < ITEMS) place(b / WP, b % WP, A[u], B[u]);
-        });
-    }
-    if (tid < WP) {
-        cx<T> A, B;
-        ld2(p.H + tile.at(N / 2, 2 * tid), A, B);
-        place(N / 2, tid, A, B);
-    }
-    WDM_SYNC();
-    for (int b = tid; b < (N / RM) * WP; b += NT) {
-        int l = b % WP, g = b / WP;
-        mid_inv<RM, T>(g * RM, [&](int row) { return Sp[row * RSP + l]; },
-                       [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
-    }
-    WDM_SYNC();
-    smem_inv_B<C, WP, RSP, T>(Sp, p.twB, tid);
-    for (int b = tid; b < mA * WP; b += NT) {
-        int l = b % WP, q = b / WP;
-        inv_level<RA, T>(q, mA, p.twA + q, [&](int row) { return Sp[row * RSP + l]; },
-                         [&](int row, cx<T> v) {
-                             // Re -> line 2l', Im -> line 2l'+1 : one (re, im) pair is two adjacent reals of Phi
-                             stv(reinterpret_cast<cx<T> *>(p.phi_out + tile.at(row, 2 * l)), v);
-                         });
-    }
-}
 
 }  // namespace wdm

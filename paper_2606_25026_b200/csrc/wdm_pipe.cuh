@@ -148,56 +148,57 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
 
 // ---------------------------------------------------------------- shared building blocks
 
-// asynchronous tile load.  Strided tiles: row j is W contiguous elements (16-byte chunks, a warp covers
-// whole 128-byte rows).  Contiguous tiles: W pencils, transposed on the fly into the padded [row][line]
-// layout (one element per copy; lanes walk along a pencil, so global reads are coalesced and the shared
-// stores hit distinct banks because the row stride W+1 is odd).
+// asynchronous tile load in 16-byte chunks (see Lay for the layouts).  Strided tiles: a row is W contiguous
+// elements, a warp covers whole 128-byte rows.  Contiguous tiles: a warp walks 512 bytes along one pencil.
 template <class C, int AX, int ROWS>
 __device__ __forceinline__ void issue_tile(cx<typename C::T> *S, const cx<typename C::T> *src, const Tile<C, AX> &tile, int gt)
 {
     using T = typename C::T;
-    constexpr int RS = Tile<C, AX>::RS, W = C::W, NTG = C::NT;
+    using L = Lay<C, AX>;
+    constexpr int W = C::W, NTG = C::NT;
+    constexpr int EPC = 16 / (int)sizeof(cx<T>);                // elements per 16-byte chunk
     if constexpr (AX == AX_STRIDED) {
-        constexpr int EPC = 16 / (int)sizeof(cx<T>);            // elements per 16-byte chunk
         constexpr int CH = W / EPC;                             // chunks per row
         static_assert(W % EPC == 0, "row must be a whole number of 16-byte chunks");
 #pragma unroll 4
         for (int c = gt; c < ROWS * CH; c += NTG) {
             int row = c / CH, part = (c - row * CH) * EPC;
-            cp_async16(S + row * RS + part, src + tile.at(row, part));
+            cp_async16(S + L::idx(row, part), src + tile.at(row, part));
         }
     } else {
+        constexpr int CH = ROWS / EPC;                          // chunks per pencil
 #pragma unroll 4
-        for (int e = gt; e < ROWS * W; e += NTG) {
-            int row = e % ROWS, l = e / ROWS;
-            cp_async_elem(S + row * RS + l, src + tile.at(row, l));
+        for (int c = gt; c < W * CH; c += NTG) {
+            int l = c / CH, row = (c - l * CH) * EPC;
+            cp_async16(S + L::idx(row, l), src + tile.at(row, l));
         }
     }
 }
 
 // level B stages with the group barrier
-template <class C, int W, int RS, typename T>
-__device__ __forceinline__ void g_fwd_B(cx<T> *S, const cx<T> *twB, int gt, int grp)
+// (IDX maps (row, line) to the shared-memory element index)
+template <class C, int W, class IDX, typename T>
+__device__ __forceinline__ void g_fwd_B(cx<T> *S, const cx<T> *twB, int gt, int grp, IDX idx)
 {
     if constexpr (C::RB > 1) {
         constexpr int NB = C::N / C::RB;
         for (int b = gt; b < NB * W; b += C::NT) {
             int l = b % W, g = b / W, blk = g / C::mB, q = g - blk * C::mB;
-            fwd_level<C::RB, T>(blk * C::MB + q, C::mB, twB + q, [&](int row) { return S[row * RS + l]; },
-                                [&](int row, cx<T> v) { S[row * RS + l] = v; });
+            fwd_level<C::RB, T>(blk * C::MB + q, C::mB, twB + q, [&](int row) { return S[idx(row, l)]; },
+                                [&](int row, cx<T> v) { S[idx(row, l)] = v; });
         }
         group_sync(grp, C::NT);
     }
 }
-template <class C, int W, int RS, typename T>
-__device__ __forceinline__ void g_inv_B(cx<T> *S, const cx<T> *twB, int gt, int grp)
+template <class C, int W, class IDX, typename T>
+__device__ __forceinline__ void g_inv_B(cx<T> *S, const cx<T> *twB, int gt, int grp, IDX idx)
 {
     if constexpr (C::RB > 1) {
         constexpr int NB = C::N / C::RB;
         for (int b = gt; b < NB * W; b += C::NT) {
             int l = b % W, g = b / W, blk = g / C::mB, q = g - blk * C::mB;
-            inv_level<C::RB, T>(blk * C::MB + q, C::mB, twB + q, [&](int row) { return S[row * RS + l]; },
-                                [&](int row, cx<T> v) { S[row * RS + l] = v; });
+            inv_level<C::RB, T>(blk * C::MB + q, C::mB, twB + q, [&](int row) { return S[idx(row, l)]; },
+                                [&](int row, cx<T> v) { S[idx(row, l)] = v; });
         }
         group_sync(grp, C::NT);
     }
@@ -217,11 +218,12 @@ struct PsiK {
     using C = C_;
     using T = typename C::T;
     using TL = Tile<C, AX>;
-    static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA, RS = TL::RS;
+    using L = Lay<C, AX>;
+    static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA;
     static constexpr int ITER = (mA * W) / NTG;
     static_assert((mA * W) % NTG == 0, "whole number of level-A butterflies per thread");
     static_assert(!RHO || AX == AX_STRIDED, "the density sweep runs along a strided axis");
-    static constexpr size_t TILE_BYTES = align128((size_t)N * RS * sizeof(cx<T>));
+    static constexpr size_t TILE_BYTES = align128(L::ELEMS * sizeof(cx<T>));
     static constexpr int AUX = DRIFT ? AUX_PHASE : AUX_NONE;
     struct Pre { T th[KICK ? ITER : 1][KICK ? RA : 1]; };
 
@@ -258,28 +260,33 @@ struct PsiK {
                 int q, l;
                 split<AX, mA, W>(gt + it * NTG, q, l);
                 cx<T> v[RA];
-                static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = S[(q + mA * r) * RS + l]; });
+                static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = S[L::idx(q + mA * r, l)]; });
                 if constexpr (KICK)
                     static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], pre.th[it][r] * p.kick); });
-                fwd_level_regs<RA, T>(v, q, mA, tb.twA + q, [&](int row, cx<T> y) { S[row * RS + l] = y; });
+                fwd_level_regs<RA, T>(v, q, mA, tb.twA + q, [&](int row, cx<T> y) { S[L::idx(row, l)] = y; });
             });
             group_sync(grp, NTG);
-            g_fwd_B<C, W, RS, T>(S, tb.twB, gt, grp);
+            auto idx = [](int row, int l) { return L::idx(row, l); };
+            g_fwd_B<C, W>(S, tb.twB, gt, grp, idx);
             for (int b = gt; b < (N / RM) * W; b += NTG) {
                 int l = b % W, g = b / W;
-                mid_both<RM, T>(g * RM, [&](int row) { return S[row * RS + l]; },
-                                [&](int row, cx<T> v) { S[row * RS + l] = v; },
-                                [&](int pos, cx<T> v) { return cmul(v, tb.phase[pos]); });
+                auto mul = [&](int pos, cx<T> v) { return cmul(v, tb.phase[pos]); };
+                if constexpr (L::VEC2)
+                    mid_both2<RM, T>(g * RM, [&](int row, cx<T> &a, cx<T> &c) { ld2(S + L::idx(row, l), a, c); },
+                                     [&](int row, cx<T> a, cx<T> c) { st2(S + L::idx(row, l), a, c); }, mul);
+                else
+                    mid_both<RM, T>(g * RM, [&](int row) { return S[L::idx(row, l)]; },
+                                    [&](int row, cx<T> v) { S[L::idx(row, l)] = v; }, mul);
             }
             group_sync(grp, NTG);
-            g_inv_B<C, W, RS, T>(S, tb.twB, gt, grp);
+            g_inv_B<C, W>(S, tb.twB, gt, grp, idx);
             if (KICK && tnext >= 0) prefetch(p, tnext, gt, pre);
             static_for<0, ITER>([&](auto it_) {
                 constexpr int it = decltype(it_)::value;
                 int q, l;
                 split<AX, mA, W>(gt + it * NTG, q, l);
                 cx<T> v[RA];
-                inv_level_regs<RA, T>(q, mA, tb.twA + q, [&](int row) { return S[row * RS + l]; }, v);
+                inv_level_regs<RA, T>(q, mA, tb.twA + q, [&](int row) { return S[L::idx(row, l)]; }, v);
                 static_for<0, RA>([&](auto r_) {
                     constexpr int r = decltype(r_)::value;
                     stv(psi + tile.at(q + mA * r, l), v[r]);
@@ -293,7 +300,7 @@ struct PsiK {
                 split<AX, mA, W>(gt + it * NTG, q, l);
                 static_for<0, RA>([&](auto r_) {
                     constexpr int r = decltype(r_)::value;
-                    cx<T> v = S[(q + mA * r) * RS + l];
+                    cx<T> v = S[L::idx(q + mA * r, l)];
                     rho[it][r] = v.x * v.x + v.y * v.y;
                 });
             });
@@ -327,7 +334,7 @@ struct PsiK {
                                  [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
             }
             group_sync(grp, NTG);
-            g_fwd_B<C, WP, RSP, T>(Sp, tb.twB, gt, grp);
+            g_fwd_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return row * RSP + l; });
             for (int b = gt; b < (N / RM) * WP; b += NTG) {
                 int l = b % WP, g = b / WP;
                 mid_fwd<RM, T>(g * RM, [&](int row) { return Sp[row * RSP + l]; },
@@ -355,8 +362,9 @@ struct HK {
     using T = typename C::T;
     static constexpr int AX = (MODE == H_Z_GREEN) ? AX_CONTIG : AX_STRIDED;
     using TL = Tile<C, AX>;
-    static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA, RS = TL::RS;
-    static constexpr size_t TILE_BYTES = align128((size_t)N * RS * sizeof(cx<T>));
+    using L = Lay<C, AX>;
+    static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA;
+    static constexpr size_t TILE_BYTES = align128(L::ELEMS * sizeof(cx<T>));
     static constexpr int AUX = MODE == H_Z_GREEN ? AUX_KSQ : AUX_NONE;
     using Pre = NoPre;
     static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
@@ -370,8 +378,9 @@ struct HK {
         cx<T> *S = reinterpret_cast<cx<T> *>(buf);
         const TL tile(p, t);
         cx<T> *H = p.data;
-        auto ldS = [&](int l) { return [S, l](int row) { return S[row * RS + l]; }; };
-        auto stS = [&](int l) { return [S, l](int row, cx<T> v) { S[row * RS + l] = v; }; };
+        auto ldS = [&](int l) { return [S, l](int row) { return S[L::idx(row, l)]; }; };
+        auto stS = [&](int l) { return [S, l](int row, cx<T> v) { S[L::idx(row, l)] = v; }; };
+        auto idx = [](int row, int l) { return L::idx(row, l); };
         if constexpr (MODE == H_Y_FWD || MODE == H_Z_GREEN) {
             for (int b = gt; b < mA * W; b += NTG) {
                 int q, l;
@@ -379,7 +388,7 @@ struct HK {
                 fwd_level<RA, T>(q, mA, tb.twA + q, ldS(l), stS(l));
             }
             group_sync(grp, NTG);
-            g_fwd_B<C, W, RS, T>(S, tb.twB, gt, grp);
+            g_fwd_B<C, W>(S, tb.twB, gt, grp, idx);
         }
         if constexpr (MODE == H_Y_FWD) {
             for (int b = gt; b < (N / RM) * W; b += NTG) {
@@ -394,14 +403,19 @@ struct HK {
                 int pen = t * W + l, kx = pen / N, ypos = pen - kx * N;
                 T kxy = ldg(p.ksq_nat + kx) + tb.ksq_pos[ypos];
                 bool zero_line = (kx == 0 && ypos == 0);
-                mid_both<RM, T>(g * RM, ldS(l), stS(l), [&](int pos, cx<T> v) {
+                auto mul = [&](int pos, cx<T> v) {
                     T k2 = kxy + tb.ksq_pos[pos];
                     T gr = (zero_line && pos == 0) ? (T)0 : p.green / k2;
                     return cscale(v, gr);
-                });
+                };
+                if constexpr (L::VEC2)
+                    mid_both2<RM, T>(g * RM, [&](int row, cx<T> &a, cx<T> &c) { ld2(S + L::idx(row, l), a, c); },
+                                     [&](int row, cx<T> a, cx<T> c) { st2(S + L::idx(row, l), a, c); }, mul);
+                else
+                    mid_both<RM, T>(g * RM, ldS(l), stS(l), mul);
             }
             group_sync(grp, NTG);
-            g_inv_B<C, W, RS, T>(S, tb.twB, gt, grp);
+            g_inv_B<C, W>(S, tb.twB, gt, grp, idx);
         }
         if constexpr (MODE == H_Y_INV) {
             for (int b = gt; b < (N / RM) * W; b += NTG) {
@@ -409,7 +423,7 @@ struct HK {
                 mid_inv<RM, T>(g * RM, ldS(l), stS(l));
             }
             group_sync(grp, NTG);
-            g_inv_B<C, W, RS, T>(S, tb.twB, gt, grp);
+            g_inv_B<C, W>(S, tb.twB, gt, grp, idx);
         }
         if constexpr (MODE == H_Y_INV || MODE == H_Z_GREEN) {
             for (int b = gt; b < mA * W; b += NTG) {
@@ -463,7 +477,7 @@ struct C2RK {
                            [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
         }
         group_sync(grp, NTG);
-        g_inv_B<C, WP, RSP, T>(Sp, tb.twB, gt, grp);
+        g_inv_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return row * RSP + l; });
         for (int b = gt; b < mA * WP; b += NTG) {
             int l = b % WP, q = b / WP;
             inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; },
