@@ -35,6 +35,21 @@ struct alignas(2 * sizeof(T)) cx {
 template <typename T> WDM_HD cx<T> mk(T a, T b) { cx<T> r; r.x = a; r.y = b; return r; }
 template <typename T> WDM_HD cx<T> cadd(cx<T> a, cx<T> b) { return mk<T>(a.x + b.x, a.y + b.y); }
 template <typename T> WDM_HD cx<T> csub(cx<T> a, cx<T> b) { return mk<T>(a.x - b.x, a.y - b.y); }
+#if defined(__CUDA_ARCH__) && __CUDA_ARCH__ >= 1000 && !defined(WDM_NO_PACKED_ADD)
+// sm_100 packed single precision: one issue slot for a complex add
+__device__ __forceinline__ cx<float> cadd(cx<float> a, cx<float> b)
+{
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(*reinterpret_cast<unsigned long long *>(&a)), "l"(*reinterpret_cast<unsigned long long *>(&b)));
+    return *reinterpret_cast<cx<float> *>(&r);
+}
+__device__ __forceinline__ cx<float> csub(cx<float> a, cx<float> b)
+{
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(*reinterpret_cast<unsigned long long *>(&a)), "l"(*reinterpret_cast<unsigned long long *>(&b)));
+    return *reinterpret_cast<cx<float> *>(&r);
+}
+#endif
 // a * b
 template <typename T> WDM_HD cx<T> cmul(cx<T> a, cx<T> b) { return mk<T>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 // a * conj(b)
