@@ -121,6 +121,21 @@ class ClockSampler:
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+def max_over_ranks(x: float, dist, device) -> float:
+    """MAX all-reduce of a per-rank scalar (the only collective of the bench: timing, never data)."""
+    if dist is None:
+        return x
+    import torch
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(cells_per_rank: int, steps: int, world: int, ms_max: float) -> float:
+    """whole-job throughput of `world` independent replicas: all ranks' cell updates / slowest rank's time"""
+    return world * cells_per_rank * steps / (ms_max * 1e-3)
+
+
 def oracle_rate(sample_name: str, steps: int, warmup: int):
     """cells/s of the CPU oracle on the named sample: `warmup` untimed then `steps` timed KDK steps."""
     import oracle
@@ -215,11 +230,8 @@ def main():
         barrier()
     ms = e0.elapsed_time(e1)
     launches = wdm.wdm_launch_count(sim.h) - l0
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * (N ** 3) * K / (ms * 1e-3)
+    ms = max_over_ranks(ms, dist, "cuda")
+    value = aggregate_value(N ** 3, K, world, ms)
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -269,10 +281,7 @@ def main():
         t0 = time.perf_counter()
         wdm.wdm_run_host(sim.h, psi_host, ke, dt, out_host)     # synchronises before returning
         el = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([el], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            el = float(t.item())
+        el = max_over_ranks(el, dist, "cuda")
         nbytes = psi_host.numel() * psi_host.element_size()
         out["e2e"] = {"value": world * N ** 3 * ke / el, "unit": UNIT, "h2d_bytes_per_step": nbytes / ke,
                       "d2h_bytes_per_step": nbytes / ke, "call": f"wdm_run_host(psi_in, {ke}, dt, psi_out)",

@@ -204,6 +204,25 @@ __device__ __forceinline__ void g_inv_B(cx<T> *S, const cx<T> *twB, int gt, int 
     }
 }
 
+// Frequencies k < N/2 enumerated so that consecutive indices sit in consecutive shared-memory rows
+// (k = sA + RA (sB + RB sM) lives at row (sA RB + sB) RM + sM; k < N/2 <=> sM < RM/2).  Returns k and its row;
+// row_of(k) gives the row of any frequency.  All divisors are powers of two.
+template <class C>
+struct HalfSpec {
+    static constexpr int HM = C::RM / 2;
+    static __device__ __forceinline__ int row_of(int k)
+    {
+        int sA = k % C::RA, sB = (k / C::RA) % C::RB, sM = k / (C::RA * C::RB);
+        return (sA * C::RB + sB) * C::RM + sM;
+    }
+    static __device__ __forceinline__ void nth(int kk, int &k, int &row)
+    {
+        int sM = kk % HM, sAB = kk / HM, sA = sAB / C::RB, sB = sAB % C::RB;
+        k = sA + C::RA * (sB + C::RB * sM);
+        row = sAB * C::RM + sM;
+    }
+};
+
 struct NoPre {};
 
 constexpr size_t align128(size_t x) { return (x + 127) & ~(size_t)127; }
@@ -342,15 +361,20 @@ struct PsiK {
             }
             group_sync(grp, NTG);
             // Hermitian split of Z = FFT(a + i b):  A_k = (Z_k + conj Z_{N-k})/2,  B_k = (Z_k - conj Z_{N-k})/(2i)
-            for (int b = gt; b < (N / 2 + 1) * WP; b += NTG) {
-                int l = b % WP, k = b / WP;
-                int pk = ldg(p.pos_of_k + k), pn = ldg(p.pos_of_k + ((N - k) & (N - 1)));
+            auto emit = [&](int k, int pk, int l) {
+                int pn = HalfSpec<C>::row_of((N - k) & (N - 1));
                 cx<T> zk = Sp[pk * RSP + l], zn = Sp[pn * RSP + l];
                 const T h = (T)0.5;
                 cx<T> A = mk<T>((zk.x + zn.x) * h, (zk.y - zn.y) * h);
                 cx<T> B = mk<T>((zk.y + zn.y) * h, (zn.x - zk.x) * h);
                 st2(p.H + tile.at(k, 2 * l), A, B);
+            };
+            for (int b = gt; b < (N / 2) * WP; b += NTG) {
+                int l = b % WP, k, pk;
+                HalfSpec<C>::nth(b / WP, k, pk);
+                emit(k, pk, l);
             }
+            if (gt < WP) emit(N / 2, HalfSpec<C>::row_of(N / 2), gt);
         }
     }
 };
@@ -460,16 +484,18 @@ struct C2RK {
         const cx<T> *R = reinterpret_cast<const cx<T> *>(buf + PACKED_BYTES);
         const TL tile(p, t);
         // Z_k = A_k + i B_k,  Z_{N-k} = conj(A_k) + i conj(B_k)
-        for (int b = gt; b < (N / 2 + 1) * WP; b += NTG) {
-            int l = b % WP, k = b / WP;
-            cx<T> A = R[k * W + 2 * l], B = R[k * W + 2 * l + 1];
-            int pk = ldg(p.pos_of_k + k);
+        auto place = [&](int k, int pk, int l) {
+            cx<T> A, B;
+            ld2(R + k * W + 2 * l, A, B);
             Sp[pk * RSP + l] = mk<T>(A.x - B.y, A.y + B.x);
-            if (k > 0 && k < N / 2) {
-                int pn = ldg(p.pos_of_k + (N - k));
-                Sp[pn * RSP + l] = mk<T>(A.x + B.y, B.x - A.y);
-            }
+            if (k > 0 && k < N / 2) Sp[HalfSpec<C>::row_of(N - k) * RSP + l] = mk<T>(A.x + B.y, B.x - A.y);
+        };
+        for (int b = gt; b < (N / 2) * WP; b += NTG) {
+            int l = b % WP, k, pk;
+            HalfSpec<C>::nth(b / WP, k, pk);
+            place(k, pk, l);
         }
+        if (gt < WP) place(N / 2, HalfSpec<C>::row_of(N / 2), gt);
         group_sync(grp, NTG);
         for (int b = gt; b < (N / RM) * WP; b += NTG) {
             int l = b % WP, g = b / WP;
