@@ -39,6 +39,8 @@ UNIT = "cell-updates/s"
 ALG_BYTES_PER_CELL_C = {
     "psi_sweep_z_kick": 2.5, "psi_sweep_y": 2.0, "psi_sweep_x_rho_r2c": 2.5,
     "poisson_y_fwd": 1.0, "poisson_z_green": 1.0, "poisson_y_inv": 1.0, "poisson_x_c2r": 1.0,
+    # L2-chained kernels: what must cross HBM is the first stage's read and the last stage's write
+    "psi_chain_z_kick_y": 2.5, "poisson_chain_y_zgreen_y": 1.0,
 }
 
 
@@ -241,6 +243,7 @@ def main():
                    "particles": npart, "dt": dt, "timed_call": f"wdm_step({K}, dt)",
                    "l2": "inputs larger than L2 (psi alone is %.2f GB vs 126 MB L2), no flush" % (N ** 3 * 8 / 1e9)
                          if N >= 512 else "working set near/below L2: L2-resident, launch-bound regime",
+                   "chain_lag_planes": list(wdm.wdm_get_chain(sim.h)),
                    "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU"},
         "gpu_launches": launches, "clocks": clk.summary(),
     }
@@ -260,6 +263,7 @@ def main():
         dom = max((k for k in kern if k in ALG_BYTES_PER_CELL_C), key=lambda k: kern[k]["launches"] * kern[k]["avg_ms"])
         peak, how = peaks()
         alg = ALG_BYTES_PER_CELL_C[dom] * csize * N ** 3
+        step_min = sum(ALG_BYTES_PER_CELL_C[k] for k in kern if k in ALG_BYTES_PER_CELL_C and kern[k]["launches"] >= kp) * csize * N ** 3
         achieved = alg / (kern[dom]["avg_ms"] * 1e-3) / 1e9
         traffic = None
         tp = os.path.join(ROOT, "profiles", "traffic.json")
@@ -271,7 +275,11 @@ def main():
                            "whole_step": {"alg_bytes_per_step": 11 * csize * N ** 3,
                                           "achieved": 11 * csize * N ** 3 / (ms / K * 1e-3) / 1e9,
                                           "frac": 11 * csize * N ** 3 / (ms / K * 1e-3) / 1e9 / peak,
-                                          "frac_of_nominal_8TBs": 11 * csize * N ** 3 / (ms / K * 1e-3) / 1e9 / 8000.0}}
+                                          "frac_of_nominal_8TBs": 11 * csize * N ** 3 / (ms / K * 1e-3) / 1e9 / 8000.0,
+                                          "note": "11c per cell = SURVEY 8(d) count for seven separate sweeps; "
+                                                  "hbm_min_* counts what the launched (chained) kernels must move",
+                                          "hbm_min_bytes_per_step": step_min,
+                                          "hbm_min_frac": step_min / (ms / K * 1e-3) / 1e9 / peak}}
         out["kernels"] = kern
 
         # ---- end to end through the C ABI with HOST buffers: copy in + K steps + copy out, wall clock

@@ -48,6 +48,7 @@ def lib():
             "wdm_get_psi_host": [vp, vp], "wdm_get_density_host": [vp, vp], "wdm_get_potential_host": [vp, vp],
             "wdm_get_particles_host": [vp, vp, vp],
             "wdm_launch_count": [vp, C.POINTER(ll)], "wdm_set_profiling": [vp, i],
+            "wdm_set_chain": [vp, i, i], "wdm_get_chain": [vp, C.POINTER(i), C.POINTER(i)],
             "wdm_kernel_stats": [vp, C.POINTER(i), C.POINTER(C.c_char_p), C.POINTER(ll), C.POINTER(d)],
         }
         for name, args in sig.items():
@@ -64,7 +65,7 @@ EXPORTS = ["wdm_workspace_bytes", "wdm_create", "wdm_create_ws", "wdm_destroy", 
            "wdm_set_psi_host", "wdm_set_particles", "wdm_set_particles_host", "wdm_step", "wdm_run_host",
            "wdm_get_psi", "wdm_get_density", "wdm_get_potential", "wdm_get_particles", "wdm_get_psi_host",
            "wdm_get_density_host", "wdm_get_potential_host", "wdm_get_particles_host", "wdm_launch_count",
-           "wdm_set_profiling", "wdm_kernel_stats", "wdm_last_error"]
+           "wdm_set_profiling", "wdm_kernel_stats", "wdm_last_error", "wdm_set_chain", "wdm_get_chain"]
 
 
 def _chk(rc, h=None):
@@ -172,6 +173,17 @@ def wdm_launch_count(h):
     out = C.c_longlong()
     _chk(lib().wdm_launch_count(h, C.byref(out)), h)
     return out.value
+
+
+def wdm_set_chain(h, mode, lag=0):
+    _chk(lib().wdm_set_chain(h, int(mode), int(lag)), h)
+
+
+def wdm_get_chain(h):
+    """(lag of the psi z->y chain, lag of the Poisson y->z->y chain) in x-planes; 0 = separate sweeps."""
+    a, b = C.c_int(), C.c_int()
+    _chk(lib().wdm_get_chain(h, C.byref(a), C.byref(b)), h)
+    return a.value, b.value
 
 
 def wdm_set_profiling(h, on):

@@ -9,6 +9,7 @@
 // and once at the end the closing half kick.  Nothing synchronises with the host.
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -87,11 +88,11 @@ __global__ void k_finish_mean(const double *acc, double inv_cells, double extra_
 }
 
 enum Slot { S_PSI_Z, S_PSI_Y, S_PSI_X_RHO, S_H_Y_FWD, S_H_Z_GREEN, S_H_Y_INV, S_C2R, S_KICK, S_PART_PUSH,
-            S_PART_DEPOSIT, S_PART_SORT, S_MISC, S_COUNT };
+            S_PART_DEPOSIT, S_PART_SORT, S_MISC, S_PSI_ZY, S_H_YZY, S_COUNT };
 static const char *kSlotNames[S_COUNT] = {"psi_sweep_z_kick", "psi_sweep_y", "psi_sweep_x_rho_r2c", "poisson_y_fwd",
                                           "poisson_z_green", "poisson_y_inv", "poisson_x_c2r", "kick_elementwise",
                                           "particle_gather_kick_drift", "particle_cic_deposit", "particle_cell_sort",
-                                          "misc"};
+                                          "misc", "psi_chain_z_kick_y", "poisson_chain_y_zgreen_y"};
 
 }  // namespace wdm
 
@@ -114,6 +115,10 @@ struct wdm_ctx {
     unsigned short *pos_of_k = nullptr;
     double phase_dt = 0;
     bool phase_valid = false, have_psi = false, stale = true;
+    // L2-chained sweeps (wdm_chain.cuh): completion counters, launch epochs, lag per chain (0: separate sweeps)
+    unsigned int *chain_done = nullptr;       // [N] for psi z->y, then [2 (N/2+1)] for H y->z->y
+    unsigned int epoch_psi = 0, epoch_h = 0;
+    int lag_psi = 0, lag_h = 0;
     ParticleState part;
     long long max_particles = -1;   // -1: unbounded (cudaMalloc on demand)
     // instrumentation
@@ -156,6 +161,7 @@ static size_t grid_bytes(int N, int dtype, long long max_particles)
     size_t n = (size_t)N * N * N, nH = (size_t)(N / 2 + 1) * N * N, c = csize(dtype), r = rsize(dtype);
     size_t b = align_up(n * c) + align_up(n * r) + align_up(nH * c);
     b += 3 * align_up((size_t)N * c) + 2 * align_up((size_t)N * r) + align_up((size_t)N * 2) + 256;
+    b += align_up((size_t)(2 * N + 2) * sizeof(unsigned int));
     if (max_particles > 0) b += align_up(n * r) + particle_bytes(N, dtype, max_particles);
     return b + 4096;
 }
@@ -280,9 +286,15 @@ static int density_poisson(wdm_ctx *c, bool drift)
     }
     SweepParams<T> p = base_params<T>(c);
     p.data = (cx<T> *)c->H; p.rowStride = N; p.outerStride = N * N;
-    { Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
-    { Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
-    { Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
+    if (c->lag_h > 0) {
+        ChainCtl ctl{c->chain_done + N, ++c->epoch_h * (unsigned int)(N / c->tab->fact.W), c->lag_h};
+        Timed t(c, S_H_YZY);
+        CU(c, c->tab->h_yzy(&p, &p, &ctl, c->stream));
+    } else {
+        { Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
+        { Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
+        { Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
+    }
     p.rowStride = N * N; p.outerStride = N;
     { Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, c->stream)); }
     return WDM_OK;
@@ -347,17 +359,18 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             if (grav) { rc = particles_deposit<T>(c); if (rc) return rc; }
         }
         {
-            SweepParams<T> p = base_params<T>(c);
-            p.data = (cx<T> *)c->psi;
-            p.kick = (T)(kdt / c->mu);
-            Timed t(c, S_PSI_Z);
-            CU(c, c->tab->psi_z(&p, grav ? 1 : 0, c->stream));
-        }
-        {
-            SweepParams<T> p = base_params<T>(c);
-            p.data = (cx<T> *)c->psi; p.rowStride = N; p.outerStride = N * N;
-            Timed t(c, S_PSI_Y);
-            CU(c, c->tab->psi_strided(&p, c->stream));
+            SweepParams<T> pz = base_params<T>(c), py = base_params<T>(c);
+            pz.data = (cx<T> *)c->psi;
+            pz.kick = (T)(kdt / c->mu);
+            py.data = (cx<T> *)c->psi; py.rowStride = N; py.outerStride = N * N;
+            if (c->lag_psi > 0) {
+                ChainCtl ctl{c->chain_done, ++c->epoch_psi * (unsigned int)(N / c->tab->fact.W), c->lag_psi};
+                Timed t(c, S_PSI_ZY);
+                CU(c, c->tab->psi_zy(&pz, &py, grav ? 1 : 0, &ctl, c->stream));
+            } else {
+                { Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, grav ? 1 : 0, c->stream)); }
+                { Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, c->stream)); }
+            }
         }
         if (grav) {
             rc = density_poisson<T>(c, true);
@@ -435,8 +448,20 @@ static int create_common(wdm_ctx **out, int N, double L, double mu, double G, in
         (rc = ctx_alloc(c, &c->H, c->nH * cs)) || (rc = ctx_alloc(c, &c->twA, N * cs)) ||
         (rc = ctx_alloc(c, &c->twB, N * cs)) || (rc = ctx_alloc(c, &c->phase, N * cs)) ||
         (rc = ctx_alloc(c, &c->ksq_pos, N * rs)) || (rc = ctx_alloc(c, &c->ksq_nat, N * rs)) ||
-        (rc = ctx_alloc(c, (void **)&c->pos_of_k, N * 2)) || (rc = ctx_alloc(c, &c->rho_mean, 64)))
+        (rc = ctx_alloc(c, (void **)&c->pos_of_k, N * 2)) || (rc = ctx_alloc(c, &c->rho_mean, 64)) ||
+        (rc = ctx_alloc(c, (void **)&c->chain_done, (size_t)(2 * N + 2) * sizeof(unsigned int))))
         return bail(rc);
+    if (cudaMemset(c->chain_done, 0, (size_t)(2 * N + 2) * sizeof(unsigned int)) != cudaSuccess)
+        return bail(fail(c, WDM_ECUDA, "cudaMemset of the chain counters failed"));
+    {
+        const char *env = getenv("WDM_CHAIN");             // 1: chained sweeps; unset/0: one launch per sweep
+        const char *lag = getenv("WDM_CHAIN_LAG");
+        int req = lag ? atoi(lag) : 0;
+        if (env && atoi(env) != 0) {
+            c->lag_psi = c->tab->chain_lag(2, N, req);
+            c->lag_h = c->tab->chain_lag(3, N / 2 + 1, req);
+        }
+    }
     rc = dtype == WDM_C64 ? upload_tables<float>(c) : upload_tables<double>(c);
     if (rc) return bail(rc);
     if (!owns && max_particles > 0) {
@@ -595,6 +620,23 @@ extern "C" int wdm_launch_count(wdm_ctx *c, long long *out)
 {
     if (!c || !out) return WDM_EINVAL;
     *out = c->launches;
+    return WDM_OK;
+}
+
+extern "C" int wdm_set_chain(wdm_ctx *c, int mode, int lag)
+{
+    if (!c) return WDM_EINVAL;
+    if (mode != 0 && mode != 1) return fail(c, WDM_EINVAL, "mode must be 0 (separate sweeps) or 1 (chained)");
+    c->lag_psi = mode ? c->tab->chain_lag(2, c->N, lag) : 0;
+    c->lag_h = mode ? c->tab->chain_lag(3, c->N / 2 + 1, lag) : 0;
+    return WDM_OK;
+}
+
+extern "C" int wdm_get_chain(wdm_ctx *c, int *lag_psi_out, int *lag_poisson_out)
+{
+    if (!c) return WDM_EINVAL;
+    if (lag_psi_out) *lag_psi_out = c->lag_psi;
+    if (lag_poisson_out) *lag_poisson_out = c->lag_h;
     return WDM_OK;
 }
 

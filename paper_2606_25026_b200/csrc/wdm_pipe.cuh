@@ -136,7 +136,9 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
         while (issued[b] < j / NBUF + 1) __nanosleep(64);
         mbar_wait(full + b, (j / NBUF) & 1);
         const int jn = j + NG;
-        K::compute(p, tb, bid + j * stride, jn < J ? bid + jn * stride : -1, buf, gt, grp, pre);
+        // called by compute() before its last stage: fetch what the group's NEXT tile needs into registers
+        auto hook = [&]() { if (jn < J) K::prefetch(p, bid + jn * stride, gt, pre); };
+        K::compute(p, tb, bid + j * stride, buf, gt, grp, pre, hook);
         group_sync(grp, NTG);                                   // every read of this buffer is done
         if (j + NBUF < J) {
             if (gt == 0) issued[b] = (j + NBUF) / NBUF + 1;
@@ -266,8 +268,9 @@ struct PsiK {
             });
         }
     }
-    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, int tnext, unsigned char *buf, int gt,
-                                                   int grp, Pre &pre)
+    template <class HOOK>
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt,
+                                                   int grp, Pre &pre, HOOK &&hook)
     {
         cx<T> *S = reinterpret_cast<cx<T> *>(buf);
         const TL tile(p, t);
@@ -299,7 +302,7 @@ struct PsiK {
             }
             group_sync(grp, NTG);
             g_inv_B<C, W>(S, tb.twB, gt, grp, idx);
-            if (KICK && tnext >= 0) prefetch(p, tnext, gt, pre);
+            hook();
             static_for<0, ITER>([&](auto it_) {
                 constexpr int it = decltype(it_)::value;
                 int q, l;
@@ -397,7 +400,8 @@ struct HK {
         issue_tile<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, tile, gt);
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
-    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, int, unsigned char *buf, int gt, int grp, Pre &)
+    template <class HOOK>
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &, HOOK &&)
     {
         cx<T> *S = reinterpret_cast<cx<T> *>(buf);
         const TL tile(p, t);
@@ -478,7 +482,8 @@ struct C2RK {
         issue_tile<C, AX_STRIDED, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf + PACKED_BYTES), p.H, tile, gt);
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
-    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, int, unsigned char *buf, int gt, int grp, Pre &)
+    template <class HOOK>
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &, HOOK &&)
     {
         cx<T> *Sp = reinterpret_cast<cx<T> *>(buf);
         const cx<T> *R = reinterpret_cast<const cx<T> *>(buf + PACKED_BYTES);
