@@ -262,7 +262,6 @@ static SweepParams<T> base_params(wdm_ctx *c)
     p.ksq_pos = (const T *)c->ksq_pos;
     p.ksq_nat = (const T *)c->ksq_nat;
     p.green = (T)(-4.0 * M_PI * c->G / ((double)N * N * N));
-    p.tilesInner = N / c->tab->fact.W;
     p.H = (cx<T> *)c->H;
     p.phi = (const T *)c->phi;
     p.phi_out = (T *)c->phi;
@@ -280,12 +279,12 @@ static int density_poisson(wdm_ctx *c, bool drift)
     const long long N = c->N;
     {
         SweepParams<T> p = base_params<T>(c);
-        p.data = (cx<T> *)c->psi; p.rowStride = N * N; p.outerStride = N;
+        p.data = (cx<T> *)c->psi;
         Timed t(c, S_PSI_X_RHO);
         CU(c, c->tab->psi_x_rho(&p, drift ? 1 : 0, c->stream));
     }
     SweepParams<T> p = base_params<T>(c);
-    p.data = (cx<T> *)c->H; p.rowStride = N; p.outerStride = N * N;
+    p.data = (cx<T> *)c->H;
     if (c->lag_h > 0) {
         ChainCtl ctl{c->chain_done + N, ++c->epoch_h * (unsigned int)(N / c->tab->fact.W), c->lag_h};
         Timed t(c, S_H_YZY);
@@ -295,7 +294,6 @@ static int density_poisson(wdm_ctx *c, bool drift)
         { Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
         { Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
     }
-    p.rowStride = N * N; p.outerStride = N;
     { Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, c->stream)); }
     return WDM_OK;
 }
@@ -362,14 +360,14 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             SweepParams<T> pz = base_params<T>(c), py = base_params<T>(c);
             pz.data = (cx<T> *)c->psi;
             pz.kick = (T)(kdt / c->mu);
-            py.data = (cx<T> *)c->psi; py.rowStride = N; py.outerStride = N * N;
+            py.data = (cx<T> *)c->psi;
             if (c->lag_psi > 0) {
                 ChainCtl ctl{c->chain_done, ++c->epoch_psi * (unsigned int)(N / c->tab->fact.W), c->lag_psi};
                 Timed t(c, S_PSI_ZY);
                 CU(c, c->tab->psi_zy(&pz, &py, grav ? 1 : 0, &ctl, c->stream));
             } else {
                 { Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, grav ? 1 : 0, c->stream)); }
-                { Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, c->stream)); }
+                { Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
             }
         }
         if (grav) {
@@ -377,9 +375,9 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             if (rc) return rc;
         } else {
             SweepParams<T> p = base_params<T>(c);
-            p.data = (cx<T> *)c->psi; p.rowStride = N * N; p.outerStride = N;
+            p.data = (cx<T> *)c->psi;
             Timed t(c, S_PSI_Y);
-            CU(c, c->tab->psi_strided(&p, c->stream));
+            CU(c, c->tab->psi_strided(&p, 1, c->stream));
         }
     }
     if (grav) {
@@ -454,13 +452,12 @@ static int create_common(wdm_ctx **out, int N, double L, double mu, double G, in
     if (cudaMemset(c->chain_done, 0, (size_t)(2 * N + 2) * sizeof(unsigned int)) != cudaSuccess)
         return bail(fail(c, WDM_ECUDA, "cudaMemset of the chain counters failed"));
     {
-        const char *env = getenv("WDM_CHAIN");             // 1: chained sweeps; unset/0: one launch per sweep
+        const char *env = getenv("WDM_CHAIN");             // bit mask as in wdm_set_chain; unset/0: one launch per sweep
         const char *lag = getenv("WDM_CHAIN_LAG");
         int req = lag ? atoi(lag) : 0;
-        if (env && atoi(env) != 0) {
-            c->lag_psi = c->tab->chain_lag(2, N, req);
-            c->lag_h = c->tab->chain_lag(3, N / 2 + 1, req);
-        }
+        int mode = env ? atoi(env) : 0;
+        if (mode & 1) c->lag_psi = c->tab->chain_lag(2, N, req);
+        if (mode & 2) c->lag_h = c->tab->chain_lag(3, N / 2 + 1, req);
     }
     rc = dtype == WDM_C64 ? upload_tables<float>(c) : upload_tables<double>(c);
     if (rc) return bail(rc);
@@ -626,9 +623,9 @@ extern "C" int wdm_launch_count(wdm_ctx *c, long long *out)
 extern "C" int wdm_set_chain(wdm_ctx *c, int mode, int lag)
 {
     if (!c) return WDM_EINVAL;
-    if (mode != 0 && mode != 1) return fail(c, WDM_EINVAL, "mode must be 0 (separate sweeps) or 1 (chained)");
-    c->lag_psi = mode ? c->tab->chain_lag(2, c->N, lag) : 0;
-    c->lag_h = mode ? c->tab->chain_lag(3, c->N / 2 + 1, lag) : 0;
+    if (mode < 0 || mode > 3) return fail(c, WDM_EINVAL, "mode is a bit mask: 1 = chain the psi z/y sweeps, 2 = chain the Poisson y/z/y sweeps");
+    c->lag_psi = (mode & 1) ? c->tab->chain_lag(2, c->N, lag) : 0;
+    c->lag_h = (mode & 2) ? c->tab->chain_lag(3, c->N / 2 + 1, lag) : 0;
     return WDM_OK;
 }
 

@@ -167,14 +167,24 @@ WDM_HD void dit_inv(cx<T> (&v)[R])
 
 // DIF level: rows rowbase + m*r -> butterfly -> twiddle -> rows rowbase + m*s (natural digit order).
 // The _regs form takes the R inputs already in registers (so the caller can issue all loads first).
+// The twiddles are fetched into registers BEFORE the butterfly when they fit (R complex values of at most
+// 64 bytes' worth of registers... R * sizeof(T) <= 64): a table load placed after the first st() cannot be moved
+// above it by the compiler (both may be shared memory), so loading on demand puts one exposed shared-memory
+// latency in front of every output.
 template <int R, typename T, class ST>
 WDM_HD void fwd_level_regs(cx<T> (&v)[R], int rowbase, int m, const cx<T> *tw, ST &&st)
 {
+    constexpr bool PRE = R * sizeof(T) <= 64;
+    cx<T> w[PRE ? R : 1];
+    if constexpr (PRE) static_for<1, R>([&](auto s_) { constexpr int s = decltype(s_)::value; w[s] = tw[s * m]; });
     dif_fwd<R>(v);
     static_for<0, R>([&](auto s_) {
         constexpr int s = decltype(s_)::value;
         cx<T> y = v[brev(s, R)];
-        if constexpr (s > 0) y = cmul(y, tw[s * m]);
+        if constexpr (s > 0) {
+            if constexpr (PRE) y = cmul(y, w[s]);
+            else y = cmul(y, tw[s * m]);
+        }
         st(rowbase + m * s, y);
     });
 }

@@ -20,7 +20,7 @@ struct SweepTable {
     int dtype;
     cudaError_t (*init)();                                               // opt in to > 48 KB dynamic shared memory
     cudaError_t (*psi_z)(const void *params, int kick, cudaStream_t);    // contiguous axis, optional kick on load
-    cudaError_t (*psi_strided)(const void *params, cudaStream_t);        // y axis (or x axis when G = 0)
+    cudaError_t (*psi_strided)(const void *params, int along_x, cudaStream_t);  // y axis (or x axis when G = 0)
     cudaError_t (*psi_x_rho)(const void *params, int drift, cudaStream_t);  // x axis + density + R2C -> H
     cudaError_t (*h_y_fwd)(const void *params, cudaStream_t);
     cudaError_t (*h_z_green)(const void *params, cudaStream_t);

@@ -26,7 +26,11 @@ WDM_DEV double ldg(const double *p) { return __ldg(p); }
 WDM_DEV unsigned short ldg(const unsigned short *p) { return __ldg(p); }
 WDM_DEV cx<float> ldv(const cx<float> *p) { float2 t = *reinterpret_cast<const float2 *>(p); return mk<float>(t.x, t.y); }
 WDM_DEV cx<double> ldv(const cx<double> *p) { double2 t = *reinterpret_cast<const double2 *>(p); return mk<double>(t.x, t.y); }
-WDM_DEV void stv(cx<float> *p, cx<float> v) { *reinterpret_cast<float2 *>(p) = make_float2(v.x, v.y); }
+// (inline PTX: with the plain float2 store ptxas copies already-adjacent register pairs into one scratch pair
+// store after store, serialising them on its write-after-read scoreboard.  No "memory" clobber: volatile asm
+// statements keep their order among themselves -- barriers, async copies -- and shared-memory accesses may
+// still be scheduled across a global store)
+WDM_DEV void stv(cx<float> *p, cx<float> v) { asm volatile("st.global.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.x), "f"(v.y)); }
 WDM_DEV void stv(cx<double> *p, cx<double> v) { *reinterpret_cast<double2 *>(p) = make_double2(v.x, v.y); }
 WDM_DEV void ld2(const cx<float> *p, cx<float> &a, cx<float> &b) { float4 t = *reinterpret_cast<const float4 *>(p); a = mk<float>(t.x, t.y); b = mk<float>(t.z, t.w); }
 WDM_DEV void st2(cx<float> *p, cx<float> a, cx<float> b) { *reinterpret_cast<float4 *>(p) = make_float4(a.x, a.y, b.x, b.y); }
@@ -34,18 +38,27 @@ WDM_DEV void ld2(const cx<double> *p, cx<double> &a, cx<double> &b) { a = ldv(p)
 WDM_DEV void st2(cx<double> *p, cx<double> a, cx<double> b) { stv(p, a); stv(p + 1, b); }
 
 // psi * exp(-i theta).  |theta| = |Phi| dt/(2 mu) is far below 1 under the CFL limit (Eq. 26),
-// so the single-precision path takes the Taylor branch (truncation error < 1e-11 for |theta| < 1/4, below
-// float rounding) and falls back to sincosf only for large phases.
+// so the single-precision path takes a Taylor branch (sin to theta^7, cos to theta^8: truncation below
+// 4e-10 for |theta| < 1/4, under float rounding) and falls back to sincosf only for large phases.
+WDM_DEV void sincos_small(float th, float &s, float &c)
+{
+    float t2 = th * th;
+    s = th * fmaf(t2, fmaf(t2, fmaf(t2, -1.0f / 5040.0f, 1.0f / 120.0f), -1.0f / 6.0f), 1.0f);
+    c = fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, 1.0f / 40320.0f, -1.0f / 720.0f), 1.0f / 24.0f), -0.5f), 1.0f);
+}
+// large phases are rare: keep the full-range sincosf (with its Payne-Hanek reduction) out of line so the hot
+// code stays small and straight
+static __device__ __noinline__ float2 sincos_large(float th)
+{
+    float s, c;
+    sincosf(th, &s, &c);
+    return make_float2(s, c);
+}
 WDM_DEV cx<float> rotate_neg(cx<float> v, float th)
 {
     float s, c;
-    if (fabsf(th) < 0.25f) {
-        float t2 = th * th;
-        s = th * fmaf(t2, fmaf(t2, fmaf(t2, -1.0f / 5040.0f, 1.0f / 120.0f), -1.0f / 6.0f), 1.0f);
-        c = fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, 1.0f / 40320.0f, -1.0f / 720.0f), 1.0f / 24.0f), -0.5f), 1.0f);
-    } else {
-        sincosf(th, &s, &c);
-    }
+    if (fabsf(th) < 0.25f) sincos_small(th, s, c);
+    else { float2 sc = sincos_large(th); s = sc.x; c = sc.y; }
     return mk<float>(v.x * c + v.y * s, v.y * c - v.x * s);
 }
 WDM_DEV cx<double> rotate_neg(cx<double> v, double th)
@@ -54,15 +67,16 @@ WDM_DEV cx<double> rotate_neg(cx<double> v, double th)
     sincos(th, &s, &c);
     return mk<double>(v.x * c + v.y * s, v.y * c - v.x * s);
 }
+// g / k2 of the Green's function (Eq. 23).  Single precision: one reciprocal (MUFU.RCP, 1 ulp)
+// and a multiply instead of the IEEE division sequence -- 2 ulp on a factor whose tolerance is 2e-5.
+WDM_DEV float green_over(float g, float k2) { return __fdividef(g, k2); }
+WDM_DEV double green_over(double g, double k2) { return g / k2; }
 
 // ---------------------------------------------------------------- parameters
 
 template <typename T>
 struct SweepParams {
     cx<T> *data;               // psi (N^3) or H ((N/2+1) N^2), transformed in place
-    long long rowStride;       // strided sweeps: elements between consecutive points of the axis
-    long long outerStride;     // strided sweeps: elements between consecutive "outer" tiles
-    int tilesInner;            // strided sweeps: tiles along the contiguous (z) direction = N / W
     const cx<T> *twA;          // level-A twiddles, s-major: twA[s*mA + q] = exp(-2 pi i q s / N)
     const cx<T> *twB;          // level-B twiddles, s-major over the sub-block
     const cx<T> *phase;        // psi sweeps: exp(-i mu k^2 dt/2)/N in position order
@@ -78,7 +92,10 @@ struct SweepParams {
     T green;                   // Green: -4 pi G / N^3
 };
 
-enum { AX_STRIDED = 0, AX_CONTIG = 1 };
+// Axis of a sweep over an array [x][y][z] (z contiguous).  The strides are compile-time constants of the
+// instantiation (N is), so every global address of a tile is one 64-bit base plus an immediate offset.
+enum { AX_Y = 0, AX_CONTIG = 1, AX_X = 2 };
+constexpr bool ax_strided(int ax) { return ax != AX_CONTIG; }
 
 // Shared-memory layout of a tile (row = position along the transformed axis, l = line).
 //   strided axis   : [row][l], row stride W  -- a half-warp (complex64) reads one whole 128-byte row, so a
@@ -100,22 +117,22 @@ struct Lay {
 
 template <class C, int AX>
 struct Tile {
-    long long base, rstride, lstride;
+    static constexpr long long N = C::N;
+    static constexpr long long RSTRIDE = AX == AX_Y ? N : (AX == AX_X ? N * N : 1);   // between points of the axis
+    static constexpr long long LSTRIDE = AX == AX_CONTIG ? N : 1;                      // between lines of the tile
+    static constexpr int INNER = C::N / C::W;                                          // strided: tiles along z
+    long long base;
     template <typename T>
-    WDM_DEV Tile(const SweepParams<T> &p, int bid)
+    WDM_DEV Tile(const SweepParams<T> &, int bid)
     {
-        if (AX == AX_STRIDED) {
-            int outer = bid / p.tilesInner, inner = bid - outer * p.tilesInner;
-            base = (long long)outer * p.outerStride + (long long)inner * C::W;
-            rstride = p.rowStride;
-            lstride = 1;
-        } else {
+        if (AX == AX_CONTIG) {
             base = (long long)bid * C::W * C::N;
-            rstride = 1;
-            lstride = C::N;
+        } else {
+            int outer = bid / INNER, inner = bid - outer * INNER;      // y sweep: outer = x; x sweep: outer = y
+            base = (long long)outer * (AX == AX_Y ? N * N : N) + (long long)inner * C::W;
         }
     }
-    WDM_DEV long long at(int row, int l) const { return base + (long long)row * rstride + (long long)l * lstride; }
+    WDM_DEV long long at(int row, int l) const { return base + (long long)row * RSTRIDE + (long long)l * LSTRIDE; }
 };
 
 // thread -> (butterfly g, line l).  Strided tiles: lines fastest (a half-warp owns one 128-byte row).
@@ -123,7 +140,7 @@ struct Tile {
 template <int AX, int NB, int W>
 WDM_DEV void split(int b, int &g, int &l)
 {
-    if (AX == AX_STRIDED) { l = b % W; g = b / W; }
+    if (ax_strided(AX)) { l = b % W; g = b / W; }
     else { g = b % NB; l = b / NB; }
 }
 

@@ -157,22 +157,49 @@ __device__ __forceinline__ void issue_tile(cx<typename C::T> *S, const cx<typena
 {
     using T = typename C::T;
     using L = Lay<C, AX>;
+    using TL = Tile<C, AX>;
     constexpr int W = C::W, NTG = C::NT;
     constexpr int EPC = 16 / (int)sizeof(cx<T>);                // elements per 16-byte chunk
-    if constexpr (AX == AX_STRIDED) {
+    // chunk c = gt + k * NTG, k = 0, 1, ...: everything that depends on k is a compile-time constant, so each
+    // copy is one instruction with immediate offsets on both addresses
+    if constexpr (ax_strided(AX)) {
         constexpr int CH = W / EPC;                             // chunks per row
         static_assert(W % EPC == 0, "row must be a whole number of 16-byte chunks");
-#pragma unroll 4
-        for (int c = gt; c < ROWS * CH; c += NTG) {
-            int row = c / CH, part = (c - row * CH) * EPC;
-            cp_async16(S + L::idx(row, part), src + tile.at(row, part));
-        }
+        static_assert(NTG % CH == 0, "a group covers whole rows per round");
+        constexpr int RPI = NTG / CH;                           // rows per round
+        constexpr int FULL = ROWS / RPI, REM = ROWS - FULL * RPI;
+        const int row0 = gt / CH, part = (gt - row0 * CH) * EPC;
+        const cx<T> *g0 = src + tile.at(row0, part);
+        cx<T> *s0 = S + L::idx(row0, part);
+        static_for<0, FULL>([&](auto k_) {
+            constexpr int k = decltype(k_)::value;
+            cp_async16(s0 + L::idx(k * RPI, 0), g0 + (long long)(k * RPI) * TL::RSTRIDE);
+        });
+        if constexpr (REM > 0)
+            if (row0 < REM) cp_async16(s0 + L::idx(FULL * RPI, 0), g0 + (long long)(FULL * RPI) * TL::RSTRIDE);
     } else {
         constexpr int CH = ROWS / EPC;                          // chunks per pencil
-#pragma unroll 4
-        for (int c = gt; c < W * CH; c += NTG) {
-            int l = c / CH, row = (c - l * CH) * EPC;
-            cp_async16(S + L::idx(row, l), src + tile.at(row, l));
+        if constexpr (NTG >= CH) {
+            static_assert(NTG % CH == 0, "a group covers whole pencils per round");
+            constexpr int LPI = NTG / CH;                       // pencils per round
+            static_assert(W % LPI == 0, "whole rounds");
+            const int l0 = gt / CH, row = (gt - l0 * CH) * EPC;
+            const cx<T> *g0 = src + tile.at(row, l0);
+            cx<T> *s0 = S + L::idx(row, l0);
+            static_for<0, W / LPI>([&](auto k_) {
+                constexpr int k = decltype(k_)::value;
+                cp_async16(s0 + L::idx(0, k * LPI), g0 + (long long)(k * LPI) * TL::LSTRIDE);
+            });
+        } else {
+            static_assert(CH % NTG == 0, "a pencil is a whole number of rounds");
+            constexpr int RPL = CH / NTG;                       // rounds per pencil
+            const cx<T> *g0 = src + tile.at(gt * EPC, 0);
+            cx<T> *s0 = S + L::idx(gt * EPC, 0);
+            static_for<0, W * RPL>([&](auto k_) {
+                constexpr int k = decltype(k_)::value;
+                constexpr int l = k / RPL, row = (k % RPL) * NTG * EPC;
+                cp_async16(s0 + L::idx(row, l), g0 + (long long)l * TL::LSTRIDE + row);
+            });
         }
     }
 }
@@ -243,7 +270,7 @@ struct PsiK {
     static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA;
     static constexpr int ITER = (mA * W) / NTG;
     static_assert((mA * W) % NTG == 0, "whole number of level-A butterflies per thread");
-    static_assert(!RHO || AX == AX_STRIDED, "the density sweep runs along a strided axis");
+    static_assert(!RHO || AX == AX_X, "the density sweep runs along x");
     static constexpr size_t TILE_BYTES = align128(L::ELEMS * sizeof(cx<T>));
     static constexpr int AUX = DRIFT ? AUX_PHASE : AUX_NONE;
     struct Pre { T th[KICK ? ITER : 1][KICK ? RA : 1]; };
@@ -261,9 +288,10 @@ struct PsiK {
                 constexpr int it = decltype(it_)::value;
                 int q, l;
                 split<AX, mA, W>(gt + it * NTG, q, l);
+                const T *gp = p.phi + tile.at(q, l);
                 static_for<0, RA>([&](auto r_) {
                     constexpr int r = decltype(r_)::value;
-                    pre.th[it][r] = ldg(p.phi + tile.at(q + mA * r, l));
+                    pre.th[it][r] = ldg(gp + (long long)(mA * r) * TL::RSTRIDE);
                 });
             });
         }
@@ -309,9 +337,10 @@ struct PsiK {
                 split<AX, mA, W>(gt + it * NTG, q, l);
                 cx<T> v[RA];
                 inv_level_regs<RA, T>(q, mA, tb.twA + q, [&](int row) { return S[L::idx(row, l)]; }, v);
+                cx<T> *gp = psi + tile.at(q, l);
                 static_for<0, RA>([&](auto r_) {
                     constexpr int r = decltype(r_)::value;
-                    stv(psi + tile.at(q + mA * r, l), v[r]);
+                    stv(gp + (long long)(mA * r) * TL::RSTRIDE, v[r]);
                     if constexpr (RHO) rho[it][r] = v[r].x * v[r].x + v[r].y * v[r].y;
                 });
             });
@@ -340,11 +369,12 @@ struct PsiK {
                 constexpr int it = decltype(it_)::value;
                 int q, l;
                 split<AX, mA, W>(gt + it * NTG, q, l);
+                const T *gp = p.rho_p ? p.rho_p + tile.at(q, l) : nullptr;
                 static_for<0, RA>([&](auto r_) {
                     constexpr int r = decltype(r_)::value;
                     int row = q + mA * r;
                     T v = rho[it][r];
-                    if (p.rho_p) v += ldg(p.rho_p + tile.at(row, l));
+                    if (gp) v += ldg(gp + (long long)(mA * r) * TL::RSTRIDE);
                     F[row * W + l] = v - mean;
                 });
             });
@@ -387,7 +417,7 @@ template <class C_, int MODE>
 struct HK {
     using C = C_;
     using T = typename C::T;
-    static constexpr int AX = (MODE == H_Z_GREEN) ? AX_CONTIG : AX_STRIDED;
+    static constexpr int AX = (MODE == H_Z_GREEN) ? AX_CONTIG : AX_Y;
     using TL = Tile<C, AX>;
     using L = Lay<C, AX>;
     static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA;
@@ -421,7 +451,8 @@ struct HK {
         if constexpr (MODE == H_Y_FWD) {
             for (int b = gt; b < (N / RM) * W; b += NTG) {
                 int l = b % W, g = b / W;
-                mid_fwd<RM, T>(g * RM, ldS(l), [&](int row, cx<T> v) { stv(H + tile.at(row, l), v); });
+                cx<T> *gp = H + tile.at(g * RM, l);
+                mid_fwd<RM, T>(g * RM, ldS(l), [&](int row, cx<T> v) { stv(gp + (long long)(row - g * RM) * TL::RSTRIDE, v); });
             }
         }
         if constexpr (MODE == H_Z_GREEN) {
@@ -433,7 +464,7 @@ struct HK {
                 bool zero_line = (kx == 0 && ypos == 0);
                 auto mul = [&](int pos, cx<T> v) {
                     T k2 = kxy + tb.ksq_pos[pos];
-                    T gr = (zero_line && pos == 0) ? (T)0 : p.green / k2;
+                    T gr = (zero_line && pos == 0) ? (T)0 : green_over(p.green, k2);
                     return cscale(v, gr);
                 };
                 if constexpr (L::VEC2)
@@ -457,7 +488,8 @@ struct HK {
             for (int b = gt; b < mA * W; b += NTG) {
                 int q, l;
                 split<AX, mA, W>(b, q, l);
-                inv_level<RA, T>(q, mA, tb.twA + q, ldS(l), [&](int row, cx<T> v) { stv(H + tile.at(row, l), v); });
+                cx<T> *gp = H + tile.at(q, l);
+                inv_level<RA, T>(q, mA, tb.twA + q, ldS(l), [&](int row, cx<T> v) { stv(gp + (long long)(row - q) * TL::RSTRIDE, v); });
             }
         }
     }
@@ -469,7 +501,7 @@ template <class C_>
 struct C2RK {
     using C = C_;
     using T = typename C::T;
-    using TL = Tile<C, AX_STRIDED>;
+    using TL = Tile<C, AX_X>;
     static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA;
     static constexpr int WP = W / 2, RSP = W / 2;
     static constexpr size_t PACKED_BYTES = align128((size_t)N * RSP * sizeof(cx<T>));
@@ -479,7 +511,7 @@ struct C2RK {
     static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
     {
         const TL tile(p, t);
-        issue_tile<C, AX_STRIDED, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf + PACKED_BYTES), p.H, tile, gt);
+        issue_tile<C, AX_X, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf + PACKED_BYTES), p.H, tile, gt);
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
     template <class HOOK>
@@ -511,10 +543,11 @@ struct C2RK {
         g_inv_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return row * RSP + l; });
         for (int b = gt; b < mA * WP; b += NTG) {
             int l = b % WP, q = b / WP;
+            T *gp = p.phi_out + tile.at(q, 2 * l);
             inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; },
                              [&](int row, cx<T> v) {
                                  // Re -> line 2l', Im -> line 2l'+1: one (re, im) pair is two adjacent reals of Phi
-                                 stv(reinterpret_cast<cx<T> *>(p.phi_out + tile.at(row, 2 * l)), v);
+                                 stv(reinterpret_cast<cx<T> *>(gp + (long long)(row - q) * TL::RSTRIDE), v);
                              });
         }
     }

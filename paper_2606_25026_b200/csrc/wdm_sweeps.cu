@@ -95,9 +95,10 @@ cudaError_t chain_launch(ChainParams<Real, (int)sizeof...(KS)> &cp, int planes, 
 
 using PsiZKick = PsiK<C, AX_CONTIG, true, false, true>;
 using PsiZ = PsiK<C, AX_CONTIG, false, false, true>;
-using PsiS = PsiK<C, AX_STRIDED, false, false, true>;
-using PsiXRho = PsiK<C, AX_STRIDED, false, true, true>;
-using RhoOnly = PsiK<C, AX_STRIDED, false, true, false>;
+using PsiS = PsiK<C, AX_Y, false, false, true>;
+using PsiX = PsiK<C, AX_X, false, false, true>;
+using PsiXRho = PsiK<C, AX_X, false, true, true>;
+using RhoOnly = PsiK<C, AX_X, false, true, false>;
 using HYF = HK<C, H_Y_FWD>;
 using HZG = HK<C, H_Z_GREEN>;
 using HYI = HK<C, H_Y_INV>;
@@ -111,7 +112,7 @@ cudaError_t init()
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     g_ctas = sms * C::MINB;
 #define OPT(K) if ((e = optin<K>()) != cudaSuccess) return e;
-    OPT(PsiZKick) OPT(PsiZ) OPT(PsiS) OPT(PsiXRho) OPT(RhoOnly) OPT(HYF) OPT(HZG) OPT(HYI) OPT(C2R)
+    OPT(PsiZKick) OPT(PsiZ) OPT(PsiS) OPT(PsiX) OPT(PsiXRho) OPT(RhoOnly) OPT(HYF) OPT(HZG) OPT(HYI) OPT(C2R)
 #undef OPT
     g_chain_ctas = g_ctas;
     if ((e = chain_optin<PsiZKick, PsiS>(sms)) != cudaSuccess) return e;
@@ -159,7 +160,10 @@ cudaError_t psi_z(const void *pp, int kick, cudaStream_t s)
 {
     return kick ? launch<PsiZKick>(pp, kTilesGrid, s) : launch<PsiZ>(pp, kTilesGrid, s);
 }
-cudaError_t psi_strided(const void *pp, cudaStream_t s) { return launch<PsiS>(pp, kTilesGrid, s); }
+cudaError_t psi_strided(const void *pp, int along_x, cudaStream_t s)
+{
+    return along_x ? launch<PsiX>(pp, kTilesGrid, s) : launch<PsiS>(pp, kTilesGrid, s);
+}
 cudaError_t psi_x_rho(const void *pp, int drift, cudaStream_t s)
 {
     return drift ? launch<PsiXRho>(pp, kTilesGrid, s) : launch<RhoOnly>(pp, kTilesGrid, s);

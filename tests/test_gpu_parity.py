@@ -330,7 +330,7 @@ def test_chained_sweeps_match_separate_sweeps(wdm, dtype, N, G):
     assert lags0 == (0, 0)
     used = set()
     for lag in (0, 1, N // 4):
-        (psi_c, phi_c), lags = run(1, lag)
+        (psi_c, phi_c), lags = run(3, lag)
         assert lags[0] > 0 and lags[1] > 0, f"chain not enabled at N={N}: {lags}"
         used.add(lags)
         eps = 1e-6 if dtype == "c64" else 1e-14
