@@ -220,11 +220,13 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
         auto go = [&](auto i_) {
             constexpr int I = decltype(i_)::value;
             using K = typename StageAt<I, KS...>::type;
+            typename K::Pers pers;          // (level-A twiddles: fetched per tile here, the stages differ)
+            pers.setup(tb, gt);
             if constexpr (I == 0) {
-                K::compute(cp.p[I], tb, r.tile, buf, gt, grp, pre, hook);
+                K::compute(cp.p[I], tb, r.tile, buf, gt, grp, pre, pers, hook);
             } else {
                 typename K::Pre none;
-                K::compute(cp.p[I], tb, r.tile, buf, gt, grp, none, hook);
+                K::compute(cp.p[I], tb, r.tile, buf, gt, grp, none, pers, hook);
             }
         };
         chain_dispatch<0, NS>(r.stage, go);

@@ -218,16 +218,87 @@ WDM_HD void inv_level(int rowbase, int m, const cx<T> *tw, LD &&ld, ST &&st)
     static_for<0, R>([&](auto r) { st(rowbase + m * decltype(r)::value, v[decltype(r)::value]); });
 }
 
-// middle level, forward . multiply . inverse without leaving registers; mul(position, value)
+// ---- level stages with the R twiddles of this butterfly already in registers (w[s] = omega^{q s}; w[0] unused).
+// A thread whose q is the same for every tile keeps them for the whole kernel.
+template <int R, typename T, class ST>
+WDM_HD void fwd_level_regs_w(cx<T> (&v)[R], int rowbase, int m, const cx<T> (&w)[R], ST &&st)
+{
+    dif_fwd<R>(v);
+    static_for<0, R>([&](auto s_) {
+        constexpr int s = decltype(s_)::value;
+        cx<T> y = v[brev(s, R)];
+        if constexpr (s > 0) y = cmul(y, w[s]);
+        st(rowbase + m * s, y);
+    });
+}
+template <int R, typename T, class LD, class ST>
+WDM_HD void fwd_level_w(int rowbase, int m, const cx<T> (&w)[R], LD &&ld, ST &&st)
+{
+    cx<T> v[R];
+    static_for<0, R>([&](auto r) { v[decltype(r)::value] = ld(rowbase + m * decltype(r)::value); });
+    dif_fwd<R>(v);
+    static_for<0, R>([&](auto s_) {
+        constexpr int s = decltype(s_)::value;
+        cx<T> y = v[brev(s, R)];
+        if constexpr (s > 0) y = cmul(y, w[s]);
+        st(rowbase + m * s, y);
+    });
+}
+template <int R, typename T, class LD, class ST>
+WDM_HD void inv_level_w(int rowbase, int m, const cx<T> (&w)[R], LD &&ld, ST &&st)
+{
+    cx<T> v[R];
+    static_for<0, R>([&](auto s_) {
+        constexpr int s = decltype(s_)::value;
+        cx<T> y = ld(rowbase + m * s);
+        if constexpr (s > 0) y = cmulc(y, w[s]);
+        v[brev(s, R)] = y;
+    });
+    dit_inv<R>(v);
+    static_for<0, R>([&](auto r) { st(rowbase + m * decltype(r)::value, v[decltype(r)::value]); });
+}
+// Two adjacent lines at once (same q, hence the same twiddles): ld2/st2 move the pair (one 16-byte access for
+// complex64), so a level costs half the memory instructions and one set of twiddles.
+template <int R, typename T, class LD2, class ST2>
+WDM_HD void fwd_level_pair(int rowbase, int m, const cx<T> (&w)[R], LD2 &&ld2, ST2 &&st2)
+{
+    cx<T> a[R], b[R];
+    static_for<0, R>([&](auto r_) { constexpr int r = decltype(r_)::value; ld2(rowbase + m * r, a[r], b[r]); });
+    dif_fwd<R>(a);
+    dif_fwd<R>(b);
+    static_for<0, R>([&](auto s_) {
+        constexpr int s = decltype(s_)::value;
+        cx<T> ya = a[brev(s, R)], yb = b[brev(s, R)];
+        if constexpr (s > 0) { ya = cmul(ya, w[s]); yb = cmul(yb, w[s]); }
+        st2(rowbase + m * s, ya, yb);
+    });
+}
+template <int R, typename T, class LD2>
+WDM_HD void inv_level_pair_regs(int rowbase, int m, const cx<T> (&w)[R], LD2 &&ld2, cx<T> (&a)[R], cx<T> (&b)[R])
+{
+    static_for<0, R>([&](auto s_) {
+        constexpr int s = decltype(s_)::value;
+        cx<T> ya, yb;
+        ld2(rowbase + m * s, ya, yb);
+        if constexpr (s > 0) { ya = cmulc(ya, w[s]); yb = cmulc(yb, w[s]); }
+        a[brev(s, R)] = ya;
+        b[brev(s, R)] = yb;
+    });
+    dit_inv<R>(a);
+    dit_inv<R>(b);
+}
+
+// middle level, forward . multiply . inverse without leaving registers; mul2(p, a, b) multiplies the values
+// at the consecutive positions p (even) and p + 1 in place, so a table lookup can fetch both factors at once
 template <int R, typename T, class LD, class ST, class MUL>
-WDM_HD void mid_both(int rowbase, LD &&ld, ST &&st, MUL &&mul)
+WDM_HD void mid_both(int rowbase, LD &&ld, ST &&st, MUL &&mul2)
 {
     cx<T> v[R];
     static_for<0, R>([&](auto r) { v[decltype(r)::value] = ld(rowbase + decltype(r)::value); });
     dif_fwd<R>(v);
-    static_for<0, R>([&](auto j_) {
-        constexpr int j = decltype(j_)::value;
-        v[j] = mul(rowbase + brev(j, R), v[j]);
+    static_for<0, R / 2>([&](auto i_) {
+        constexpr int i = decltype(i_)::value;
+        mul2(rowbase + 2 * i, v[brev(2 * i, R)], v[brev(2 * i + 1, R)]);
     });
     dit_inv<R>(v);
     static_for<0, R>([&](auto r) { st(rowbase + decltype(r)::value, v[decltype(r)::value]); });
@@ -235,14 +306,14 @@ WDM_HD void mid_both(int rowbase, LD &&ld, ST &&st, MUL &&mul)
 
 // same, the R consecutive rows moved as pairs (16-byte shared-memory vectors for complex64)
 template <int R, typename T, class LD2, class ST2, class MUL>
-WDM_HD void mid_both2(int rowbase, LD2 &&ld2, ST2 &&st2, MUL &&mul)
+WDM_HD void mid_both2(int rowbase, LD2 &&ld2, ST2 &&st2, MUL &&mul2)
 {
     cx<T> v[R];
     static_for<0, R / 2>([&](auto i_) { constexpr int i = decltype(i_)::value; ld2(rowbase + 2 * i, v[2 * i], v[2 * i + 1]); });
     dif_fwd<R>(v);
-    static_for<0, R>([&](auto j_) {
-        constexpr int j = decltype(j_)::value;
-        v[j] = mul(rowbase + brev(j, R), v[j]);
+    static_for<0, R / 2>([&](auto i_) {
+        constexpr int i = decltype(i_)::value;
+        mul2(rowbase + 2 * i, v[brev(2 * i, R)], v[brev(2 * i + 1, R)]);
     });
     dit_inv<R>(v);
     static_for<0, R / 2>([&](auto i_) { constexpr int i = decltype(i_)::value; st2(rowbase + 2 * i, v[2 * i], v[2 * i + 1]); });

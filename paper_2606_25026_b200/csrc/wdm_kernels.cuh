@@ -32,19 +32,28 @@ WDM_DEV cx<double> ldv(const cx<double> *p) { double2 t = *reinterpret_cast<cons
 // still be scheduled across a global store)
 WDM_DEV void stv(cx<float> *p, cx<float> v) { asm volatile("st.global.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.x), "f"(v.y)); }
 WDM_DEV void stv(cx<double> *p, cx<double> v) { *reinterpret_cast<double2 *>(p) = make_double2(v.x, v.y); }
+// two adjacent reals (p aligned to both)
+WDM_DEV void ld2r(const float *p, float &a, float &b) { float2 t = *reinterpret_cast<const float2 *>(p); a = t.x; b = t.y; }
+WDM_DEV void ld2r(const double *p, double &a, double &b) { double2 t = *reinterpret_cast<const double2 *>(p); a = t.x; b = t.y; }
+// two adjacent complex64 values to global memory as one 16-byte store (p 16-byte aligned)
+WDM_DEV void stg2(cx<float> *p, cx<float> a, cx<float> b)
+{
+    asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+}
+WDM_DEV void stg2(cx<double> *p, cx<double> a, cx<double> b) { stv(p, a); stv(p + 1, b); }
 WDM_DEV void ld2(const cx<float> *p, cx<float> &a, cx<float> &b) { float4 t = *reinterpret_cast<const float4 *>(p); a = mk<float>(t.x, t.y); b = mk<float>(t.z, t.w); }
 WDM_DEV void st2(cx<float> *p, cx<float> a, cx<float> b) { *reinterpret_cast<float4 *>(p) = make_float4(a.x, a.y, b.x, b.y); }
 WDM_DEV void ld2(const cx<double> *p, cx<double> &a, cx<double> &b) { a = ldv(p); b = ldv(p + 1); }
 WDM_DEV void st2(cx<double> *p, cx<double> a, cx<double> b) { stv(p, a); stv(p + 1, b); }
 
 // psi * exp(-i theta).  |theta| = |Phi| dt/(2 mu) is far below 1 under the CFL limit (Eq. 26),
-// so the single-precision path takes a Taylor branch (sin to theta^7, cos to theta^8: truncation below
-// 4e-10 for |theta| < 1/4, under float rounding) and falls back to sincosf only for large phases.
+// so the single-precision path takes a Taylor branch for |theta| < 1/4 (sin to theta^5, cos to theta^6:
+// truncation below 1.3e-8 and 4e-10, under float rounding) and falls back to sincosf only for large phases.
 WDM_DEV void sincos_small(float th, float &s, float &c)
 {
     float t2 = th * th;
-    s = th * fmaf(t2, fmaf(t2, fmaf(t2, -1.0f / 5040.0f, 1.0f / 120.0f), -1.0f / 6.0f), 1.0f);
-    c = fmaf(t2, fmaf(t2, fmaf(t2, fmaf(t2, 1.0f / 40320.0f, -1.0f / 720.0f), 1.0f / 24.0f), -0.5f), 1.0f);
+    s = th * fmaf(t2, fmaf(t2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
+    c = fmaf(t2, fmaf(t2, fmaf(t2, -1.0f / 720.0f, 1.0f / 24.0f), -0.5f), 1.0f);
 }
 // large phases are rare: keep the full-range sincosf (with its Payne-Hanek reduction) out of line so the hot
 // code stays small and straight
@@ -67,6 +76,30 @@ WDM_DEV cx<double> rotate_neg(cx<double> v, double th)
     sincos(th, &s, &c);
     return mk<double>(v.x * c + v.y * s, v.y * c - v.x * s);
 }
+// R values at once: ONE test on the largest |theta| picks the branch for the whole butterfly, so the common
+// case is straight-line code (same arithmetic per element as rotate_neg)
+template <int R>
+WDM_DEV void rotate_neg_all(cx<float> (&v)[R], const float (&th0)[R], float scale)
+{
+    float m = 0.0f;
+    static_for<0, R>([&](auto r_) { constexpr int r = decltype(r_)::value; m = fmaxf(m, fabsf(th0[r])); });
+    if (m * fabsf(scale) < 0.25f) {
+        static_for<0, R>([&](auto r_) {
+            constexpr int r = decltype(r_)::value;
+            float s, c;
+            sincos_small(th0[r] * scale, s, c);
+            v[r] = mk<float>(v[r].x * c + v[r].y * s, v[r].y * c - v[r].x * s);
+        });
+    } else {
+        static_for<0, R>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], th0[r] * scale); });
+    }
+}
+template <int R>
+WDM_DEV void rotate_neg_all(cx<double> (&v)[R], const double (&th0)[R], double scale)
+{
+    static_for<0, R>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], th0[r] * scale); });
+}
+
 // g / k2 of the Green's function (Eq. 23).  Single precision: one reciprocal (MUFU.RCP, 1 ulp)
 // and a multiply instead of the IEEE division sequence -- 2 ulp on a factor whose tolerance is 2e-5.
 WDM_DEV float green_over(float g, float k2) { return __fdividef(g, k2); }

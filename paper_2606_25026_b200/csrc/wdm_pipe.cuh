@@ -67,6 +67,25 @@ struct Tabs {
     const T *ksq_pos;
 };
 enum { AUX_NONE = 0, AUX_PHASE = 1, AUX_KSQ = 2 };
+
+// Paired mapping of the level-A stages on a strided tile: thread gt owns the butterflies q = gt / (W/2) of
+// the two adjacent lines 2 (gt % (W/2)) and + 1 -- 16-byte shared-memory accesses, and ONE set of twiddles,
+// which is the same for every tile the thread will ever see: PairTw keeps it in registers for the whole kernel.
+template <class C>
+constexpr bool pair_ok() { return sizeof(typename C::T) == 4 && C::mA * C::W == 2 * C::NT && C::RA * sizeof(typename C::T) <= 64; }
+
+template <class C, bool ON>
+struct PairTw {
+    using T = typename C::T;
+    cx<T> w[ON ? C::RA : 1];
+    __device__ __forceinline__ void setup(const Tabs<T> &tb, int gt)
+    {
+        if constexpr (ON) {
+            const int q = gt / (C::W / 2);
+            static_for<1, C::RA>([&](auto s_) { constexpr int s = decltype(s_)::value; w[s] = tb.twA[s * C::mA + q]; });
+        }
+    }
+};
 constexpr size_t kMaxSmem = 227 * 1024;
 
 template <class K>
@@ -129,6 +148,8 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
             cp_async_arrive(full + j);
         }
     typename K::Pre pre;
+    typename K::Pers pers;
+    pers.setup(tb, gt);
     if (grp < J) K::prefetch(p, bid + grp * stride, gt, pre);
     for (int j = grp; j < J; j += NG) {
         const int b = j % NBUF;
@@ -138,7 +159,7 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
         const int jn = j + NG;
         // called by compute() before its last stage: fetch what the group's NEXT tile needs into registers
         auto hook = [&]() { if (jn < J) K::prefetch(p, bid + jn * stride, gt, pre); };
-        K::compute(p, tb, bid + j * stride, buf, gt, grp, pre, hook);
+        K::compute(p, tb, bid + j * stride, buf, gt, grp, pre, pers, hook);
         group_sync(grp, NTG);                                   // every read of this buffer is done
         if (j + NBUF < J) {
             if (gt == 0) issued[b] = (j + NBUF) / NBUF + 1;
@@ -274,6 +295,14 @@ struct PsiK {
     static constexpr size_t TILE_BYTES = align128(L::ELEMS * sizeof(cx<T>));
     static constexpr int AUX = DRIFT ? AUX_PHASE : AUX_NONE;
     struct Pre { T th[KICK ? ITER : 1][KICK ? RA : 1]; };
+#ifndef WDM_RHO_PAIR
+#define WDM_RHO_PAIR 1
+#endif
+    static constexpr bool PAIR = ax_strided(AX) && pair_ok<C>() && (!RHO || WDM_RHO_PAIR);
+    // the density sweep is short of registers at the end of its last psi stage (two lines of outputs, their
+    // |psi|^2 and the twiddles): it fetches the twiddles where it needs them instead of keeping them
+    static constexpr bool KEEP_TW = PAIR && !RHO;
+    using Pers = PairTw<C, KEEP_TW>;
 
     static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
     {
@@ -298,29 +327,49 @@ struct PsiK {
     }
     template <class HOOK>
     static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt,
-                                                   int grp, Pre &pre, HOOK &&hook)
+                                                   int grp, Pre &pre, const Pers &pers, HOOK &&hook)
     {
         cx<T> *S = reinterpret_cast<cx<T> *>(buf);
         const TL tile(p, t);
         cx<T> *psi = p.data;
         T rho[RHO ? ITER : 1][RHO ? RA : 1];
-        if constexpr (DRIFT) {
-            static_for<0, ITER>([&](auto it_) {
-                constexpr int it = decltype(it_)::value;
-                int q, l;
-                split<AX, mA, W>(gt + it * NTG, q, l);
-                cx<T> v[RA];
-                static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = S[L::idx(q + mA * r, l)]; });
-                if constexpr (KICK)
-                    static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], pre.th[it][r] * p.kick); });
-                fwd_level_regs<RA, T>(v, q, mA, tb.twA + q, [&](int row, cx<T> y) { S[L::idx(row, l)] = y; });
+        const int pq = gt / (W / 2), pl = 2 * (gt % (W / 2));      // paired mapping: butterfly q of lines pl, pl + 1
+        // level-A twiddles of butterfly pq: the kernel-long copy, or fetched now
+        auto twiddles = [&](cx<T> (&w)[RA]) {
+            static_for<1, RA>([&](auto s_) {
+                constexpr int s = decltype(s_)::value;
+                if constexpr (KEEP_TW) w[s] = pers.w[s];
+                else w[s] = tb.twA[s * mA + pq];
             });
+        };
+        if constexpr (DRIFT) {
+            if constexpr (PAIR) {
+                cx<T> w[RA];
+                twiddles(w);
+                fwd_level_pair<RA, T>(pq, mA, w, [&](int row, cx<T> &a, cx<T> &c) { ld2(S + L::idx(row, pl), a, c); },
+                                      [&](int row, cx<T> a, cx<T> c) { st2(S + L::idx(row, pl), a, c); });
+            } else {
+                static_for<0, ITER>([&](auto it_) {
+                    constexpr int it = decltype(it_)::value;
+                    int q, l;
+                    split<AX, mA, W>(gt + it * NTG, q, l);
+                    cx<T> v[RA];
+                    static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = S[L::idx(q + mA * r, l)]; });
+                    if constexpr (KICK) rotate_neg_all<RA>(v, pre.th[it], p.kick);
+                    fwd_level_regs<RA, T>(v, q, mA, tb.twA + q, [&](int row, cx<T> y) { S[L::idx(row, l)] = y; });
+                });
+            }
             group_sync(grp, NTG);
             auto idx = [](int row, int l) { return L::idx(row, l); };
             g_fwd_B<C, W>(S, tb.twB, gt, grp, idx);
             for (int b = gt; b < (N / RM) * W; b += NTG) {
                 int l = b % W, g = b / W;
-                auto mul = [&](int pos, cx<T> v) { return cmul(v, tb.phase[pos]); };
+                auto mul = [&](int pos, cx<T> &a, cx<T> &c) {
+                    cx<T> pa, pc;
+                    ld2(tb.phase + pos, pa, pc);          // both kinetic factors in one 16-byte load
+                    a = cmul(a, pa);
+                    c = cmul(c, pc);
+                };
                 if constexpr (L::VEC2)
                     mid_both2<RM, T>(g * RM, [&](int row, cx<T> &a, cx<T> &c) { ld2(S + L::idx(row, l), a, c); },
                                      [&](int row, cx<T> a, cx<T> c) { st2(S + L::idx(row, l), a, c); }, mul);
@@ -331,30 +380,58 @@ struct PsiK {
             group_sync(grp, NTG);
             g_inv_B<C, W>(S, tb.twB, gt, grp, idx);
             hook();
-            static_for<0, ITER>([&](auto it_) {
-                constexpr int it = decltype(it_)::value;
-                int q, l;
-                split<AX, mA, W>(gt + it * NTG, q, l);
-                cx<T> v[RA];
-                inv_level_regs<RA, T>(q, mA, tb.twA + q, [&](int row) { return S[L::idx(row, l)]; }, v);
-                cx<T> *gp = psi + tile.at(q, l);
+            if constexpr (PAIR) {
+                cx<T> a[RA], c[RA];
+                {
+                    cx<T> w[RA];
+                    twiddles(w);
+                    inv_level_pair_regs<RA, T>(pq, mA, w, [&](int row, cx<T> &x, cx<T> &y) { ld2(S + L::idx(row, pl), x, y); }, a, c);
+                }
+                cx<T> *gp = psi + tile.at(pq, pl);
                 static_for<0, RA>([&](auto r_) {
                     constexpr int r = decltype(r_)::value;
-                    stv(gp + (long long)(mA * r) * TL::RSTRIDE, v[r]);
-                    if constexpr (RHO) rho[it][r] = v[r].x * v[r].x + v[r].y * v[r].y;
+                    stg2(gp + (long long)(mA * r) * TL::RSTRIDE, a[r], c[r]);
+                    if constexpr (RHO) {
+                        rho[0][r] = a[r].x * a[r].x + a[r].y * a[r].y;
+                        rho[1][r] = c[r].x * c[r].x + c[r].y * c[r].y;
+                    }
                 });
-            });
+            } else {
+                static_for<0, ITER>([&](auto it_) {
+                    constexpr int it = decltype(it_)::value;
+                    int q, l;
+                    split<AX, mA, W>(gt + it * NTG, q, l);
+                    cx<T> v[RA];
+                    inv_level_regs<RA, T>(q, mA, tb.twA + q, [&](int row) { return S[L::idx(row, l)]; }, v);
+                    cx<T> *gp = psi + tile.at(q, l);
+                    static_for<0, RA>([&](auto r_) {
+                        constexpr int r = decltype(r_)::value;
+                        stv(gp + (long long)(mA * r) * TL::RSTRIDE, v[r]);
+                        if constexpr (RHO) rho[it][r] = v[r].x * v[r].x + v[r].y * v[r].y;
+                    });
+                });
+            }
         } else if constexpr (RHO) {
-            static_for<0, ITER>([&](auto it_) {
-                constexpr int it = decltype(it_)::value;
-                int q, l;
-                split<AX, mA, W>(gt + it * NTG, q, l);
+            if constexpr (PAIR) {
                 static_for<0, RA>([&](auto r_) {
                     constexpr int r = decltype(r_)::value;
-                    cx<T> v = S[L::idx(q + mA * r, l)];
-                    rho[it][r] = v.x * v.x + v.y * v.y;
+                    cx<T> a, c;
+                    ld2(S + L::idx(pq + mA * r, pl), a, c);
+                    rho[0][r] = a.x * a.x + a.y * a.y;
+                    rho[1][r] = c.x * c.x + c.y * c.y;
                 });
-            });
+            } else {
+                static_for<0, ITER>([&](auto it_) {
+                    constexpr int it = decltype(it_)::value;
+                    int q, l;
+                    split<AX, mA, W>(gt + it * NTG, q, l);
+                    static_for<0, RA>([&](auto r_) {
+                        constexpr int r = decltype(r_)::value;
+                        cx<T> v = S[L::idx(q + mA * r, l)];
+                        rho[it][r] = v.x * v.x + v.y * v.y;
+                    });
+                });
+            }
         }
         if constexpr (RHO) {
             // rho tile as N rows x W reals == N rows x W/2 packed complex lines (lines 2l', 2l'+1)
@@ -365,25 +442,45 @@ struct PsiK {
             // zeroed in the Green's function anyway -- subtracting here only keeps the large mean out of the
             // single-precision partial sums of the low-k modes.
             const T mean = ldg(p.rho_mean);
-            static_for<0, ITER>([&](auto it_) {
-                constexpr int it = decltype(it_)::value;
-                int q, l;
-                split<AX, mA, W>(gt + it * NTG, q, l);
-                const T *gp = p.rho_p ? p.rho_p + tile.at(q, l) : nullptr;
+            cx<T> *Sp = reinterpret_cast<cx<T> *>(buf);
+            if constexpr (PAIR) {
+                // the pair (pl, pl + 1) at rows pq + mA r IS packed line pl / 2 at the rows of this thread's own
+                // level-A butterfly of the real-to-complex transform: straight from registers
+                const T *gp = p.rho_p ? p.rho_p + tile.at(pq, pl) : nullptr;
+                cx<T> v[RA];
                 static_for<0, RA>([&](auto r_) {
                     constexpr int r = decltype(r_)::value;
-                    int row = q + mA * r;
-                    T v = rho[it][r];
-                    if (gp) v += ldg(gp + (long long)(mA * r) * TL::RSTRIDE);
-                    F[row * W + l] = v - mean;
+                    T va = rho[0][r], vc = rho[1][r];
+                    if (gp) {
+                        cx<T> e = ldg(reinterpret_cast<const cx<T> *>(gp + (long long)(mA * r) * TL::RSTRIDE));
+                        va += e.x;
+                        vc += e.y;
+                    }
+                    v[r] = mk<T>(va - mean, vc - mean);
                 });
-            });
-            group_sync(grp, NTG);
-            cx<T> *Sp = reinterpret_cast<cx<T> *>(buf);
-            for (int b = gt; b < mA * WP; b += NTG) {
-                int l = b % WP, q = b / WP;
-                fwd_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; },
-                                 [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
+                cx<T> w[RA];
+                twiddles(w);
+                fwd_level_regs_w<RA, T>(v, pq, mA, w, [&](int row, cx<T> y) { Sp[row * RSP + pl / 2] = y; });
+            } else {
+                static_for<0, ITER>([&](auto it_) {
+                    constexpr int it = decltype(it_)::value;
+                    int q, l;
+                    split<AX, mA, W>(gt + it * NTG, q, l);
+                    const T *gp = p.rho_p ? p.rho_p + tile.at(q, l) : nullptr;
+                    static_for<0, RA>([&](auto r_) {
+                        constexpr int r = decltype(r_)::value;
+                        int row = q + mA * r;
+                        T v = rho[it][r];
+                        if (gp) v += ldg(gp + (long long)(mA * r) * TL::RSTRIDE);
+                        F[row * W + l] = v - mean;
+                    });
+                });
+                group_sync(grp, NTG);
+                for (int b = gt; b < mA * WP; b += NTG) {
+                    int l = b % WP, q = b / WP;
+                    fwd_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; },
+                                     [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
+                }
             }
             group_sync(grp, NTG);
             g_fwd_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return row * RSP + l; });
@@ -424,6 +521,8 @@ struct HK {
     static constexpr size_t TILE_BYTES = align128(L::ELEMS * sizeof(cx<T>));
     static constexpr int AUX = MODE == H_Z_GREEN ? AUX_KSQ : AUX_NONE;
     using Pre = NoPre;
+    static constexpr bool PAIR = ax_strided(AX) && pair_ok<C>();
+    using Pers = PairTw<C, PAIR>;
     static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
     {
         const TL tile(p, t);
@@ -431,19 +530,26 @@ struct HK {
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
     template <class HOOK>
-    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &, HOOK &&)
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &,
+                                                   const Pers &pers, HOOK &&)
     {
         cx<T> *S = reinterpret_cast<cx<T> *>(buf);
         const TL tile(p, t);
         cx<T> *H = p.data;
+        const int pq = gt / (W / 2), pl = 2 * (gt % (W / 2));      // paired mapping (see PairTw)
         auto ldS = [&](int l) { return [S, l](int row) { return S[L::idx(row, l)]; }; };
         auto stS = [&](int l) { return [S, l](int row, cx<T> v) { S[L::idx(row, l)] = v; }; };
         auto idx = [](int row, int l) { return L::idx(row, l); };
         if constexpr (MODE == H_Y_FWD || MODE == H_Z_GREEN) {
-            for (int b = gt; b < mA * W; b += NTG) {
-                int q, l;
-                split<AX, mA, W>(b, q, l);
-                fwd_level<RA, T>(q, mA, tb.twA + q, ldS(l), stS(l));
+            if constexpr (PAIR) {
+                fwd_level_pair<RA, T>(pq, mA, pers.w, [&](int row, cx<T> &a, cx<T> &c) { ld2(S + L::idx(row, pl), a, c); },
+                                      [&](int row, cx<T> a, cx<T> c) { st2(S + L::idx(row, pl), a, c); });
+            } else {
+                for (int b = gt; b < mA * W; b += NTG) {
+                    int q, l;
+                    split<AX, mA, W>(b, q, l);
+                    fwd_level<RA, T>(q, mA, tb.twA + q, ldS(l), stS(l));
+                }
             }
             group_sync(grp, NTG);
             g_fwd_B<C, W>(S, tb.twB, gt, grp, idx);
@@ -462,10 +568,12 @@ struct HK {
                 int pen = t * W + l, kx = pen / N, ypos = pen - kx * N;
                 T kxy = ldg(p.ksq_nat + kx) + tb.ksq_pos[ypos];
                 bool zero_line = (kx == 0 && ypos == 0);
-                auto mul = [&](int pos, cx<T> v) {
-                    T k2 = kxy + tb.ksq_pos[pos];
-                    T gr = (zero_line && pos == 0) ? (T)0 : green_over(p.green, k2);
-                    return cscale(v, gr);
+                auto mul = [&](int pos, cx<T> &a, cx<T> &c) {
+                    T ka, kc;
+                    ld2r(tb.ksq_pos + pos, ka, kc);
+                    T ga = (zero_line && pos == 0) ? (T)0 : green_over(p.green, kxy + ka);
+                    a = cscale(a, ga);
+                    c = cscale(c, green_over(p.green, kxy + kc));
                 };
                 if constexpr (L::VEC2)
                     mid_both2<RM, T>(g * RM, [&](int row, cx<T> &a, cx<T> &c) { ld2(S + L::idx(row, l), a, c); },
@@ -485,11 +593,18 @@ struct HK {
             g_inv_B<C, W>(S, tb.twB, gt, grp, idx);
         }
         if constexpr (MODE == H_Y_INV || MODE == H_Z_GREEN) {
-            for (int b = gt; b < mA * W; b += NTG) {
-                int q, l;
-                split<AX, mA, W>(b, q, l);
-                cx<T> *gp = H + tile.at(q, l);
-                inv_level<RA, T>(q, mA, tb.twA + q, ldS(l), [&](int row, cx<T> v) { stv(gp + (long long)(row - q) * TL::RSTRIDE, v); });
+            if constexpr (PAIR) {
+                cx<T> a[RA], c[RA];
+                inv_level_pair_regs<RA, T>(pq, mA, pers.w, [&](int row, cx<T> &x, cx<T> &y) { ld2(S + L::idx(row, pl), x, y); }, a, c);
+                cx<T> *gp = H + tile.at(pq, pl);
+                static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; stg2(gp + (long long)(mA * r) * TL::RSTRIDE, a[r], c[r]); });
+            } else {
+                for (int b = gt; b < mA * W; b += NTG) {
+                    int q, l;
+                    split<AX, mA, W>(b, q, l);
+                    cx<T> *gp = H + tile.at(q, l);
+                    inv_level<RA, T>(q, mA, tb.twA + q, ldS(l), [&](int row, cx<T> v) { stv(gp + (long long)(row - q) * TL::RSTRIDE, v); });
+                }
             }
         }
     }
@@ -508,6 +623,8 @@ struct C2RK {
     static constexpr size_t TILE_BYTES = PACKED_BYTES + align128((size_t)(N / 2 + 1) * W * sizeof(cx<T>));
     static constexpr int AUX = AUX_NONE;
     using Pre = NoPre;
+    static constexpr bool PAIR = pair_ok<C>();          // packed line gt % (W/2), butterfly gt / (W/2): the PairTw twiddles
+    using Pers = PairTw<C, PAIR>;
     static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
     {
         const TL tile(p, t);
@@ -515,7 +632,8 @@ struct C2RK {
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
     template <class HOOK>
-    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &, HOOK &&)
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &,
+                                                   const Pers &pers, HOOK &&)
     {
         cx<T> *Sp = reinterpret_cast<cx<T> *>(buf);
         const cx<T> *R = reinterpret_cast<const cx<T> *>(buf + PACKED_BYTES);
@@ -544,6 +662,10 @@ struct C2RK {
         for (int b = gt; b < mA * WP; b += NTG) {
             int l = b % WP, q = b / WP;
             T *gp = p.phi_out + tile.at(q, 2 * l);
+            if constexpr (PAIR)
+                inv_level_w<RA, T>(q, mA, pers.w, [&](int row) { return Sp[row * RSP + l]; },
+                                   [&](int row, cx<T> v) { stv(reinterpret_cast<cx<T> *>(gp + (long long)(row - q) * TL::RSTRIDE), v); });
+            else
             inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; },
                              [&](int row, cx<T> v) {
                                  // Re -> line 2l', Im -> line 2l'+1: one (re, im) pair is two adjacent reals of Phi
