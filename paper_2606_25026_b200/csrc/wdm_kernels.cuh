@@ -76,30 +76,6 @@ WDM_DEV cx<double> rotate_neg(cx<double> v, double th)
     sincos(th, &s, &c);
     return mk<double>(v.x * c + v.y * s, v.y * c - v.x * s);
 }
-// R values at once: ONE test on the largest |theta| picks the branch for the whole butterfly, so the common
-// case is straight-line code (same arithmetic per element as rotate_neg)
-template <int R>
-WDM_DEV void rotate_neg_all(cx<float> (&v)[R], const float (&th0)[R], float scale)
-{
-    float m = 0.0f;
-    static_for<0, R>([&](auto r_) { constexpr int r = decltype(r_)::value; m = fmaxf(m, fabsf(th0[r])); });
-    if (m * fabsf(scale) < 0.25f) {
-        static_for<0, R>([&](auto r_) {
-            constexpr int r = decltype(r_)::value;
-            float s, c;
-            sincos_small(th0[r] * scale, s, c);
-            v[r] = mk<float>(v[r].x * c + v[r].y * s, v[r].y * c - v[r].x * s);
-        });
-    } else {
-        static_for<0, R>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], th0[r] * scale); });
-    }
-}
-template <int R>
-WDM_DEV void rotate_neg_all(cx<double> (&v)[R], const double (&th0)[R], double scale)
-{
-    static_for<0, R>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], th0[r] * scale); });
-}
-
 // g / k2 of the Green's function (Eq. 23).  Single precision: one reciprocal (MUFU.RCP, 1 ulp)
 // and a multiply instead of the IEEE division sequence -- 2 ulp on a factor whose tolerance is 2e-5.
 WDM_DEV float green_over(float g, float k2) { return __fdividef(g, k2); }

@@ -355,7 +355,8 @@ struct PsiK {
                     split<AX, mA, W>(gt + it * NTG, q, l);
                     cx<T> v[RA];
                     static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = S[L::idx(q + mA * r, l)]; });
-                    if constexpr (KICK) rotate_neg_all<RA>(v, pre.th[it], p.kick);
+                    if constexpr (KICK)
+                        static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], pre.th[it][r] * p.kick); });
                     fwd_level_regs<RA, T>(v, q, mA, tb.twA + q, [&](int row, cx<T> y) { S[L::idx(row, l)] = y; });
                 });
             }
