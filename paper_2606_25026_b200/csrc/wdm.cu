@@ -116,6 +116,8 @@ struct wdm_ctx {
     double phase_dt = 0;
     bool phase_valid = false, have_psi = false, stale = true;
     // L2-chained sweeps (wdm_chain.cuh): completion counters, launch epochs, lag per chain (0: separate sweeps)
+    // TMA descriptors (see SweepParams): psi along y / x, H along y / x, H single row along x
+    CUtensorMap tm_psi_y, tm_psi_x, tm_h_y, tm_h_x, tm_h_x1;
     unsigned int *chain_done = nullptr;       // [N] for psi z->y, then [2 (N/2+1)] for H y->z->y
     unsigned int epoch_psi = 0, epoch_h = 0;
     int lag_psi = 0, lag_h = 0;
@@ -223,6 +225,51 @@ struct Timed {
     ~Timed() { if (on) cudaEventRecord(c->ev[2 * idx + 1], c->stream); }
 };
 
+// ---------------------------------------------------------------- TMA descriptors
+
+// Box of W complex elements along z by `rows` points along axis (1 = y, 2 = x) of a [nx][N][N] complex array.
+// Encoded in units of one real (float / double), no swizzle, no interleave: the box lands in shared memory as
+// dense [row][W] -- the strided tile layout.
+static int make_tmap(wdm_ctx *c, CUtensorMap *out, void *base, int nx, int axis, int rows)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q);
+        if (e != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn)
+            return fail(c, WDM_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
+        encode = (encode_fn)fn;
+    }
+    const size_t r = rsize(c->dtype);
+    const cuuint64_t N = (cuuint64_t)c->N;
+    cuuint64_t dims[3] = {2 * N, N, (cuuint64_t)nx};
+    cuuint64_t strides[2] = {2 * N * r, 2 * N * N * r};
+    cuuint32_t box[3] = {(cuuint32_t)(2 * c->tab->fact.W), axis == 1 ? (cuuint32_t)rows : 1u, axis == 2 ? (cuuint32_t)rows : 1u};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult res = encode(out, c->dtype == WDM_C64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims,
+                          strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (res != CUDA_SUCCESS) return fail(c, WDM_ECUDA, "cuTensorMapEncodeTiled failed (%d) for N = %d axis %d rows %d", (int)res, c->N, axis, rows);
+    return WDM_OK;
+}
+
+static int box_rows(int n) { return n < 256 ? n : 256; }
+
+static int make_tmaps(wdm_ctx *c)
+{
+    const int N = c->N;
+    int rc;
+    if ((rc = make_tmap(c, &c->tm_psi_y, c->psi, N, 1, box_rows(N))) || (rc = make_tmap(c, &c->tm_psi_x, c->psi, N, 2, box_rows(N))) ||
+        (rc = make_tmap(c, &c->tm_h_y, c->H, N / 2 + 1, 1, box_rows(N))) ||
+        (rc = make_tmap(c, &c->tm_h_x, c->H, N / 2 + 1, 2, box_rows(N / 2))) || (rc = make_tmap(c, &c->tm_h_x1, c->H, N / 2 + 1, 2, 1)))
+        return rc;
+    return WDM_OK;
+}
+
 // ---------------------------------------------------------------- tables
 
 template <typename T>
@@ -280,21 +327,27 @@ static int density_poisson(wdm_ctx *c, bool drift)
     {
         SweepParams<T> p = base_params<T>(c);
         p.data = (cx<T> *)c->psi;
+        p.tmap = c->tm_psi_x;
+        p.tag = S_PSI_X_RHO;
         Timed t(c, S_PSI_X_RHO);
         CU(c, c->tab->psi_x_rho(&p, drift ? 1 : 0, c->stream));
     }
     SweepParams<T> p = base_params<T>(c);
     p.data = (cx<T> *)c->H;
+    p.tmap = c->tm_h_y;
     if (c->lag_h > 0) {
         ChainCtl ctl{c->chain_done + N, ++c->epoch_h * (unsigned int)(N / c->tab->fact.W), c->lag_h};
+        p.tag = S_H_YZY;
         Timed t(c, S_H_YZY);
         CU(c, c->tab->h_yzy(&p, &p, &ctl, c->stream));
     } else {
-        { Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
-        { Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
-        { Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
+        { p.tag = S_H_Y_FWD; Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
+        { p.tag = S_H_Z_GREEN; Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
+        { p.tag = S_H_Y_INV; Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
     }
-    { Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, c->stream)); }
+    p.tmap = c->tm_h_x;
+    p.tmap2 = c->tm_h_x1;
+    { p.tag = S_C2R; Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, c->stream)); }
     return WDM_OK;
 }
 
@@ -361,13 +414,15 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             pz.data = (cx<T> *)c->psi;
             pz.kick = (T)(kdt / c->mu);
             py.data = (cx<T> *)c->psi;
+            py.tmap = c->tm_psi_y;
             if (c->lag_psi > 0) {
                 ChainCtl ctl{c->chain_done, ++c->epoch_psi * (unsigned int)(N / c->tab->fact.W), c->lag_psi};
+                pz.tag = S_PSI_ZY;
                 Timed t(c, S_PSI_ZY);
                 CU(c, c->tab->psi_zy(&pz, &py, grav ? 1 : 0, &ctl, c->stream));
             } else {
-                { Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, grav ? 1 : 0, c->stream)); }
-                { Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
+                { pz.tag = S_PSI_Z; Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, grav ? 1 : 0, c->stream)); }
+                { py.tag = S_PSI_Y; Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
             }
         }
         if (grav) {
@@ -376,6 +431,7 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
         } else {
             SweepParams<T> p = base_params<T>(c);
             p.data = (cx<T> *)c->psi;
+            p.tmap = c->tm_psi_x;
             Timed t(c, S_PSI_Y);
             CU(c, c->tab->psi_strided(&p, 1, c->stream));
         }
@@ -461,6 +517,7 @@ static int create_common(wdm_ctx **out, int N, double L, double mu, double G, in
     }
     rc = dtype == WDM_C64 ? upload_tables<float>(c) : upload_tables<double>(c);
     if (rc) return bail(rc);
+    if ((rc = make_tmaps(c))) return bail(rc);
     if (!owns && max_particles > 0) {
         void *rho_p = nullptr, *pm = nullptr;
         if ((rc = ctx_alloc(c, &rho_p, c->n * rs)) || (rc = ctx_alloc(c, &pm, particle_bytes(N, dtype, max_particles)))) return bail(rc);

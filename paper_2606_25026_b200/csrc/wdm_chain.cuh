@@ -153,7 +153,7 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
     const int bid = blockIdx.x, stride = gridDim.x;
     const int J = (cp.total - bid + stride - 1) / stride;
     if (tid == 0)
-        for (int b = 0; b < NBUF; ++b) { mbar_init(full + b, NTG); issued[b] = (b < J) ? 1 : 0; }
+        for (int b = 0; b < NBUF; ++b) { mbar_init(full + b, 1); issued[b] = (b < J) ? 1 : 0; }
     const SweepParams<T> &p0 = cp.p[0];
     Tabs<T> tb{p0.twA, p0.twB, p0.phase, p0.ksq_pos};
     if constexpr (SM::TW_IN_SMEM) {
@@ -178,30 +178,28 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
     }
     __syncthreads();
 
-    // request tile number j of this CTA into buffer b (all threads of the calling group)
+    // request tile number j of this CTA into buffer b: ONE thread of the group (gt == 0) -- it waits for the
+    // planes the tile depends on, then issues the bulk copies; the other threads go on to their next tile
     auto request = [&](int j, int b) {
         const TileRef r = chain_decode(cp, bid + j * stride);
         if (r.stage > 0 && !(cp.debug & 1)) {
-            if (gt == 0) {
-                const unsigned int *ctr = cp.done + (size_t)(r.stage - 1) * cp.units + r.unit;
-                while ((int)(ld_acquire(ctr) - cp.target) < 0) __nanosleep(200);
-            }
-            group_sync(grp, NTG);
+            const unsigned int *ctr = cp.done + (size_t)(r.stage - 1) * cp.units + r.unit;
+            while ((int)(ld_acquire(ctr) - cp.target) < 0) __nanosleep(100);
+            asm volatile("fence.proxy.async;" ::: "memory");       // acquired (generic proxy) before the bulk reads (async proxy)
         }
         unsigned char *buf = smem + (size_t)b * SM::TILE_BYTES;
         auto go = [&](auto i_) {
             constexpr int I = decltype(i_)::value;
             using K = typename StageAt<I, KS...>::type;
-            K::issue(cp.p[I], r.tile, buf, gt);
+            K::issue(cp.p[I], r.tile, buf, full + b);
         };
         chain_dispatch<0, NS>(r.stage, go);
-        cp_async_arrive(full + b);
     };
 
     // first round of fills: a group requests its own first tile now and the rest of the round only after it
     // has computed that tile (a group must never wait on a dependency while it sits on an uncomputed tile
     // that the dependency may, transitively, need)
-    if (grp < J) request(grp, grp);
+    if (grp < J && gt == 0) request(grp, grp);
     typename K0::Pre pre;
     auto prefetch_for = [&](int j) {
         if (j < J) {
@@ -214,8 +212,10 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
         const int b = j % NBUF;
         unsigned char *buf = smem + (size_t)b * SM::TILE_BYTES;
         const TileRef r = chain_decode(cp, bid + j * stride);
+        WDM_T(t_top);
         while (issued[b] < j / NBUF + 1) __nanosleep(64);
         mbar_wait(full + b, (j / NBUF) & 1);
+        WDM_T(t_data);
         auto hook = [&]() { prefetch_for(j + NG); };
         auto go = [&](auto i_) {
             constexpr int I = decltype(i_)::value;
@@ -230,17 +230,22 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
             }
         };
         chain_dispatch<0, NS>(r.stage, go);
+        fence_proxy_async();
         group_sync(grp, NTG);                                   // buffer free; every store of the tile issued
+        WDM_T(t_done);
         if (gt == 0) {
-            if (r.stage < NS - 1 && !(cp.debug & 2)) {
-                __threadfence();
-                red_release_add(cp.done + (size_t)r.stage * cp.units + r.unit, 1u);
+            // release: the group's stores (ordered before this thread by the barrier) are visible before the count
+            if (r.stage < NS - 1 && !(cp.debug & 2)) red_release_add(cp.done + (size_t)r.stage * cp.units + r.unit, 1u);
+            if (j < NG)
+                for (int jj = j + NG; jj < NBUF && jj < J; jj += NG) request(jj, jj);
+            if (j + NBUF < J) {
+                issued[b] = (j + NBUF) / NBUF + 1;
+                request(j + NBUF, b);
             }
-            if (j + NBUF < J) issued[b] = (j + NBUF) / NBUF + 1;
         }
-        if (j < NG)
-            for (int jj = j + NG; jj < NBUF && jj < J; jj += NG) request(jj, jj);
-        if (j + NBUF < J) request(j + NBUF, b);
+#ifdef WDM_TRACE
+        if (gt == 0) trace_put(cp.p[0].tag, grp, NG, j / NG, r.stage, t_top, t_data, t_done, clock64());
+#endif
     }
 }
 

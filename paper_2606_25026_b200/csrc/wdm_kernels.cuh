@@ -12,6 +12,8 @@
 // kernels themselves (persistent, software-pipelined) are in wdm_pipe.cuh.
 #pragma once
 
+#include <cuda.h>          // CUtensorMap (type only: the encoder is fetched through the runtime, no libcuda link)
+
 #include "wdm_fft.cuh"
 
 #define WDM_DEV __device__ __forceinline__
@@ -99,6 +101,10 @@ struct SweepParams {
     const T *ksq_pos;          // Green: k^2 of the frequency held at a position
     const T *ksq_nat;          // Green: k^2 of frequency index k (natural)
     T green;                   // Green: -4 pi G / N^3
+    // TMA descriptors of the array a strided sweep walks: boxes of (W elements along z) x (<= 256 rows along the
+    // sweep axis); tmap2 is the one-row box that fetches row N/2 of the half spectrum in the complex-to-real sweep
+    CUtensorMap tmap, tmap2;
+    int tag;                   // which launch of the step this is (kernel-stats slot; read by developer traces only)
 };
 
 // Axis of a sweep over an array [x][y][z] (z contiguous).  The strides are compile-time constants of the
@@ -132,7 +138,8 @@ struct Tile {
     static constexpr int INNER = C::N / C::W;                                          // strided: tiles along z
     long long base;
     template <typename T>
-    WDM_DEV Tile(const SweepParams<T> &, int bid)
+    WDM_DEV Tile(const SweepParams<T> &, int bid) : Tile(bid) {}
+    WDM_DEV explicit Tile(int bid)
     {
         if (AX == AX_CONTIG) {
             base = (long long)bid * C::W * C::N;

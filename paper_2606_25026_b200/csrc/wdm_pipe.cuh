@@ -50,10 +50,48 @@ __device__ __forceinline__ void cp_async8(void *dst, const void *src)
 }
 __device__ __forceinline__ void cp_async_elem(cx<float> *dst, const cx<float> *src) { cp_async8(dst, src); }
 __device__ __forceinline__ void cp_async_elem(cx<double> *dst, const cx<double> *src) { cp_async16(dst, src); }
+// TMA: the mbarrier of a tile buffer has ONE expected arrival -- the issuing thread's arrive.expect_tx with the
+// tile's byte count -- and completes when the bulk copies have delivered that many bytes.
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
+                 "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+// orders this thread's earlier shared-memory accesses (generic proxy) before later bulk copies (async proxy)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void group_sync(int group, int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "r"(nthreads) : "memory");
 }
+
+// ---------------------------------------------------------------- per-tile timeline (developer builds only, -DWDM_TRACE)
+#ifdef WDM_TRACE
+__device__ long long *g_wdm_trace;          // [cta][group][tile slot][8]: stage, t_top, t_data, t_done, t_requested
+__device__ int g_wdm_trace_tag;             // only launches with this SweepParams::tag write
+constexpr int kTraceSlots = 640;
+__device__ __forceinline__ void trace_put(int tag, int grp, int ng, int slot, int stage, long long t0, long long t1, long long t2, long long t3)
+{
+    if (g_wdm_trace && tag == g_wdm_trace_tag && slot < kTraceSlots) {
+        long long *r = g_wdm_trace + (((size_t)blockIdx.x * ng + grp) * kTraceSlots + slot) * 8;
+        r[0] = stage; r[1] = t0; r[2] = t1; r[3] = t2; r[4] = t3;
+    }
+}
+#define WDM_T(x) long long x = clock64()
+#else
+#define WDM_T(x)
+#endif
 
 // ---------------------------------------------------------------- the pipeline driver
 // K provides:  using C;  TILE_BYTES;  AUX;  struct Pre;  issue(p, tile, buf, gt);  prefetch(p, tile, gt, pre);
@@ -117,7 +155,7 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
     const int bid = blockIdx.x, stride = gridDim.x;
     const int J = (ntiles - bid + stride - 1) / stride;        // tiles of this CTA: bid + j*stride
     if (tid == 0)
-        for (int b = 0; b < NBUF; ++b) { mbar_init(full + b, NTG); issued[b] = (b < J) ? 1 : 0; }
+        for (int b = 0; b < NBUF; ++b) { mbar_init(full + b, 1); issued[b] = (b < J) ? 1 : 0; }
     using SM = PipeSmem<K>;
     using T = typename C::T;
     Tabs<T> tb{p.twA, p.twB, p.phase, p.ksq_pos};
@@ -143,10 +181,7 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
     }
     __syncthreads();
     for (int j = 0; j < NBUF && j < J; ++j)
-        if (j % NG == grp) {
-            K::issue(p, bid + j * stride, smem + (size_t)j * K::TILE_BYTES, gt);
-            cp_async_arrive(full + j);
-        }
+        if (j % NG == grp && gt == 0) K::issue(p, bid + j * stride, smem + (size_t)j * K::TILE_BYTES, full + j);
     typename K::Pre pre;
     typename K::Pers pers;
     pers.setup(tb, gt);
@@ -154,74 +189,63 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
     for (int j = grp; j < J; j += NG) {
         const int b = j % NBUF;
         unsigned char *buf = smem + (size_t)b * K::TILE_BYTES;
+        WDM_T(t_top);
         while (issued[b] < j / NBUF + 1) __nanosleep(64);
         mbar_wait(full + b, (j / NBUF) & 1);
+        WDM_T(t_data);
         const int jn = j + NG;
         // called by compute() before its last stage: fetch what the group's NEXT tile needs into registers
         auto hook = [&]() { if (jn < J) K::prefetch(p, bid + jn * stride, gt, pre); };
         K::compute(p, tb, bid + j * stride, buf, gt, grp, pre, pers, hook);
+        fence_proxy_async();                                    // this thread's accesses to the buffer, before its refill
         group_sync(grp, NTG);                                   // every read of this buffer is done
-        if (j + NBUF < J) {
-            if (gt == 0) issued[b] = (j + NBUF) / NBUF + 1;
-            K::issue(p, bid + (j + NBUF) * stride, buf, gt);
-            cp_async_arrive(full + b);
+        WDM_T(t_done);
+        if (j + NBUF < J && gt == 0) {
+            issued[b] = (j + NBUF) / NBUF + 1;
+            K::issue(p, bid + (j + NBUF) * stride, buf, full + b);
         }
+#ifdef WDM_TRACE
+        if (gt == 0) trace_put(p.tag, grp, NG, j / NG, 0, t_top, t_data, t_done, clock64());
+#endif
     }
 }
 
 // ---------------------------------------------------------------- shared building blocks
 
-// asynchronous tile load in 16-byte chunks (see Lay for the layouts).  Strided tiles: a row is W contiguous
-// elements, a warp covers whole 128-byte rows.  Contiguous tiles: a warp walks 512 bytes along one pencil.
+// Asynchronous tile load by ONE thread (the caller elects it): TMA boxes for strided tiles, one bulk copy per
+// pencil for contiguous tiles (their shared-memory lines are padded, which a box cannot express).  `bid` is the
+// tile index, ROWS the number of points along the sweep axis to fetch, tm1 the one-row box used when ROWS is
+// not a multiple of the main box (complex-to-real: N/2 + 1 rows).
 template <class C, int AX, int ROWS>
-__device__ __forceinline__ void issue_tile(cx<typename C::T> *S, const cx<typename C::T> *src, const Tile<C, AX> &tile, int gt)
+__device__ __forceinline__ void tile_load(cx<typename C::T> *S, const cx<typename C::T> *src, const CUtensorMap *tm, const CUtensorMap *tm1,
+                                          int bid, uint64_t *bar)
 {
     using T = typename C::T;
     using L = Lay<C, AX>;
     using TL = Tile<C, AX>;
-    constexpr int W = C::W, NTG = C::NT;
-    constexpr int EPC = 16 / (int)sizeof(cx<T>);                // elements per 16-byte chunk
-    // chunk c = gt + k * NTG, k = 0, 1, ...: everything that depends on k is a compile-time constant, so each
-    // copy is one instruction with immediate offsets on both addresses
+    constexpr int W = C::W;
+    constexpr uint32_t BYTES = (uint32_t)((size_t)ROWS * W * sizeof(cx<T>));
+    mbar_expect_tx(bar, BYTES);
     if constexpr (ax_strided(AX)) {
-        constexpr int CH = W / EPC;                             // chunks per row
-        static_assert(W % EPC == 0, "row must be a whole number of 16-byte chunks");
-        static_assert(NTG % CH == 0, "a group covers whole rows per round");
-        constexpr int RPI = NTG / CH;                           // rows per round
-        constexpr int FULL = ROWS / RPI, REM = ROWS - FULL * RPI;
-        const int row0 = gt / CH, part = (gt - row0 * CH) * EPC;
-        const cx<T> *g0 = src + tile.at(row0, part);
-        cx<T> *s0 = S + L::idx(row0, part);
-        static_for<0, FULL>([&](auto k_) {
-            constexpr int k = decltype(k_)::value;
-            cp_async16(s0 + L::idx(k * RPI, 0), g0 + (long long)(k * RPI) * TL::RSTRIDE);
-        });
-        if constexpr (REM > 0)
-            if (row0 < REM) cp_async16(s0 + L::idx(FULL * RPI, 0), g0 + (long long)(FULL * RPI) * TL::RSTRIDE);
-    } else {
-        constexpr int CH = ROWS / EPC;                          // chunks per pencil
-        if constexpr (NTG >= CH) {
-            static_assert(NTG % CH == 0, "a group covers whole pencils per round");
-            constexpr int LPI = NTG / CH;                       // pencils per round
-            static_assert(W % LPI == 0, "whole rounds");
-            const int l0 = gt / CH, row = (gt - l0 * CH) * EPC;
-            const cx<T> *g0 = src + tile.at(row, l0);
-            cx<T> *s0 = S + L::idx(row, l0);
-            static_for<0, W / LPI>([&](auto k_) {
-                constexpr int k = decltype(k_)::value;
-                cp_async16(s0 + L::idx(0, k * LPI), g0 + (long long)(k * LPI) * TL::LSTRIDE);
-            });
-        } else {
-            static_assert(CH % NTG == 0, "a pencil is a whole number of rounds");
-            constexpr int RPL = CH / NTG;                       // rounds per pencil
-            const cx<T> *g0 = src + tile.at(gt * EPC, 0);
-            cx<T> *s0 = S + L::idx(gt * EPC, 0);
-            static_for<0, W * RPL>([&](auto k_) {
-                constexpr int k = decltype(k_)::value;
-                constexpr int l = k / RPL, row = (k % RPL) * NTG * EPC;
-                cp_async16(s0 + L::idx(row, l), g0 + (long long)l * TL::LSTRIDE + row);
-            });
+        constexpr int EVEN = ROWS & ~1;                                  // ROWS = N, or N/2 + 1
+        constexpr int RB = EVEN < 256 ? EVEN : 256;                      // rows per box (as encoded on the host)
+        constexpr int FULL = ROWS / RB;
+        const int outer = bid / TL::INNER, inner = bid - outer * TL::INNER;
+        const int c0 = inner * 2 * W;
+#pragma unroll
+        for (int k = 0; k < FULL; ++k) {
+            if (AX == AX_Y) tma_load_3d(S + (size_t)k * RB * W, tm, c0, k * RB, outer, bar);
+            else tma_load_3d(S + (size_t)k * RB * W, tm, c0, outer, k * RB, bar);
         }
+        if constexpr (ROWS - FULL * RB > 0) {
+            static_assert(ROWS - FULL * RB == 1 && AX == AX_X, "only the half spectrum has an odd row");
+            tma_load_3d(S + (size_t)FULL * RB * W, tm1, c0, outer, FULL * RB, bar);
+        }
+    } else {
+        const TL tile(bid);
+#pragma unroll 4
+        for (int l = 0; l < W; ++l)
+            bulk_load(S + L::idx(0, l), src + tile.at(0, l), (uint32_t)(ROWS * sizeof(cx<T>)), bar);
     }
 }
 
@@ -304,10 +328,10 @@ struct PsiK {
     static constexpr bool KEEP_TW = PAIR && !RHO;
     using Pers = PairTw<C, KEEP_TW>;
 
-    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
+    // (one thread)
+    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar)
     {
-        const TL tile(p, t);
-        issue_tile<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, tile, gt);
+        tile_load<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, &p.tmap, &p.tmap2, t, bar);
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &p, int t, int gt, Pre &pre)
     {
@@ -524,10 +548,10 @@ struct HK {
     using Pre = NoPre;
     static constexpr bool PAIR = ax_strided(AX) && pair_ok<C>();
     using Pers = PairTw<C, PAIR>;
-    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
+    // (one thread)
+    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar)
     {
-        const TL tile(p, t);
-        issue_tile<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, tile, gt);
+        tile_load<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, &p.tmap, &p.tmap2, t, bar);
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
     template <class HOOK>
@@ -626,10 +650,9 @@ struct C2RK {
     using Pre = NoPre;
     static constexpr bool PAIR = pair_ok<C>();          // packed line gt % (W/2), butterfly gt / (W/2): the PairTw twiddles
     using Pers = PairTw<C, PAIR>;
-    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, int gt)
+    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar)
     {
-        const TL tile(p, t);
-        issue_tile<C, AX_X, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf + PACKED_BYTES), p.H, tile, gt);
+        tile_load<C, AX_X, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf + PACKED_BYTES), p.H, &p.tmap, &p.tmap2, t, bar);
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
     template <class HOOK>
