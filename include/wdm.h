@@ -95,8 +95,8 @@ int wdm_get_particles_host(wdm_ctx *ctx, void *pos_out_host, void *vel_out_host)
  * mode is a bit mask.  Bit 0 (1): the z and y sweeps of psi (Eq. 18(b)) run as one
  * kernel.  Bit 1 (2): the y-forward, z-Green, y-inverse sweeps of the Poisson solve (Eq. 18(c)
  * PAPER.md:194, Eq. 23) run as one kernel.  In a chained kernel the later stage trails
- * the earlier one by `lag` x-planes and reads them from L2 instead of HBM.  mode 0 (default): one
- * launch per sweep.  lag <= 0 picks the lag automatically.  wdm_get_chain reports the lags in use
+ * the earlier one by `lag` x-planes and reads them from L2 instead of HBM.  mode 0: one launch per
+ * sweep.  Default: 2 for N >= 512, else 0.  lag <= 0 picks the lag automatically.  wdm_get_chain reports the lags in use
  * (0 = that chain runs as separate sweeps, e.g. because the grid is too small for it to be
  * meaningful).  The environment variables WDM_CHAIN=<mode> and WDM_CHAIN_LAG=<planes> set the
  * defaults of new contexts. */

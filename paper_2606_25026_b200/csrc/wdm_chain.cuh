@@ -178,20 +178,23 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
     }
     __syncthreads();
 
-    // request tile number j of this CTA into buffer b: ONE thread of the group (gt == 0) -- it waits for the
-    // planes the tile depends on, then issues the bulk copies; the other threads go on to their next tile
+    // request tile number j of this CTA into buffer b: the FIRST WARP of the group (gt < 32) -- lane 0 waits for
+    // the planes the tile depends on, then the warp issues the bulk copies; the other warps go on to their next tile
     auto request = [&](int j, int b) {
         const TileRef r = chain_decode(cp, bid + j * stride);
         if (r.stage > 0 && !(cp.debug & 1)) {
-            const unsigned int *ctr = cp.done + (size_t)(r.stage - 1) * cp.units + r.unit;
-            while ((int)(ld_acquire(ctr) - cp.target) < 0) __nanosleep(100);
+            if (gt == 0) {
+                const unsigned int *ctr = cp.done + (size_t)(r.stage - 1) * cp.units + r.unit;
+                while ((int)(ld_acquire(ctr) - cp.target) < 0) __nanosleep(100);
+            }
+            __syncwarp();
             asm volatile("fence.proxy.async;" ::: "memory");       // acquired (generic proxy) before the bulk reads (async proxy)
         }
         unsigned char *buf = smem + (size_t)b * SM::TILE_BYTES;
         auto go = [&](auto i_) {
             constexpr int I = decltype(i_)::value;
             using K = typename StageAt<I, KS...>::type;
-            K::issue(cp.p[I], r.tile, buf, full + b);
+            K::issue(cp.p[I], r.tile, buf, full + b, gt);
         };
         chain_dispatch<0, NS>(r.stage, go);
     };
@@ -199,7 +202,7 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
     // first round of fills: a group requests its own first tile now and the rest of the round only after it
     // has computed that tile (a group must never wait on a dependency while it sits on an uncomputed tile
     // that the dependency may, transitively, need)
-    if (grp < J && gt == 0) request(grp, grp);
+    if (grp < J && gt < 32) request(grp, grp);
     typename K0::Pre pre;
     auto prefetch_for = [&](int j) {
         if (j < J) {
@@ -233,13 +236,13 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
         fence_proxy_async();
         group_sync(grp, NTG);                                   // buffer free; every store of the tile issued
         WDM_T(t_done);
-        if (gt == 0) {
+        if (gt < 32) {
             // release: the group's stores (ordered before this thread by the barrier) are visible before the count
-            if (r.stage < NS - 1 && !(cp.debug & 2)) red_release_add(cp.done + (size_t)r.stage * cp.units + r.unit, 1u);
+            if (gt == 0 && r.stage < NS - 1 && !(cp.debug & 2)) red_release_add(cp.done + (size_t)r.stage * cp.units + r.unit, 1u);
             if (j < NG)
                 for (int jj = j + NG; jj < NBUF && jj < J; jj += NG) request(jj, jj);
             if (j + NBUF < J) {
-                issued[b] = (j + NBUF) / NBUF + 1;
+                if (gt == 0) issued[b] = (j + NBUF) / NBUF + 1;
                 request(j + NBUF, b);
             }
         }

@@ -153,9 +153,21 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
     volatile int *issued = reinterpret_cast<volatile int *>(full + NBUF);
     const int tid = threadIdx.x, grp = tid / NTG, gt = tid - grp * NTG;
     const int bid = blockIdx.x, stride = gridDim.x;
-    const int J = (ntiles - bid + stride - 1) / stride;        // tiles of this CTA: bid + j*stride
+    // Tile assignment.  The k-th tile of a CTA is computed by group k % NG in buffer k % NBUF; tile_of[b] is the
+    // global tile index of the current fill of buffer b, or -1 when there is nothing left.  The first NBUF tiles
+    // are static (bid + k * grid); every later one is a ticket from a device-wide counter, drawn when the tile
+    // whose buffer it will take starts computing -- SMs that run faster (the sweeps are memory bound, and not
+    // every SM sees the same share of the bandwidth) simply take more tiles.
+    volatile int *tile_of = issued + NBUF;
+    static_assert(NBUF * (sizeof(uint64_t) + 2 * sizeof(int)) <= 64, "control block");
+    const int nstatic = NBUF * stride;
     if (tid == 0)
-        for (int b = 0; b < NBUF; ++b) { mbar_init(full + b, 1); issued[b] = (b < J) ? 1 : 0; }
+        for (int b = 0; b < NBUF; ++b) {
+            mbar_init(full + b, 1);
+            const int t0 = bid + b * stride;
+            tile_of[b] = t0 < ntiles ? t0 : -1;
+            issued[b] = 1;
+        }
     using SM = PipeSmem<K>;
     using T = typename C::T;
     Tabs<T> tb{p.twA, p.twB, p.phase, p.ksq_pos};
@@ -180,53 +192,83 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
         tb.ksq_pos = a;
     }
     __syncthreads();
-    for (int j = 0; j < NBUF && j < J; ++j)
-        if (j % NG == grp && gt == 0) K::issue(p, bid + j * stride, smem + (size_t)j * K::TILE_BYTES, full + j);
+    for (int k = 0; k < NBUF; ++k)
+        if (k % NG == grp && gt < 32 && tile_of[k] >= 0) K::issue(p, tile_of[k], smem + (size_t)k * K::TILE_BYTES, full + k, gt);
     typename K::Pre pre;
     typename K::Pers pers;
     pers.setup(tb, gt);
-    if (grp < J) K::prefetch(p, bid + grp * stride, gt, pre);
-    for (int j = grp; j < J; j += NG) {
-        const int b = j % NBUF;
+    int pre_tile = -1;                                          // tile whose prefetched operands `pre` holds
+    for (int k = grp;; k += NG) {
+        const int b = k % NBUF;
         unsigned char *buf = smem + (size_t)b * K::TILE_BYTES;
         WDM_T(t_top);
-        while (issued[b] < j / NBUF + 1) __nanosleep(64);
-        mbar_wait(full + b, (j / NBUF) & 1);
+        while (issued[b] < k / NBUF + 1) __nanosleep(64);
+        const int t = tile_of[b];
+        if (t < 0) {
+            // nothing left for this group: pass the end mark on to the tile that would have followed in this
+            // buffer (its owner may still be waiting for it)
+            if (gt == 0) issued[b] = (k + NBUF) / NBUF + 1;
+            break;
+        }
+        unsigned int ticket = 0;
+        if (gt == 0) ticket = (unsigned int)nstatic + atomicAdd(p.ticket, 1u);   // consumed after the compute: latency hidden
+        mbar_wait(full + b, (k / NBUF) & 1);
         WDM_T(t_data);
-        const int jn = j + NG;
-        // called by compute() before its last stage: fetch what the group's NEXT tile needs into registers
-        auto hook = [&]() { if (jn < J) K::prefetch(p, bid + jn * stride, gt, pre); };
-        K::compute(p, tb, bid + j * stride, buf, gt, grp, pre, pers, hook);
+        if (pre_tile != t) K::prefetch(p, t, gt, pre);
+        // called by compute() before its last stage: fetch what the group's NEXT tile needs into registers, if
+        // that tile has been assigned by now
+        auto hook = [&]() {
+            const int b2 = (k + NG) % NBUF;
+            if (issued[b2] >= (k + NG) / NBUF + 1) {
+                const int t2 = tile_of[b2];
+                if (t2 >= 0) { K::prefetch(p, t2, gt, pre); pre_tile = t2; }
+            }
+        };
+        K::compute(p, tb, t, buf, gt, grp, pre, pers, hook);
         fence_proxy_async();                                    // this thread's accesses to the buffer, before its refill
         group_sync(grp, NTG);                                   // every read of this buffer is done
         WDM_T(t_done);
-        if (j + NBUF < J && gt == 0) {
-            issued[b] = (j + NBUF) / NBUF + 1;
-            K::issue(p, bid + (j + NBUF) * stride, buf, full + b);
+        if (gt < 32) {
+            int tn = (int)__shfl_sync(0xffffffffu, ticket, 0);
+            if (tn >= ntiles) tn = -1;
+            if (gt == 0) {
+                tile_of[b] = tn;
+                __threadfence_block();
+                issued[b] = (k + NBUF) / NBUF + 1;
+            }
+            if (tn >= 0) K::issue(p, tn, buf, full + b, gt);
         }
 #ifdef WDM_TRACE
-        if (gt == 0) trace_put(p.tag, grp, NG, j / NG, 0, t_top, t_data, t_done, clock64());
+        if (gt == 0) trace_put(p.tag, grp, NG, k / NG, 0, t_top, t_data, t_done, clock64());
 #endif
+    }
+    // the last CTA to leave rewinds the ticket counter for the next launch on this stream
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned int left = atomicAdd(p.ticket + 1, 1u);
+        if (left == gridDim.x - 1) { p.ticket[0] = 0; p.ticket[1] = 0; }
     }
 }
 
 // ---------------------------------------------------------------- shared building blocks
 
-// Asynchronous tile load by ONE thread (the caller elects it): TMA boxes for strided tiles, one bulk copy per
-// pencil for contiguous tiles (their shared-memory lines are padded, which a box cannot express).  `bid` is the
+// Asynchronous tile load by the first warp of a group (lane = gt < 32): lane 0 announces the byte count and issues
+// the TMA boxes of a strided tile; a contiguous tile is one bulk copy per pencil (its shared-memory lines are
+// padded, which a box cannot express), lane l issuing pencils l, l + 32, ....  `bid` is the
 // tile index, ROWS the number of points along the sweep axis to fetch, tm1 the one-row box used when ROWS is
 // not a multiple of the main box (complex-to-real: N/2 + 1 rows).
 template <class C, int AX, int ROWS>
 __device__ __forceinline__ void tile_load(cx<typename C::T> *S, const cx<typename C::T> *src, const CUtensorMap *tm, const CUtensorMap *tm1,
-                                          int bid, uint64_t *bar)
+                                          int bid, uint64_t *bar, int lane)
 {
     using T = typename C::T;
     using L = Lay<C, AX>;
     using TL = Tile<C, AX>;
     constexpr int W = C::W;
     constexpr uint32_t BYTES = (uint32_t)((size_t)ROWS * W * sizeof(cx<T>));
-    mbar_expect_tx(bar, BYTES);
+    if (lane == 0) mbar_expect_tx(bar, BYTES);
     if constexpr (ax_strided(AX)) {
+        if (lane != 0) return;
         constexpr int EVEN = ROWS & ~1;                                  // ROWS = N, or N/2 + 1
         constexpr int RB = EVEN < 256 ? EVEN : 256;                      // rows per box (as encoded on the host)
         constexpr int FULL = ROWS / RB;
@@ -243,8 +285,7 @@ __device__ __forceinline__ void tile_load(cx<typename C::T> *S, const cx<typenam
         }
     } else {
         const TL tile(bid);
-#pragma unroll 4
-        for (int l = 0; l < W; ++l)
+        for (int l = lane; l < W; l += 32)
             bulk_load(S + L::idx(0, l), src + tile.at(0, l), (uint32_t)(ROWS * sizeof(cx<T>)), bar);
     }
 }
@@ -328,10 +369,10 @@ struct PsiK {
     static constexpr bool KEEP_TW = PAIR && !RHO;
     using Pers = PairTw<C, KEEP_TW>;
 
-    // (one thread)
-    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar)
+    // (first warp of the group, lane = gt)
+    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar, int lane)
     {
-        tile_load<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, &p.tmap, &p.tmap2, t, bar);
+        tile_load<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, &p.tmap, &p.tmap2, t, bar, lane);
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &p, int t, int gt, Pre &pre)
     {
@@ -548,10 +589,10 @@ struct HK {
     using Pre = NoPre;
     static constexpr bool PAIR = ax_strided(AX) && pair_ok<C>();
     using Pers = PairTw<C, PAIR>;
-    // (one thread)
-    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar)
+    // (first warp of the group, lane = gt)
+    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar, int lane)
     {
-        tile_load<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, &p.tmap, &p.tmap2, t, bar);
+        tile_load<C, AX, N>(reinterpret_cast<cx<T> *>(buf), p.data, &p.tmap, &p.tmap2, t, bar, lane);
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
     template <class HOOK>
@@ -650,9 +691,9 @@ struct C2RK {
     using Pre = NoPre;
     static constexpr bool PAIR = pair_ok<C>();          // packed line gt % (W/2), butterfly gt / (W/2): the PairTw twiddles
     using Pers = PairTw<C, PAIR>;
-    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar)
+    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar, int lane)
     {
-        tile_load<C, AX_X, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf + PACKED_BYTES), p.H, &p.tmap, &p.tmap2, t, bar);
+        tile_load<C, AX_X, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf + PACKED_BYTES), p.H, &p.tmap, &p.tmap2, t, bar, lane);
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
     template <class HOOK>

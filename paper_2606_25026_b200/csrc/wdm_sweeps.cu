@@ -132,8 +132,9 @@ int chain_lag(int stages, int planes, int requested)
     int safe = grid / kTilesPerPlane + 1;                                   // lag * tpu + 1 > grid
     int lag = requested;
     if (lag <= 0) {
-        int inflight = (C::NG + 1) * grid;
-        lag = (inflight + inflight / 8) / (kTilesPerPlane * stages) + 1;
+        int inflight = (C::NG + 1) * grid;                                  // measured optimum: about twice the tiles in flight
+        lag = 2 * inflight / (kTilesPerPlane * stages) + 1;
+        if (lag > planes / 2) lag = planes / 2;                             // small grids: keep the stages overlapped
     }
     if (lag < safe) lag = safe;
     if (lag >= planes) return 0;
