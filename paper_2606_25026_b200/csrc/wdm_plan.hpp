@@ -25,7 +25,7 @@ struct Fact {
     X(32, 4, 1, 8, 16, 128, 2, 4)   \
     X(64, 8, 1, 8, 16, 128, 2, 4)   \
     X(128, 8, 1, 16, 16, 128, 2, 2) \
-    X(256, 16, 1, 16, 16, 256, 2, 1) \
+    X(256, 16, 1, 16, 16, 128, 2, 2) \
     X(512, 16, 1, 32, 16, 256, 2, 1) \
     X(1024, 32, 1, 32, 8, 256, 2, 1)
 #define WDM_FACT_C128(X)            \
