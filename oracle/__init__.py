@@ -43,6 +43,7 @@ def lib():
             "wdmo_step": [vp, i, d], "wdmo_get_psi": [vp, dp], "wdmo_get_density": [vp, dp],
             "wdmo_get_potential": [vp, dp], "wdmo_get_particles": [vp, dp, dp],
             "wdmo_get_accel": [vp, dp], "wdmo_threads": [],
+            "wdmo_set_kick_terms": [vp, d, dp, d, i],
         }
         for name, args in sig.items():
             fn = getattr(_lib, name)
@@ -151,6 +152,11 @@ class Oracle:
         else:
             m = _f64(mass)
             _check(lib().wdmo_set_particles(self._h, self.np_, _dp(pos), _dp(vel), _dp(m), 0.0), "set_particles")
+
+    def set_kick_terms(self, kappa=0.0, phi_ext=None, absorb_alpha=0.0, absorb_nb=50):
+        """V = Phi + phi_ext + kappa |psi|^2 in the kicks (Eq. 13-14); absorbing layer of Eq. 22 after every step."""
+        pe = None if phi_ext is None else _f64(phi_ext)
+        _check(lib().wdmo_set_kick_terms(self._h, float(kappa), _dp(pe), float(absorb_alpha), int(absorb_nb)), "set_kick_terms")
 
     def step(self, nsteps, dt):
         _check(lib().wdmo_step(self._h, nsteps, dt), "step")

@@ -53,6 +53,11 @@ typedef struct wdmo_ctx {
     long long np;
     double *pos, *vel, *acc, *mass; /* np x 3, np */
     int have_psi, stale;
+    /* extra kick terms (Eq. 13-14, Eq. 22, Alg. 1 l.15-18; readings G26-G28) */
+    double kappa;        /* local self-interaction: V += kappa |psi|^2                         */
+    double *phi_ext;     /* static external potential added to the Poisson potential, or NULL  */
+    double alpha;        /* absorbing-layer coefficient (0 = no layer)                          */
+    int nb;              /* absorbing-layer transition width L / nb                             */
 } wdmo_ctx;
 
 static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
@@ -331,6 +336,7 @@ int wdmo_destroy(wdmo_ctx *c)
     if (!c) return WDMO_OK;
     free(c->psi); free(c->work); free(c->rho); free(c->phi);
     free(c->pos); free(c->vel); free(c->acc); free(c->mass);
+    free(c->phi_ext);
     free(c);
     return WDMO_OK;
 }
@@ -382,6 +388,9 @@ static int update_potential(wdmo_ctx *c)
     if (c->np > 0) cic_deposit(c->rho, c->N, c->L, c->np, c->pos, c->mass);
     int rc = poisson(c->rho, c->phi, c->work, c->N, c->L, c->G);
     if (rc) return rc;
+    /* Phi_total = Phi_DM + Phi_ext (Alg. 1 l.15); particles feel the total as well (G27) */
+    if (c->phi_ext)
+        for (size_t i = 0; i < c->n; ++i) c->phi[i] += c->phi_ext[i];
     if (c->np > 0) cic_gather(c->phi, c->N, c->L, c->np, c->pos, c->acc);
     return WDMO_OK;
 }
@@ -401,7 +410,9 @@ static void half_kick(wdmo_ctx *c, double h)
 {
 #pragma omp parallel for schedule(static)
     for (long long i = 0; i < (long long)c->n; ++i) {
-        double th = -c->phi[i] * h / c->mu;
+        double re = creal(c->psi[i]), im = cimag(c->psi[i]);
+        double V = c->phi[i] + c->kappa * (re * re + im * im);      /* Eq. 13-14: V = Phi_total + kappa |psi|^2 */
+        double th = -V * h / c->mu;
         c->psi[i] *= cos(th) + I * sin(th);
     }
     for (long long i = 0; i < 3 * c->np; ++i) c->vel[i] += c->acc[i] * h;
@@ -431,6 +442,44 @@ static int drift(wdmo_ctx *c, double dt)
     return WDMO_OK;
 }
 
+/* one axis of Eq. 22: b(x) = 2 - tanh((x + L/2)/w) + tanh((x - L/2)/w), w = L/nb: 0 inside, -> 1 at the faces */
+static double absorb_profile(double x, double L, int nb)
+{
+    double w = L / (double)nb;
+    return 2.0 - tanh((x + 0.5 * L) / w) + tanh((x - 0.5 * L) / w);
+}
+
+/* psi *= B(x), B = exp(-alpha (b(x) + b(y) + b(z)) dt)   (Eq. 22; Alg. 1 l.17-18; G28) */
+static void absorb(wdmo_ctx *c, double dt)
+{
+    int N = c->N;
+    for (int ix = 0; ix < N; ++ix)
+        for (int iy = 0; iy < N; ++iy)
+            for (int iz = 0; iz < N; ++iz) {
+                double x = -0.5 * c->L + ix * c->dx, y = -0.5 * c->L + iy * c->dx, z = -0.5 * c->L + iz * c->dx;
+                double b = absorb_profile(x, c->L, c->nb) + absorb_profile(y, c->L, c->nb) + absorb_profile(z, c->L, c->nb);
+                c->psi[((size_t)ix * N + iy) * N + iz] *= exp(-c->alpha * b * dt);
+            }
+}
+
+/* kappa: self-interaction strength; phi_ext: N^3 values or NULL; alpha = 0 switches the absorbing layer off */
+int wdmo_set_kick_terms(wdmo_ctx *c, double kappa, const double *phi_ext, double alpha, int nb)
+{
+    if (!c || alpha < 0 || (alpha > 0 && nb < 1)) return WDMO_EINVAL;
+    c->kappa = kappa;
+    c->alpha = alpha;
+    c->nb = nb;
+    free(c->phi_ext);
+    c->phi_ext = NULL;
+    if (phi_ext) {
+        c->phi_ext = (double *)malloc(c->n * sizeof(double));
+        if (!c->phi_ext) return WDMO_ENOMEM;
+        memcpy(c->phi_ext, phi_ext, c->n * sizeof(double));
+    }
+    c->stale = 1;
+    return WDMO_OK;
+}
+
 int wdmo_step(wdmo_ctx *c, int nsteps, double dt)
 {
     if (!c || nsteps < 0) return WDMO_EINVAL;
@@ -443,6 +492,7 @@ int wdmo_step(wdmo_ctx *c, int nsteps, double dt)
         rc = update_potential(c);               /* (c) rho, Phi^{n+1}, a^{n+1}               */
         if (rc) return rc;
         half_kick(c, 0.5 * dt);                 /* (d) with the new Phi + closing half kick  */
+        if (c->alpha > 0) absorb(c, dt);        /* Alg. 1 l.17-18                            */
     }
     return WDMO_OK;
 }

@@ -326,3 +326,93 @@ def test_kick_sign_and_half_step():
     assert relerr(ratio, np.exp(-1j * phi * dt / mu)) < 1e-5
     assert np.max(np.abs(phi)) * dt / mu > 1e-3          # the phase is resolvable
     assert phi[4, 4, 4] == phi.min() < 0                 # attractive well at the particle
+
+
+# ---------------------------------------------------------------- P11-P13: the extra kick terms
+
+def test_p11_self_interaction_plane_wave_closed_form():
+    """V = kappa |psi|^2 (Eq. 14): for psi = A e^{ik.x} the density is uniform, so Phi = 0 and
+    psi(t) = A exp(i(k.x - mu k^2 t/2 - kappa A^2 t/mu)) exactly, for any dt (the split step is exact here)."""
+    N, L, mu, kappa, A = 16, 1.3, 0.7, 2.5, 0.8
+    X, Y, Z = grid(N, L)
+    n = np.array([2, -1, 3]); k = 2 * np.pi * n / L
+    psi0 = A * np.exp(1j * (k[0] * X + k[1] * Y + k[2] * Z))
+    for nsteps, dt in ((1, 0.05), (7, 0.011)):
+        o = oracle.Oracle(N, L, mu, 1.0 / FOUR_PI)
+        o.set_kick_terms(kappa=kappa)
+        o.set_psi(psi0)
+        o.step(nsteps, dt)
+        t = nsteps * dt
+        exact = psi0 * np.exp(-1j * (0.5 * mu * (k @ k) * t + kappa * A * A * t / mu))
+        assert relerr(o.psi(), exact) < 1e-12
+    # sign: an attractive interaction (kappa < 0) advances the phase the other way
+    o = oracle.Oracle(N, L, mu, 0.0); o.set_kick_terms(kappa=-kappa); o.set_psi(psi0); o.step(1, 0.05)
+    exact = psi0 * np.exp(-1j * (0.5 * mu * (k @ k) * 0.05 - kappa * A * A * 0.05 / mu))
+    assert relerr(o.psi(), exact) < 1e-12
+
+
+def test_p12_external_potential_harmonic_ground_state_second_order():
+    """Phi_ext = omega^2 r^2 / 2 (Eq. 13 with a static V): the Gaussian of width a^2 = mu/omega is stationary,
+    psi(t) = psi0 exp(-3 i omega t / 2).  The split step reaches it with an error that falls 4x per halving
+    of dt, which pins the sign and the 1/mu of the external term and its place in the potential."""
+    N, L, mu, a = 32, 1.0, 1.0, 0.06
+    omega = mu / a ** 2
+    X, Y, Z = grid(N, L)
+    r2 = X ** 2 + Y ** 2 + Z ** 2
+    psi0 = np.exp(-r2 / (2 * a * a)).astype(complex)
+    T = 1.0 / omega
+    errs = []
+    for nsteps in (8, 16, 32):
+        o = oracle.Oracle(N, L, mu, 0.0)
+        o.set_kick_terms(phi_ext=0.5 * omega ** 2 * r2)
+        o.set_psi(psi0)
+        o.step(nsteps, T / nsteps)
+        errs.append(relerr(o.psi(), psi0 * np.exp(-1.5j * omega * T)))
+        assert relerr(o.potential(), 0.5 * omega ** 2 * r2) < 1e-15      # G = 0: Phi_total is the external term
+    assert errs[2] < 2e-4
+    assert 3.5 < errs[0] / errs[1] < 4.5 and 3.5 < errs[1] / errs[2] < 4.5
+
+
+def test_p12_particles_feel_the_external_potential():
+    """Phi_total = Phi_DM + Phi_ext (Alg. 1 l.15) is what the particles gather: massless particle on a node of
+    A cos(k x) gets a = A sin(k x_i) sin(k dx)/dx (central difference of the cosine)."""
+    N, L, A = 16, 1.0, 0.3
+    dx = L / N
+    X, Y, Z = grid(N, L)
+    kk = 2 * np.pi * 3 / L
+    o = oracle.Oracle(N, L, 1.0, 0.0)
+    o.set_kick_terms(phi_ext=A * np.cos(kk * X))
+    o.set_psi(np.ones((N, N, N), complex))
+    xi = -0.5 * L + 5 * dx
+    o.set_particles(np.array([[xi, 0.0, 0.0]]), np.zeros((1, 3)), 0.0)
+    o.step(0, 0.0)
+    acc = o.accel()
+    assert abs(acc[0, 0] - A * np.sin(kk * xi) * np.sin(kk * dx) / dx) < 1e-12
+    assert abs(acc[0, 1]) < 1e-13 and abs(acc[0, 2]) < 1e-13
+
+
+def test_p13_absorbing_layer_special_points():
+    """Eq. 22 after every step.  From a uniform field (the drift leaves it uniform, G = 0) one step gives
+    psi = B(x).  What the formula fixes without retyping it: B = 1 deep inside; on a face (x = -L/2, the
+    other two coordinates inside) b = 2 - tanh(0) + tanh(-nb) = 1, so B = e^{-alpha dt}; on an edge
+    e^{-2 alpha dt}; at the corner e^{-3 alpha dt}; B is even in every coordinate; the norm only decreases."""
+    N, L, alpha, nb, dt = 32, 2.0, 10.0, 50, 0.013
+    o = oracle.Oracle(N, L, 1.0, 0.0)
+    o.set_kick_terms(absorb_alpha=alpha, absorb_nb=nb)
+    o.set_psi(np.ones((N, N, N), complex))
+    o.step(1, dt)
+    B = o.psi()
+    assert np.max(np.abs(B.imag)) < 1e-15
+    B = B.real
+    m = N // 2
+    assert abs(B[m, m, m] - 1.0) < 1e-14 and abs(B[m - 5, m + 6, m + 3] - 1.0) < 1e-12
+    e = math.exp(-alpha * dt)
+    assert abs(B[0, m, m] - e) < 1e-12 and abs(B[m, 0, m] - e) < 1e-12 and abs(B[m, m, 0] - e) < 1e-12
+    assert abs(B[0, 0, m] - e ** 2) < 1e-12 and abs(B[0, 0, 0] - e ** 3) < 1e-12
+    for i in range(1, N // 2):                    # x_i = -x_{N-i}: even profile
+        assert abs(B[i, m, m] - B[N - i, m, m]) < 1e-13
+    assert np.all(np.diff(B[: m + 1, m, m]) >= -1e-15)       # rises monotonically from the face to the centre
+    # several steps: the layer only removes norm (the drift in between is unitary)
+    n0 = float(np.sum(np.abs(o.psi()) ** 2))
+    o.step(3, dt)
+    assert float(np.sum(np.abs(o.psi()) ** 2)) < n0
