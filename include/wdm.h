@@ -91,6 +91,18 @@ int wdm_get_density_host(wdm_ctx *ctx, void *rho_out_host);
 int wdm_get_potential_host(wdm_ctx *ctx, void *phi_out_host);
 int wdm_get_particles_host(wdm_ctx *ctx, void *pos_out_host, void *vel_out_host);
 
+/* Extra terms of the potential kick (generalised equation, Eq. 13-14) and the absorbing
+ * layer (Eq. 22; Alg. 1 l.15-18).  All act inside the fused kick: no extra pass over psi.
+ *   kappa        local self-interaction, V += kappa |psi|^2 (potential units, like Phi; any sign)
+ *   phi_ext_dev  static external potential, N^3 reals in the layout of Phi, or NULL.  NOT copied: the
+ *                buffer must stay valid and unchanged while it is set.  It is added to the Poisson
+ *                potential (Phi_total = Phi_DM + Phi_ext): psi and the particles feel the sum, and
+ *                wdm_get_potential returns the sum.
+ *   absorb_alpha, absorb_nb   after every step psi *= exp(-alpha (b(x) + b(y) + b(z)) dt) with
+ *                b(x) = 2 - tanh((x + L/2)/w) + tanh((x - L/2)/w), w = L/absorb_nb; alpha = 0: off.
+ * Defaults: 0, NULL, 0.  Marks the potential stale (recomputed by the next step / get). */
+int wdm_set_kick_terms(wdm_ctx *ctx, double kappa, const void *phi_ext_dev, double absorb_alpha, int absorb_nb);
+
 /* Execution mode of the plane-local sweeps (no effect on results beyond rounding order).
  * mode is a bit mask.  Bit 0 (1): the z and y sweeps of psi (Eq. 18(b)) run as one
  * kernel.  Bit 1 (2): the y-forward, z-Green, y-inverse sweeps of the Poisson solve (Eq. 18(c)

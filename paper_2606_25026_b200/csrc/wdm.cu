@@ -7,6 +7,7 @@
 //   psi sweep x + rho = |psi|^2 + rho_p + real-to-complex x-spectrum -> H
 //   H sweep y forward, H sweep z forward . Green . inverse, H sweep y inverse, x complex-to-real -> Phi
 // and once at the end the closing half kick.  Nothing synchronises with the host.
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -46,6 +47,20 @@ __global__ void k_kick(cx<T> *psi, const T *phi, T coef, size_t n)
 {
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
         stv(psi + i, rotate_neg(ldv(psi + i), ldg(phi + i) * coef));
+}
+
+// general form (extra kick terms, see SweepParams::kick_extra); mask = 3 N axis factors or nullptr
+template <typename T>
+__global__ void k_kick_general(cx<T> *psi, const T *phi, T coef, T kd, T ka, const T *mask, int N, size_t n)
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        T m = (T)1;
+        if (mask) {
+            const size_t z = i % N, y = (i / N) % N, x = i / ((size_t)N * N);
+            m = ldg(mask + x) * ldg(mask + N + y) * ldg(mask + 2 * N + z);
+        }
+        stv(psi + i, kick_general(ldv(psi + i), ldg(phi + i), m, coef, kd, ka));
+    }
 }
 
 template <typename T>
@@ -116,6 +131,13 @@ struct wdm_ctx {
     double phase_dt = 0;
     bool phase_valid = false, have_psi = false, stale = true;
     // L2-chained sweeps (wdm_chain.cuh): completion counters, launch epochs, lag per chain (0: separate sweeps)
+    // extra kick terms (wdm_set_kick_terms; readings G26-G28)
+    double kappa = 0, alpha = 0;
+    int absorb_nb = 50;
+    const void *phi_ext = nullptr;            // caller-owned N^3 reals or nullptr
+    void *mask = nullptr;                     // 3 N axis factors exp(-alpha b dt) for mask_dt
+    double mask_dt = 0;
+    bool mask_valid = false;
     // TMA descriptors (see SweepParams): psi along y / x, H along y / x, H single row along x
     CUtensorMap tm_psi_y, tm_psi_x, tm_h_y, tm_h_x, tm_h_x1;
     unsigned int *chain_done = nullptr;       // [N] for psi z->y, then [2 (N/2+1)] for H y->z->y
@@ -163,7 +185,7 @@ static size_t grid_bytes(int N, int dtype, long long max_particles)
     size_t n = (size_t)N * N * N, nH = (size_t)(N / 2 + 1) * N * N, c = csize(dtype), r = rsize(dtype);
     size_t b = align_up(n * c) + align_up(n * r) + align_up(nH * c);
     b += 3 * align_up((size_t)N * c) + 2 * align_up((size_t)N * r) + align_up((size_t)N * 2) + 256;
-    b += align_up((size_t)(2 * N + 2 + 8) * sizeof(unsigned int));
+    b += align_up((size_t)(2 * N + 2 + 8) * sizeof(unsigned int)) + align_up((size_t)3 * N * r);
     if (max_particles > 0) b += align_up(n * r) + particle_bytes(N, dtype, max_particles);
     return b + 4096;
 }
@@ -297,6 +319,27 @@ static int ensure_phase(wdm_ctx *c, double dt)
     return WDM_OK;
 }
 
+// axis factors of the absorbing layer, exp(-alpha b(x_i) dt) with b(x) = 2 - tanh((x + L/2)/w) + tanh((x - L/2)/w),
+// w = L/nb (Eq. 22): the same table along x, y and z of the cubic box
+template <typename T>
+static int ensure_mask(wdm_ctx *c, double dt)
+{
+    if (!(c->alpha > 0) || (c->mask_valid && c->mask_dt == dt)) return WDM_OK;
+    const int N = c->N;
+    std::vector<T> m(3 * (size_t)N);
+    const double w = c->L / (double)c->absorb_nb;
+    for (int i = 0; i < N; ++i) {
+        const double x = -0.5 * c->L + (c->L / N) * i;
+        const double b = 2.0 - std::tanh((x + 0.5 * c->L) / w) + std::tanh((x - 0.5 * c->L) / w);
+        m[i] = m[N + i] = m[2 * N + i] = (T)std::exp(-c->alpha * b * dt);
+    }
+    CU(c, cudaMemcpyAsync(c->mask, m.data(), m.size() * sizeof(T), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    c->mask_dt = dt;
+    c->mask_valid = true;
+    return WDM_OK;
+}
+
 template <typename T>
 static SweepParams<T> base_params(wdm_ctx *c)
 {
@@ -315,6 +358,7 @@ static SweepParams<T> base_params(wdm_ctx *c)
     p.rho_p = c->part.n > 0 ? (const T *)c->part.rho_p : nullptr;
     p.rho_mean = (const T *)((const unsigned char *)c->rho_mean + 16);
     p.ticket = c->chain_done + 2 * N + 2;
+    p.phi_ext = (const T *)c->phi_ext;
     return p;
 }
 
@@ -388,7 +432,8 @@ static int refresh(wdm_ctx *c)
         if (rc) return rc;
     } else {
         Timed t(c, S_MISC);
-        CU(c, cudaMemsetAsync(c->phi, 0, c->n * sizeof(T), c->stream));
+        if (c->phi_ext) CU(c, cudaMemcpyAsync(c->phi, c->phi_ext, c->n * sizeof(T), cudaMemcpyDeviceToDevice, c->stream));
+        else CU(c, cudaMemsetAsync(c->phi, 0, c->n * sizeof(T), c->stream));
     }
     c->stale = false;
     return WDM_OK;
@@ -401,28 +446,38 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
     if (rc || nsteps == 0) return rc;
     rc = ensure_phase<T>(c, dt);
     if (rc) return rc;
+    rc = ensure_mask<T>(c, dt);
+    if (rc) return rc;
     const long long N = c->N;
     const bool grav = c->G > 0;
+    const bool have_phi = grav || c->phi_ext != nullptr;                 // particles and psi feel a potential
+    const bool layer = c->alpha > 0;
+    const bool kicks = have_phi || c->kappa != 0.0 || layer;
     for (int s = 0; s < nsteps; ++s) {
-        const double kdt = (s == 0 ? 0.5 : 1.0) * dt;     // merged closing + opening half kicks (G21)
+        // merged closing (h_d, of the previous step) + opening (h_a) half kicks (G21); the layer sits between them
+        const double hd = s == 0 ? 0.0 : 0.5 * dt, ha = 0.5 * dt, kdt = hd + ha;
         if (c->part.n > 0) {
             // v += a(Phi^n, x^n) kdt ; x += v dt ; wrap ; then deposit x^{n+1}  (readings G14-G16)
-            { Timed t(c, S_PART_PUSH); CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, grav ? kdt : 0.0, dt, c->stream)); }
+            { Timed t(c, S_PART_PUSH); CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, have_phi ? kdt : 0.0, dt, c->stream)); }
             if (grav) { rc = particles_deposit<T>(c); if (rc) return rc; }
         }
         {
             SweepParams<T> pz = base_params<T>(c), py = base_params<T>(c);
             pz.data = (cx<T> *)c->psi;
             pz.kick = (T)(kdt / c->mu);
+            pz.kself_d = (T)(c->kappa * hd / c->mu);
+            pz.kself_a = (T)(c->kappa * ha / c->mu);
+            pz.mask = layer && s > 0 ? (const T *)c->mask : nullptr;
+            pz.kick_extra = (c->kappa != 0.0 || pz.mask != nullptr) ? 1 : 0;
             py.data = (cx<T> *)c->psi;
             py.tmap = c->tm_psi_y;
             if (c->lag_psi > 0) {
                 ChainCtl ctl{c->chain_done, ++c->epoch_psi * (unsigned int)(N / c->tab->fact.W), c->lag_psi};
                 pz.tag = S_PSI_ZY;
                 Timed t(c, S_PSI_ZY);
-                CU(c, c->tab->psi_zy(&pz, &py, grav ? 1 : 0, &ctl, c->stream));
+                CU(c, c->tab->psi_zy(&pz, &py, kicks ? 1 : 0, &ctl, c->stream));
             } else {
-                { pz.tag = S_PSI_Z; Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, grav ? 1 : 0, c->stream)); }
+                { pz.tag = S_PSI_Z; Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? 1 : 0, c->stream)); }
                 { py.tag = S_PSI_Y; Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
             }
         }
@@ -437,16 +492,20 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             CU(c, c->tab->psi_strided(&p, 1, c->stream));
         }
     }
-    if (grav) {
-        {
-            Timed t(c, S_KICK);
+    if (kicks) {
+        // closing half kick of the last step, then its absorbing layer
+        Timed t(c, S_KICK);
+        if (c->kappa != 0.0 || layer)
+            k_kick_general<T><<<148 * 8, 256, 0, c->stream>>>((cx<T> *)c->psi, (const T *)c->phi, (T)(0.5 * dt / c->mu),
+                                                                (T)(c->kappa * 0.5 * dt / c->mu), (T)0, layer ? (const T *)c->mask : nullptr,
+                                                                c->N, c->n);
+        else
             k_kick<T><<<148 * 8, 256, 0, c->stream>>>((cx<T> *)c->psi, (const T *)c->phi, (T)(0.5 * dt / c->mu), c->n);
-            CU(c, cudaGetLastError());
-        }
-        if (c->part.n > 0) {
-            Timed t(c, S_PART_PUSH);
-            CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, 0.5 * dt, 0.0, c->stream));
-        }
+        CU(c, cudaGetLastError());
+    }
+    if (have_phi && c->part.n > 0) {
+        Timed t(c, S_PART_PUSH);
+        CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, 0.5 * dt, 0.0, c->stream));
     }
     return WDM_OK;
 }
@@ -504,7 +563,8 @@ static int create_common(wdm_ctx **out, int N, double L, double mu, double G, in
         (rc = ctx_alloc(c, &c->twB, N * cs)) || (rc = ctx_alloc(c, &c->phase, N * cs)) ||
         (rc = ctx_alloc(c, &c->ksq_pos, N * rs)) || (rc = ctx_alloc(c, &c->ksq_nat, N * rs)) ||
         (rc = ctx_alloc(c, (void **)&c->pos_of_k, N * 2)) || (rc = ctx_alloc(c, &c->rho_mean, 64)) ||
-        (rc = ctx_alloc(c, (void **)&c->chain_done, (size_t)(2 * N + 2 + 8) * sizeof(unsigned int))))
+        (rc = ctx_alloc(c, (void **)&c->chain_done, (size_t)(2 * N + 2 + 8) * sizeof(unsigned int))) ||
+        (rc = ctx_alloc(c, &c->mask, (size_t)3 * N * rs)))
         return bail(rc);
     if (cudaMemset(c->chain_done, 0, (size_t)(2 * N + 2 + 8) * sizeof(unsigned int)) != cudaSuccess)
         return bail(fail(c, WDM_ECUDA, "cudaMemset of the chain counters failed"));
@@ -677,6 +737,20 @@ extern "C" int wdm_launch_count(wdm_ctx *c, long long *out)
 {
     if (!c || !out) return WDM_EINVAL;
     *out = c->launches;
+    return WDM_OK;
+}
+
+extern "C" int wdm_set_kick_terms(wdm_ctx *c, double kappa, const void *phi_ext_dev, double absorb_alpha, int absorb_nb)
+{
+    if (!c) return WDM_EINVAL;
+    if (kappa != kappa || !(absorb_alpha >= 0) || (absorb_alpha > 0 && absorb_nb < 1))
+        return fail(c, WDM_EINVAL, "need a finite kappa, absorb_alpha >= 0 and absorb_nb >= 1");
+    c->kappa = kappa;
+    c->phi_ext = phi_ext_dev;
+    c->alpha = absorb_alpha;
+    c->absorb_nb = absorb_nb;
+    c->mask_valid = false;
+    c->stale = true;                 // Phi_total changes with the external term
     return WDM_OK;
 }
 

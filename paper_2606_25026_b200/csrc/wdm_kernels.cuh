@@ -78,6 +78,16 @@ WDM_DEV cx<double> rotate_neg(cx<double> v, double th)
     sincos(th, &s, &c);
     return mk<double>(v.x * c + v.y * s, v.y * c - v.x * s);
 }
+// the general kick of one element (see SweepParams::kick_extra); m = product of the three axis factors or 1
+template <typename T>
+WDM_DEV cx<T> kick_general(cx<T> v, T phi, T m, T kick, T kd, T ka)
+{
+    const T a2 = v.x * v.x + v.y * v.y;
+    const T th = phi * kick + a2 * (kd + ka * m * m);
+    cx<T> r = rotate_neg(v, th);
+    return mk<T>(r.x * m, r.y * m);
+}
+
 // g / k2 of the Green's function (Eq. 23).  Single precision: one reciprocal (MUFU.RCP, 1 ulp)
 // and a multiply instead of the IEEE division sequence -- 2 ulp on a factor whose tolerance is 2e-5.
 WDM_DEV float green_over(float g, float k2) { return __fdividef(g, k2); }
@@ -93,6 +103,13 @@ struct SweepParams {
     const cx<T> *phase;        // psi sweeps: exp(-i mu k^2 dt/2)/N in position order
     const T *phi;              // KICK: potential, same shape as psi
     T kick;                    // KICK: theta = phi * kick   (dt/(2 mu) or dt/mu)
+    // extra kick terms (Eq. 13-14, Eq. 22; readings G26-G28), used only when kick_extra != 0.  A merged kick is the
+    // closing half kick of one step (weight kself_d, then the absorbing layer m) and the opening one of the next
+    // (kself_a, on the attenuated field):  psi <- m psi exp(-i (phi kick + |psi|^2 (kself_d + kself_a m^2)))
+    int kick_extra;
+    T kself_d, kself_a;        // kappa h_d / mu, kappa h_a / mu
+    const T *mask;             // 3 N reals, exp(-alpha b(x_axis) dt) along x, y, z; nullptr: no layer in this kick
+    const T *phi_ext;          // C2R: static external potential added to Phi on its way out, or nullptr
     const T *rho_p;            // RHO: particle mesh density or nullptr
     const T *rho_mean;         // RHO: device scalar <rho>, subtracted before the transform (Eq. 23)
     cx<T> *H;                  // RHO / C2R: half spectrum

@@ -420,8 +420,23 @@ struct PsiK {
                     split<AX, mA, W>(gt + it * NTG, q, l);
                     cx<T> v[RA];
                     static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = S[L::idx(q + mA * r, l)]; });
-                    if constexpr (KICK)
-                        static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], pre.th[it][r] * p.kick); });
+                    if constexpr (KICK) {
+                        if (p.kick_extra) {
+                            // self-interaction and / or absorbing layer: the pencil of line l is (x, y) = divmod(t W + l, N)
+                            T mxy = (T)1;
+                            if (p.mask) {
+                                const int pen = t * W + l, x = pen / N, y = pen - x * N;
+                                mxy = ldg(p.mask + x) * ldg(p.mask + N + y);
+                            }
+                            static_for<0, RA>([&](auto r_) {
+                                constexpr int r = decltype(r_)::value;
+                                const T m = p.mask ? mxy * ldg(p.mask + 2 * N + q + mA * r) : (T)1;
+                                v[r] = kick_general(v[r], pre.th[it][r], m, p.kick, p.kself_d, p.kself_a);
+                            });
+                        } else {
+                            static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], pre.th[it][r] * p.kick); });
+                        }
+                    }
                     fwd_level_regs<RA, T>(v, q, mA, tb.twA + q, [&](int row, cx<T> y) { S[L::idx(row, l)] = y; });
                 });
             }
@@ -727,15 +742,18 @@ struct C2RK {
         for (int b = gt; b < mA * WP; b += NTG) {
             int l = b % WP, q = b / WP;
             T *gp = p.phi_out + tile.at(q, 2 * l);
-            if constexpr (PAIR)
-                inv_level_w<RA, T>(q, mA, pers.w, [&](int row) { return Sp[row * RSP + l]; },
-                                   [&](int row, cx<T> v) { stv(reinterpret_cast<cx<T> *>(gp + (long long)(row - q) * TL::RSTRIDE), v); });
-            else
-            inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; },
-                             [&](int row, cx<T> v) {
-                                 // Re -> line 2l', Im -> line 2l'+1: one (re, im) pair is two adjacent reals of Phi
-                                 stv(reinterpret_cast<cx<T> *>(gp + (long long)(row - q) * TL::RSTRIDE), v);
-                             });
+            const T *ge = p.phi_ext ? p.phi_ext + tile.at(q, 2 * l) : nullptr;     // Phi_total = Phi_DM + Phi_ext (Alg. 1 l.15)
+            auto out = [&](int row, cx<T> v) {
+                // Re -> line 2l', Im -> line 2l'+1: one (re, im) pair is two adjacent reals of Phi
+                if (ge) {
+                    cx<T> e = ldg(reinterpret_cast<const cx<T> *>(ge + (long long)(row - q) * TL::RSTRIDE));
+                    v.x += e.x;
+                    v.y += e.y;
+                }
+                stv(reinterpret_cast<cx<T> *>(gp + (long long)(row - q) * TL::RSTRIDE), v);
+            };
+            if constexpr (PAIR) inv_level_w<RA, T>(q, mA, pers.w, [&](int row) { return Sp[row * RSP + l]; }, out);
+            else inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; }, out);
         }
     }
 };

@@ -338,3 +338,68 @@ def test_chained_sweeps_match_separate_sweeps(wdm, dtype, N, G):
         e_phi = float((phi_c - phi_s).abs().max() / phi_s.abs().max()) if G > 0 else 0.0
         assert e_psi <= eps and e_phi <= 10 * eps, f"lags {lags}: psi {e_psi}, Phi {e_phi}"
     assert len(used) >= 2
+
+
+# ---------------------------------------------------------------- extra kick terms
+
+def _ext_potential(N, L, amp):
+    x = -0.5 * L + (L / N) * np.arange(N)
+    X, Y, Z = np.meshgrid(x, x, x, indexing="ij")
+    return amp * (np.cos(2 * np.pi * X / L) + 0.5 * np.sin(4 * np.pi * Y / L) * np.cos(2 * np.pi * Z / L) + 3.0 * (X * X + Y * Y + Z * Z))
+
+
+@pytest.mark.parametrize("dtype,N", [("c128", 32), ("c64", 64), ("c64", 128), ("c64", 256)])
+@pytest.mark.parametrize("terms", ["kappa", "ext", "layer", "all", "all_G0"])
+def test_kick_terms_match_oracle(wdm, dtype, N, terms):
+    """Self-interaction, external potential and absorbing layer inside the fused kick (Eq. 13-14, Eq. 22):
+    one call of several steps (merged kicks with the layer between them) and step-by-step calls both match."""
+    if N == 256 and terms not in ("all",):
+        pytest.skip("256^3 only for the combined case")
+    L, mu = 1.3, 0.8
+    G = 0.0 if terms == "all_G0" else 30.0
+    psi0 = (0.3 * wl.random_field(N, dtype, 40 + N) + 1.2).astype(np.complex64 if dtype == "c64" else np.complex128)
+    dt = 0.2 * (L / N) ** 2
+    kw = {}
+    if terms in ("kappa", "all", "all_G0"):
+        kw["kappa"] = -40.0
+    if terms in ("ext", "all", "all_G0"):
+        kw["phi_ext"] = _ext_potential(N, L, 25.0).astype(np.float32 if dtype == "c64" else np.float64)
+    if terms in ("layer", "all", "all_G0"):
+        kw["absorb_alpha"] = 3.0 / dt / 8      # strong enough to matter within a few steps
+        kw["absorb_nb"] = 12
+    nsteps = 4
+    w = wl.Workload(f"kick{N}", N, dtype, nsteps, L=L, hbar_over_m=mu, G=G, psi=psi0)
+    sim, o = pair(wdm, w)
+    sim.set_kick_terms(**kw)
+    o.set_kick_terms(**kw)
+    sim.step(nsteps, dt)
+    o.step(nsteps, dt)
+    t = tol(dtype, nsteps)
+    assert rel(sim.psi().cpu().numpy(), o.psi()) <= t
+    assert rel(sim.potential().cpu().numpy(), o.potential()) <= t
+    # the same steps one call at a time from the same start
+    sim2, _ = pair(wdm, w)
+    sim2.set_kick_terms(**kw)
+    for _ in range(nsteps):
+        sim2.step(1, dt)
+    assert rel(sim2.psi().cpu().numpy(), o.psi()) <= t
+    sim.close(); sim2.close()
+
+
+def test_kick_terms_with_particles(wdm):
+    """Particles feel Phi_total = Phi_DM + Phi_ext (Alg. 1 l.15)."""
+    w = wl.small_coupled(32, dtype="c64")
+    ext = _ext_potential(w.N, w.L, 5.0).astype(np.float32)
+    sim, o = pair(wdm, w, max_particles=len(w.pos))
+    sim.set_kick_terms(kappa=3.0, phi_ext=ext)
+    o.set_kick_terms(kappa=3.0, phi_ext=ext)
+    sim.step(5, w.dt)
+    o.step(5, w.dt)
+    p, v = sim.particles()
+    po, vo = o.particles()
+    d = p.cpu().numpy() - po
+    d -= w.L * np.round(d / w.L)
+    assert np.abs(d).max() <= POS_TOL * w.L
+    assert rel(v.cpu().numpy(), vo) <= 1e-4
+    assert rel(sim.psi().cpu().numpy(), o.psi()) <= tol("c64", 5)
+    sim.close()
