@@ -43,7 +43,7 @@ def lib():
             "wdmo_step": [vp, i, d], "wdmo_get_psi": [vp, dp], "wdmo_get_density": [vp, dp],
             "wdmo_get_potential": [vp, dp], "wdmo_get_particles": [vp, dp, dp],
             "wdmo_get_accel": [vp, dp], "wdmo_threads": [],
-            "wdmo_set_kick_terms": [vp, d, dp, d, i],
+            "wdmo_set_kick_terms": [vp, d, dp, d, i], "wdmo_diagnostics": [vp, dp],
         }
         for name, args in sig.items():
             fn = getattr(_lib, name)
@@ -175,6 +175,12 @@ class Oracle:
         out = np.empty((self.N,) * 3)
         _check(lib().wdmo_get_potential(self._h, _dp(out)), "get_potential")
         return out
+
+    def diagnostics(self):
+        """dict(M, max_rho, max_phi, V, K, Q, dt_max) of the current state (Sect. 3.5-3.6; central differences)."""
+        out = np.zeros(8)
+        _check(lib().wdmo_diagnostics(self._h, _dp(out)), "diagnostics")
+        return dict(zip(("M", "max_rho", "max_phi", "V", "K", "Q", "dt_max"), out[:7]))
 
     def particles(self):
         pos = np.empty((self.np_, 3)); vel = np.empty((self.np_, 3))

@@ -540,6 +540,57 @@ int wdmo_get_accel(wdmo_ctx *c, double *acc)
     return WDMO_OK;
 }
 
+/* Volume-integrated diagnostics of the current state (Sect. 3.5-3.6), gradients by the
+ * second-order central differences of Eq. 21, periodic:
+ *   out[0] M     = sum |psi|^2 dx^3
+ *   out[1] max |psi|^2            out[2] max |Phi_total|           (the maxima of Eq. 26)
+ *   out[3] V     = sum rho Phi dx^3                                 (as printed: no 1/2)
+ *   out[4] K     = 1/2 sum |rho v|^2 / rho dx^3,  rho v = mu Im(psi* grad psi)   (v = mu grad theta)
+ *   out[5] Q     = mu^2/2 sum |grad sqrt(rho)|^2 dx^3              (Eq. 12 with its hbar^2/2m prefactor, per unit m)
+ *   out[6] dt_max of Eq. 26 without the safety factor:
+ *          0.5 min{ 4/(3 pi) dx^2/mu, 2 pi mu / max|Phi|, 2 pi mu / (|kappa| max|psi|^2) }
+ * Phi is refreshed first if stale. */
+int wdmo_diagnostics(wdmo_ctx *c, double *out)
+{
+    if (!c || !out) return WDMO_EINVAL;
+    int rc = refresh(c);
+    if (rc) return rc;
+    int N = c->N;
+    double dx = c->dx, dV = dx * dx * dx, mu = c->mu;
+    double M = 0, V = 0, K = 0, Q = 0, maxrho = 0, maxphi = 0;
+    for (int ix = 0; ix < N; ++ix)
+        for (int iy = 0; iy < N; ++iy)
+            for (int iz = 0; iz < N; ++iz) {
+                size_t i = ((size_t)ix * N + iy) * N + iz;
+                size_t nb[3][2] = {{((size_t)wrap_index(ix + 1, N) * N + iy) * N + iz, ((size_t)wrap_index(ix - 1, N) * N + iy) * N + iz},
+                                   {((size_t)ix * N + wrap_index(iy + 1, N)) * N + iz, ((size_t)ix * N + wrap_index(iy - 1, N)) * N + iz},
+                                   {((size_t)ix * N + iy) * N + wrap_index(iz + 1, N), ((size_t)ix * N + iy) * N + wrap_index(iz - 1, N)}};
+                cplx p = c->psi[i];
+                double rho = creal(p) * creal(p) + cimag(p) * cimag(p);
+                M += rho;
+                V += rho * c->phi[i];
+                if (rho > maxrho) maxrho = rho;
+                if (fabs(c->phi[i]) > maxphi) maxphi = fabs(c->phi[i]);
+                double j2 = 0, g2 = 0;
+                for (int a = 0; a < 3; ++a) {
+                    cplx grad = (c->psi[nb[a][0]] - c->psi[nb[a][1]]) / (2.0 * dx);
+                    double j = mu * cimag(conj(p) * grad);                       /* rho v along axis a */
+                    double gs = (cabs(c->psi[nb[a][0]]) - cabs(c->psi[nb[a][1]])) / (2.0 * dx);   /* grad sqrt(rho) */
+                    j2 += j * j;
+                    g2 += gs * gs;
+                }
+                if (rho > 0) K += 0.5 * j2 / rho;
+                Q += 0.5 * mu * mu * g2;
+            }
+    out[0] = M * dV; out[1] = maxrho; out[2] = maxphi; out[3] = V * dV; out[4] = K * dV; out[5] = Q * dV;
+    double dtm = 4.0 / (3.0 * M_PI) * dx * dx / mu;
+    if (maxphi > 0 && 2.0 * M_PI * mu / maxphi < dtm) dtm = 2.0 * M_PI * mu / maxphi;
+    if (c->kappa != 0 && maxrho > 0 && 2.0 * M_PI * mu / (fabs(c->kappa) * maxrho) < dtm) dtm = 2.0 * M_PI * mu / (fabs(c->kappa) * maxrho);
+    out[6] = 0.5 * dtm;
+    out[7] = 0;
+    return WDMO_OK;
+}
+
 int wdmo_threads(void)
 {
 #ifdef _OPENMP

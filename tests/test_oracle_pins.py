@@ -416,3 +416,51 @@ def test_p13_absorbing_layer_special_points():
     n0 = float(np.sum(np.abs(o.psi()) ** 2))
     o.step(3, dt)
     assert float(np.sum(np.abs(o.psi()) ** 2)) < n0
+
+
+# ---------------------------------------------------------------- P14: diagnostics
+
+def test_p14_diagnostics_plane_wave_closed_forms():
+    """psi = A e^{ik.x}: rho = A^2, rho v = mu A^2 sin(k dx)/dx per axis (central difference of the phase), so
+    K = A^2 mu^2 sum_a (sin(k_a dx)/dx)^2 L^3 / 2, Q = 0, M = A^2 L^3, Phi = 0 => V = 0, max rho = A^2."""
+    N, L, mu, A = 16, 1.3, 0.7, 0.8
+    dx = L / N
+    X, Y, Z = grid(N, L)
+    k = 2 * np.pi * np.array([2, -1, 3]) / L
+    o = oracle.Oracle(N, L, mu, 1.0 / FOUR_PI)
+    o.set_psi(A * np.exp(1j * (k[0] * X + k[1] * Y + k[2] * Z)))
+    d = o.diagnostics()
+    assert abs(d["M"] - A * A * L ** 3) < 1e-12
+    assert abs(d["max_rho"] - A * A) < 1e-14 and d["max_phi"] < 1e-12 and abs(d["V"]) < 1e-12
+    assert abs(d["K"] - 0.5 * A * A * mu * mu * np.sum((np.sin(k * dx) / dx) ** 2) * L ** 3) < 1e-10
+    assert abs(d["Q"]) < 1e-12
+    # Eq. 26: Phi = 0, kappa = 0 -> the kinetic bound alone, 0.5 * 4/(3 pi) dx^2 (m/hbar)
+    assert abs(d["dt_max"] - 0.5 * 4 / (3 * np.pi) * dx * dx / mu) < 1e-15
+
+
+def test_p14_diagnostics_real_gaussian_and_cosine_density():
+    """Real psi: K = 0.  Gaussian psi = exp(-r^2/2a^2): Q -> (mu^2/2) (3/2a^2) pi^{3/2} a^3 with second-order
+    convergence in dx.  rho = r0 + r1 cos(kx): Phi = -4 pi G r1 cos(kx)/k^2, V = int rho Phi = -4 pi G r1^2 L^3/(2 k^2);
+    max|Phi| = 4 pi G r1/k^2 then bounds dt through the second term of Eq. 26."""
+    L, mu, a = 1.0, 0.9, 0.09
+    exact = 0.5 * mu * mu * 1.5 / a ** 2 * np.pi ** 1.5 * a ** 3
+    errs = []
+    for N in (16, 32, 64):
+        X, Y, Z = grid(N, L)
+        o = oracle.Oracle(N, L, mu, 0.0)
+        o.set_psi(np.exp(-(X ** 2 + Y ** 2 + Z ** 2) / (2 * a * a)).astype(complex))
+        d = o.diagnostics()
+        assert abs(d["K"]) < 1e-20
+        errs.append(abs(d["Q"] - exact) / exact)
+    assert errs[2] < 0.05 and 3.0 < errs[1] / errs[2] < 5.0
+    N, G, r0, r1 = 32, 7.0, 2.0, 0.5
+    X, Y, Z = grid(N, L)
+    kk = 2 * np.pi * 3 / L
+    o = oracle.Oracle(N, L, mu, G)
+    o.set_psi(np.sqrt(r0 + r1 * np.cos(kk * X)).astype(complex))
+    d = o.diagnostics()
+    assert abs(d["V"] + 4 * np.pi * G * r1 * r1 * L ** 3 / (2 * kk * kk)) < 1e-10
+    assert abs(d["max_phi"] - 4 * np.pi * G * r1 / kk ** 2) < 1e-10 and abs(d["max_rho"] - (r0 + r1)) < 1e-12
+    o.set_kick_terms(kappa=-1e4)
+    d = o.diagnostics()
+    assert abs(d["dt_max"] - 0.5 * 2 * np.pi * mu / (1e4 * (r0 + r1))) < 1e-15     # third term of Eq. 26 is the smallest
