@@ -103,6 +103,16 @@ int wdm_get_particles_host(wdm_ctx *ctx, void *pos_out_host, void *vel_out_host)
  * Defaults: 0, NULL, 0.  Marks the potential stale (recomputed by the next step / get). */
 int wdm_set_kick_terms(wdm_ctx *ctx, double kappa, const void *phi_ext_dev, double absorb_alpha, int absorb_nb);
 
+/* Diagnostics of the current state (Sect. 3.5-3.6) by one reduction pass on the device; the
+ * gradients are the second-order central differences of Eq. 21.  Synchronises the stream.
+ * out_host[0] M = sum |psi|^2 dx^3       [1] max |psi|^2       [2] max |Phi_total|
+ *         [3] V = sum |psi|^2 Phi dx^3 (as printed: no factor 1/2)
+ *         [4] K = 1/2 sum |rho v|^2/rho dx^3, rho v = (hbar/m) Im(psi* grad psi)
+ *         [5] Q = (hbar/m)^2/2 sum |grad sqrt(rho)|^2 dx^3
+ *         [6] dt_max of Eq. 26, without the safety factor      [7] reserved (0)
+ * The potential is recomputed first if stale.  Particles do not enter (rho is the wave density). */
+int wdm_get_diagnostics(wdm_ctx *ctx, double *out_host);
+
 /* Execution mode of the plane-local sweeps (no effect on results beyond rounding order).
  * mode is a bit mask.  Bit 0 (1): the z and y sweeps of psi (Eq. 18(b)) run as one
  * kernel.  Bit 1 (2): the y-forward, z-Green, y-inverse sweeps of the Poisson solve (Eq. 18(c)

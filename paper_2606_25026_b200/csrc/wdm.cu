@@ -102,6 +102,53 @@ __global__ void k_finish_mean(const double *acc, double inv_cells, double extra_
     *mean = (T)(acc[0] * inv_cells + (acc[1] + extra_mass) * inv_volume);
 }
 
+// Diagnostics of Sect. 3.5-3.6 in one pass over (psi, Phi): per cell rho, rho Phi, the momentum
+// density mu Im(psi* grad psi) and grad sqrt(rho) by the central differences of Eq. 21 (periodic).
+// acc[0..3] = sum rho, sum rho Phi, sum |rho v|^2 / (2 rho), sum mu^2/2 |grad sqrt rho|^2;  mx[0..1] = bit
+// patterns of max rho and max |Phi| as doubles (non-negative doubles order like their bit patterns).
+template <typename T>
+__global__ void __launch_bounds__(256) k_diag(const cx<T> *__restrict__ psi, const T *__restrict__ phi, int N, double mu, double inv2dx,
+                                              double *acc, unsigned long long *mx)
+{
+    const size_t n = (size_t)N * N * N;
+    const int M = N - 1;
+    double s0 = 0, s1 = 0, s2 = 0, s3 = 0, m0 = 0, m1 = 0;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int z = (int)(i % N), y = (int)((i / N) % N), x = (int)(i / ((size_t)N * N));
+        const cx<T> p = ldg(psi + i);
+        const double pr = p.x, pi = p.y, rho = pr * pr + pi * pi, f = ldg(phi + i);
+        const size_t nb[3][2] = {{((size_t)((x + 1) & M) * N + y) * N + z, ((size_t)((x - 1) & M) * N + y) * N + z},
+                                 {((size_t)x * N + ((y + 1) & M)) * N + z, ((size_t)x * N + ((y - 1) & M)) * N + z},
+                                 {((size_t)x * N + y) * N + ((z + 1) & M), ((size_t)x * N + y) * N + ((z - 1) & M)}};
+        double j2 = 0, g2 = 0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const cx<T> u = ldg(psi + nb[a][0]), d = ldg(psi + nb[a][1]);
+            const double gr = ((double)u.x - (double)d.x) * inv2dx, gi = ((double)u.y - (double)d.y) * inv2dx;
+            const double j = mu * (pr * gi - pi * gr);                               // Im(conj(p) * grad)
+            const double gs = (sqrt((double)u.x * u.x + (double)u.y * u.y) - sqrt((double)d.x * d.x + (double)d.y * d.y)) * inv2dx;
+            j2 += j * j;
+            g2 += gs * gs;
+        }
+        s0 += rho;
+        s1 += rho * f;
+        if (rho > 0) s2 += 0.5 * j2 / rho;
+        s3 += 0.5 * mu * mu * g2;
+        m0 = fmax(m0, rho);
+        m1 = fmax(m1, fabs(f));
+    }
+    for (int d = 16; d; d >>= 1) {
+        s0 += __shfl_down_sync(0xffffffffu, s0, d); s1 += __shfl_down_sync(0xffffffffu, s1, d);
+        s2 += __shfl_down_sync(0xffffffffu, s2, d); s3 += __shfl_down_sync(0xffffffffu, s3, d);
+        m0 = fmax(m0, __shfl_down_sync(0xffffffffu, m0, d)); m1 = fmax(m1, __shfl_down_sync(0xffffffffu, m1, d));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(acc, s0); atomicAdd(acc + 1, s1); atomicAdd(acc + 2, s2); atomicAdd(acc + 3, s3);
+        atomicMax(mx, (unsigned long long)__double_as_longlong(m0));
+        atomicMax(mx + 1, (unsigned long long)__double_as_longlong(m1));
+    }
+}
+
 enum Slot { S_PSI_Z, S_PSI_Y, S_PSI_X_RHO, S_H_Y_FWD, S_H_Z_GREEN, S_H_Y_INV, S_C2R, S_KICK, S_PART_PUSH,
             S_PART_DEPOSIT, S_PART_SORT, S_MISC, S_PSI_ZY, S_H_YZY, S_COUNT };
 static const char *kSlotNames[S_COUNT] = {"psi_sweep_z_kick", "psi_sweep_y", "psi_sweep_x_rho_r2c", "poisson_y_fwd",
@@ -737,6 +784,41 @@ extern "C" int wdm_launch_count(wdm_ctx *c, long long *out)
 {
     if (!c || !out) return WDM_EINVAL;
     *out = c->launches;
+    return WDM_OK;
+}
+
+extern "C" int wdm_get_diagnostics(wdm_ctx *c, double *out_host)
+{
+    if (!c) return WDM_EINVAL;
+    if (!out_host) return fail(c, WDM_EINVAL, "null output");
+    int rc = do_refresh(c);
+    if (rc) return rc;
+    // scratch: the 64-byte block of the <rho> accumulators is free between refreshes except for the mean at byte 16;
+    // use the first 48 bytes of the head of H instead (H is dead outside a Poisson solve)
+    double *acc = (double *)c->H;
+    unsigned long long *mx = (unsigned long long *)(acc + 4);
+    {
+        Timed t(c, S_MISC);
+        CU(c, cudaMemsetAsync(acc, 0, 6 * sizeof(double), c->stream));
+        const double inv2dx = 0.5 * c->N / c->L;
+        if (c->dtype == WDM_C64) k_diag<float><<<148 * 8, 256, 0, c->stream>>>((const cx<float> *)c->psi, (const float *)c->phi, c->N, c->mu, inv2dx, acc, mx);
+        else k_diag<double><<<148 * 8, 256, 0, c->stream>>>((const cx<double> *)c->psi, (const double *)c->phi, c->N, c->mu, inv2dx, acc, mx);
+        CU(c, cudaGetLastError());
+    }
+    double h[6];
+    CU(c, cudaMemcpyAsync(h, acc, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    const double dx = c->L / c->N, dV = dx * dx * dx;
+    double maxrho, maxphi;
+    memcpy(&maxrho, &h[4], 8);
+    memcpy(&maxphi, &h[5], 8);
+    out_host[0] = h[0] * dV; out_host[1] = maxrho; out_host[2] = maxphi;
+    out_host[3] = h[1] * dV; out_host[4] = h[2] * dV; out_host[5] = h[3] * dV;
+    double dtm = 4.0 / (3.0 * M_PI) * dx * dx / c->mu;                                       // Eq. 26
+    if (maxphi > 0 && 2.0 * M_PI * c->mu / maxphi < dtm) dtm = 2.0 * M_PI * c->mu / maxphi;
+    if (c->kappa != 0 && maxrho > 0 && 2.0 * M_PI * c->mu / (fabs(c->kappa) * maxrho) < dtm) dtm = 2.0 * M_PI * c->mu / (fabs(c->kappa) * maxrho);
+    out_host[6] = 0.5 * dtm;
+    out_host[7] = 0;
     return WDM_OK;
 }
 

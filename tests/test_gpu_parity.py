@@ -403,3 +403,27 @@ def test_kick_terms_with_particles(wdm):
     assert rel(v.cpu().numpy(), vo) <= 1e-4
     assert rel(sim.psi().cpu().numpy(), o.psi()) <= tol("c64", 5)
     sim.close()
+
+
+# ---------------------------------------------------------------- diagnostics
+
+@pytest.mark.parametrize("dtype,N,rtol", [("c128", 32, 1e-11), ("c64", 64, 2e-5), ("c64", 256, 2e-5)])
+def test_diagnostics_match_oracle(wdm, dtype, N, rtol):
+    """wdm_get_diagnostics (one device reduction pass) against the oracle's plain loops: mass, maxima of Eq. 26,
+    V, K, Q (central differences of Eq. 21) and dt_max, on the initial state and after two steps."""
+    psi0 = (0.3 * wl.random_field(N, dtype, 77) + 1.0).astype(np.complex64 if dtype == "c64" else np.complex128)
+    w = wl.Workload(f"diag{N}", N, dtype, 2, L=1.3, hbar_over_m=0.8, G=30.0, psi=psi0)
+    dt = 0.2 * (w.L / N) ** 2
+    sim, o = pair(wdm, w)
+    for kappa in (0.0, -5e3):
+        sim.set_kick_terms(kappa=kappa)
+        o.set_kick_terms(kappa=kappa)
+        a, b = sim.diagnostics(), o.diagnostics()
+        for key in ("M", "max_rho", "max_phi", "V", "K", "Q", "dt_max"):
+            assert abs(a[key] - b[key]) <= rtol * max(abs(b[key]), 1e-300) * (50 if key in ("max_phi", "V") and dtype == "c64" else 1), (key, a[key], b[key])
+    sim.set_kick_terms(); o.set_kick_terms()
+    sim.step(2, dt); o.step(2, dt)
+    a, b = sim.diagnostics(), o.diagnostics()
+    for key in ("M", "max_rho", "max_phi", "V", "K", "Q", "dt_max"):
+        assert abs(a[key] - b[key]) <= 100 * rtol * abs(b[key]), (key, a[key], b[key])
+    sim.close()
