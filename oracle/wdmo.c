@@ -58,6 +58,9 @@ typedef struct wdmo_ctx {
     double *phi_ext;     /* static external potential added to the Poisson potential, or NULL  */
     double alpha;        /* absorbing-layer coefficient (0 = no layer)                          */
     int nb;              /* absorbing-layer transition width L / nb                             */
+    /* particle variants (reading G29) */
+    int nsub;            /* leapfrog sub-steps per SPE step (>= 1)                              */
+    int pstatic;         /* :particles_static -- particles never move, they only source Phi    */
 } wdmo_ctx;
 
 static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
@@ -317,6 +320,7 @@ int wdmo_create(wdmo_ctx **out, int N, double L, double hbar_over_m, double G)
     wdmo_ctx *c = (wdmo_ctx *)calloc(1, sizeof(*c));
     if (!c) return WDMO_ENOMEM;
     c->N = N; c->L = L; c->mu = hbar_over_m; c->G = G; c->dx = L / N;
+    c->nsub = 1;
     c->n = (size_t)N * N * N;
     c->psi = (cplx *)malloc(sizeof(cplx) * c->n);
     c->work = (cplx *)malloc(sizeof(cplx) * c->n);
@@ -415,7 +419,9 @@ static void half_kick(wdmo_ctx *c, double h)
         double th = -V * h / c->mu;
         c->psi[i] *= cos(th) + I * sin(th);
     }
-    for (long long i = 0; i < 3 * c->np; ++i) c->vel[i] += c->acc[i] * h;
+    /* particle half kick of the FIRST / LAST sub-step (sub-step size dt/nsub, so h/nsub here) */
+    if (!c->pstatic)
+        for (long long i = 0; i < 3 * c->np; ++i) c->vel[i] += c->acc[i] * (h / c->nsub);
 }
 
 /* psi = F^-1{ exp(-i mu k^2 dt/2) F{psi} }  (Eq. 18b) ;  x += v dt, wrapped */
@@ -438,7 +444,19 @@ static int drift(wdmo_ctx *c, double dt)
     }
     rc = fft3_inplace(c->psi, N, +1);
     if (rc) return rc;
-    for (long long i = 0; i < 3 * c->np; ++i) c->pos[i] = wrap_pos(c->pos[i] + c->vel[i] * dt, c->L);
+    /* particles: nsub drifts of dt/nsub in the potential Phi^n of the start of the step (still in c->phi);
+     * between two drifts a full kick (closing + opening half kicks of neighbouring sub-steps) with the
+     * acceleration gathered at the new position ("multiple sub-steps within each SPE step") */
+    if (!c->pstatic && c->np > 0) {
+        double h = dt / c->nsub;
+        for (int j = 1; j <= c->nsub; ++j) {
+            for (long long i = 0; i < 3 * c->np; ++i) c->pos[i] = wrap_pos(c->pos[i] + c->vel[i] * h, c->L);
+            if (j < c->nsub) {
+                cic_gather(c->phi, c->N, c->L, c->np, c->pos, c->acc);
+                for (long long i = 0; i < 3 * c->np; ++i) c->vel[i] += c->acc[i] * h;
+            }
+        }
+    }
     return WDMO_OK;
 }
 
@@ -460,6 +478,15 @@ static void absorb(wdmo_ctx *c, double dt)
                 double b = absorb_profile(x, c->L, c->nb) + absorb_profile(y, c->L, c->nb) + absorb_profile(z, c->L, c->nb);
                 c->psi[((size_t)ix * N + iy) * N + iz] *= exp(-c->alpha * b * dt);
             }
+}
+
+/* nsub >= 1 leapfrog sub-steps per SPE step; pstatic != 0: particles are a fixed mass distribution */
+int wdmo_set_particle_mode(wdmo_ctx *c, int nsub, int pstatic)
+{
+    if (!c || nsub < 1) return WDMO_EINVAL;
+    c->nsub = nsub;
+    c->pstatic = pstatic != 0;
+    return WDMO_OK;
 }
 
 /* kappa: self-interaction strength; phi_ext: N^3 values or NULL; alpha = 0 switches the absorbing layer off */

@@ -464,3 +464,63 @@ def test_p14_diagnostics_real_gaussian_and_cosine_density():
     o.set_kick_terms(kappa=-1e4)
     d = o.diagnostics()
     assert abs(d["dt_max"] - 0.5 * 2 * np.pi * mu / (1e4 * (r0 + r1))) < 1e-15     # third term of Eq. 26 is the smallest
+
+
+# ---------------------------------------------------------------- P15: particle variants
+
+def test_p15_substeps_harmonic_leapfrog_closed_form():
+    """G = 0, Phi_ext = omega^2 x^2/2: the central difference of x^2 and the CIC interpolation of a linear
+    function are exact, so the particle feels a = -omega^2 x exactly and the KDK leapfrog of sub-step h = dt/nsub
+    has the closed form x_n = x0 cos(n theta), cos(theta) = 1 - (omega h)^2/2 (v0 = 0).  nsub = 1 is the default
+    scheme; more sub-steps follow the same closed form with the smaller h."""
+    N, L, omega = 32, 1.0, 3.0
+    X, Y, Z = grid(N, L)
+    x0 = 0.2137
+    for nsub in (1, 4):
+        dt, nsteps = 0.05, 6
+        o = oracle.Oracle(N, L, 1.0, 0.0)
+        o.set_kick_terms(phi_ext=0.5 * omega ** 2 * X ** 2)
+        o.set_psi(np.ones((N, N, N), complex))
+        o.set_particles(np.array([[x0, 0.01, -0.02]]), np.zeros((1, 3)), 0.0)
+        o.set_particle_mode(substeps=nsub)
+        o.step(nsteps, dt)
+        h = dt / nsub
+        theta = math.acos(1 - 0.5 * (omega * h) ** 2)
+        p, v = o.particles()
+        assert abs(p[0, 0] - x0 * math.cos(nsteps * nsub * theta)) < 1e-12
+        assert abs(p[0, 1] - 0.01) < 1e-15 and abs(p[0, 2] + 0.02) < 1e-15
+    # default mode == one sub-step, bit for bit
+    res = []
+    for mode in (None, 1):
+        o = oracle.Oracle(16, 1.0, 1.0, 1.0 / FOUR_PI)
+        w = wl.small_coupled(16, dtype="c128")
+        o.set_psi(w.psi); o.set_particles(w.pos, w.vel, w.mass)
+        if mode:
+            o.set_particle_mode(substeps=mode)
+        o.step(3, w.dt)
+        res.append(o.particles())
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
+
+
+def test_p15_static_particles_only_source_the_potential():
+    """:particles_static: positions and velocities never change, but the particles' mass is in the
+    Poisson source: the potential at step 0 equals the dynamic mode's, and psi evolves differently from a run
+    without particles."""
+    w = wl.small_coupled(16, dtype="c128")
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    o.set_psi(w.psi); o.set_particles(w.pos, w.vel, w.mass); o.set_particle_mode(static=True)
+    o.step(0, 0.0)
+    phi_static = o.potential()
+    od = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    od.set_psi(w.psi); od.set_particles(w.pos, w.vel, w.mass); od.step(0, 0.0)
+    assert np.array_equal(phi_static, od.potential())
+    o.step(4, w.dt)
+    p, v = o.particles()
+    pw = w.pos - w.L * np.floor((w.pos + w.L / 2) / w.L)
+    assert np.array_equal(p, pw) and np.array_equal(v, w.vel)
+    o0 = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    o0.set_psi(w.psi); o0.step(4, w.dt)
+    assert relerr(o.psi(), o0.psi()) > 1e-6
+    # total mass in the source: sum rho dx^3 = M_psi + sum m_p
+    dx3 = (w.L / w.N) ** 3
+    assert abs(o.density().sum() * dx3 - (np.sum(np.abs(o.psi()) ** 2) * dx3 + np.sum(np.broadcast_to(w.mass, (len(w.pos),))))) < 1e-10
