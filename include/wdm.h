@@ -103,6 +103,12 @@ int wdm_get_particles_host(wdm_ctx *ctx, void *pos_out_host, void *vel_out_host)
  * Defaults: 0, NULL, 0.  Marks the potential stale (recomputed by the next step / get). */
 int wdm_set_kick_terms(wdm_ctx *ctx, double kappa, const void *phi_ext_dev, double absorb_alpha, int absorb_nb);
 
+/* Particle variants.  substeps >= 1: leapfrog sub-steps of dt/substeps per wave step, all in the
+ * potential of the start of the step, the acceleration re-gathered at every new position; the half kicks that open
+ * and close a wave step use the potentials of its two ends (substeps = 1 is the default scheme).  is_static != 0
+ * (":particles_static"): the particles never move; their mass stays in the Poisson source.  Default: 1, 0. */
+int wdm_set_particle_mode(wdm_ctx *ctx, int substeps, int is_static);
+
 /* Diagnostics of the current state (Sect. 3.5-3.6) by one reduction pass on the device; the
  * gradients are the second-order central differences of Eq. 21.  Synchronises the stream.
  * out_host[0] M = sum |psi|^2 dx^3       [1] max |psi|^2       [2] max |Phi_total|

@@ -178,6 +178,9 @@ struct wdm_ctx {
     double phase_dt = 0;
     bool phase_valid = false, have_psi = false, stale = true;
     // L2-chained sweeps (wdm_chain.cuh): completion counters, launch epochs, lag per chain (0: separate sweeps)
+    // particle variants (wdm_set_particle_mode; reading G29)
+    int nsub = 1;
+    bool pstatic = false;
     // extra kick terms (wdm_set_kick_terms; readings G26-G28)
     double kappa = 0, alpha = 0;
     int absorb_nb = 50;
@@ -503,9 +506,9 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
     for (int s = 0; s < nsteps; ++s) {
         // merged closing (h_d, of the previous step) + opening (h_a) half kicks (G21); the layer sits between them
         const double hd = s == 0 ? 0.0 : 0.5 * dt, ha = 0.5 * dt, kdt = hd + ha;
-        if (c->part.n > 0) {
-            // v += a(Phi^n, x^n) kdt ; x += v dt ; wrap ; then deposit x^{n+1}  (readings G14-G16)
-            { Timed t(c, S_PART_PUSH); CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, have_phi ? kdt : 0.0, dt, c->stream)); }
+        if (c->part.n > 0 && !c->pstatic) {
+            // v += a(Phi^n, x^n) kdt/nsub ; nsub x { x += v dt/nsub ; wrap ; [kick] } ; then deposit x^{n+1}  (G14-G16, G29)
+            { Timed t(c, S_PART_PUSH); CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, have_phi ? kdt / c->nsub : 0.0, dt, c->nsub, c->stream)); }
             if (grav) { rc = particles_deposit<T>(c); if (rc) return rc; }
         }
         {
@@ -550,9 +553,9 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             k_kick<T><<<148 * 8, 256, 0, c->stream>>>((cx<T> *)c->psi, (const T *)c->phi, (T)(0.5 * dt / c->mu), c->n);
         CU(c, cudaGetLastError());
     }
-    if (have_phi && c->part.n > 0) {
+    if (have_phi && c->part.n > 0 && !c->pstatic) {
         Timed t(c, S_PART_PUSH);
-        CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, 0.5 * dt, 0.0, c->stream));
+        CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, 0.5 * dt / c->nsub, 0.0, 1, c->stream));
     }
     return WDM_OK;
 }
@@ -784,6 +787,15 @@ extern "C" int wdm_launch_count(wdm_ctx *c, long long *out)
 {
     if (!c || !out) return WDM_EINVAL;
     *out = c->launches;
+    return WDM_OK;
+}
+
+extern "C" int wdm_set_particle_mode(wdm_ctx *c, int substeps, int is_static)
+{
+    if (!c) return WDM_EINVAL;
+    if (substeps < 1) return fail(c, WDM_EINVAL, "substeps must be >= 1");
+    c->nsub = substeps;
+    c->pstatic = is_static != 0;
     return WDM_OK;
 }
 

@@ -131,49 +131,75 @@ __global__ void k_scatter(const T *pos, const T *vel, const T *mass, const int *
     orig2[d] = orig[i];
 }
 
-// gather a = sum_corners w * (-(phi[node+e] - phi[node-e]) / (2 dx)), kick, drift, wrap
+// a = sum_corners w * (phi[node+e] - phi[node-e]) per axis (the caller scales by -1/(2 dx)): CIC gather of the
+// central-difference gradient (Eq. 21) with the deposit's weights (G13)
 template <typename T>
-__global__ void k_push(T *pos, T *vel, const T *__restrict__ phi, long long n, int N, T L, T kick_dt, T drift_dt)
+__device__ __forceinline__ void gather_grad(const T *__restrict__ phi, const T (&x)[3], int N, T L, T (&a)[3])
+{
+    const T inv_dx = (T)N / L;
+    Cic<T> c = cic_of<T>(x, (T)0.5 * L, inv_dx, N);
+    const int M = N - 1;
+    // indices i0-1 .. i0+2 along each axis
+    int ix[4], iy[4], iz[4];
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+        ix[d] = (c.i0[0] + d - 1) & M;
+        iy[d] = (c.i0[1] + d - 1) & M;
+        iz[d] = (c.i0[2] + d - 1) & M;
+    }
+    a[0] = a[1] = a[2] = (T)0;
+#pragma unroll
+    for (int bx = 0; bx < 2; ++bx)
+#pragma unroll
+        for (int by = 0; by < 2; ++by)
+#pragma unroll
+            for (int bz = 0; bz < 2; ++bz) {
+                T w = (bx ? c.f[0] : (T)1 - c.f[0]) * (by ? c.f[1] : (T)1 - c.f[1]) * (bz ? c.f[2] : (T)1 - c.f[2]);
+                size_t X = ix[bx + 1], Y = iy[by + 1], Z = iz[bz + 1];
+                T gx = __ldg(phi + ((size_t)ix[bx + 2] * N + Y) * N + Z) - __ldg(phi + ((size_t)ix[bx] * N + Y) * N + Z);
+                T gy = __ldg(phi + (X * N + iy[by + 2]) * N + Z) - __ldg(phi + (X * N + iy[by]) * N + Z);
+                T gz = __ldg(phi + (X * N + Y) * N + iz[bz + 2]) - __ldg(phi + (X * N + Y) * N + iz[bz]);
+                a[0] += w * gx; a[1] += w * gy; a[2] += w * gz;
+            }
+}
+
+// v += a(x) kick_dt ; then nsub drifts of drift_dt / nsub, wrapped, with a full kick of that size (gathered at the
+// new position, in the same potential) between two drifts (several N-body sub-steps per SPE step)
+template <typename T>
+__global__ void k_push(T *pos, T *vel, const T *__restrict__ phi, long long n, int N, T L, T kick_dt, T drift_dt, int nsub)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= n) return;
     T x[3] = {pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
     T v[3] = {vel[3 * i], vel[3 * i + 1], vel[3 * i + 2]};
+    const T g = -(T)0.5 * (T)N / L;
+    bool kicked = false;
     if (kick_dt != (T)0) {
-        const T inv_dx = (T)N / L;
-        Cic<T> c = cic_of<T>(x, (T)0.5 * L, inv_dx, N);
-        const int M = N - 1;
-        // indices i0-1 .. i0+2 along each axis
-        int ix[4], iy[4], iz[4];
+        T a[3];
+        gather_grad<T>(phi, x, N, L, a);
 #pragma unroll
-        for (int d = 0; d < 4; ++d) {
-            ix[d] = (c.i0[0] + d - 1) & M;
-            iy[d] = (c.i0[1] + d - 1) & M;
-            iz[d] = (c.i0[2] + d - 1) & M;
-        }
-        T a[3] = {0, 0, 0};
-#pragma unroll
-        for (int bx = 0; bx < 2; ++bx)
-#pragma unroll
-            for (int by = 0; by < 2; ++by)
-#pragma unroll
-                for (int bz = 0; bz < 2; ++bz) {
-                    T w = (bx ? c.f[0] : (T)1 - c.f[0]) * (by ? c.f[1] : (T)1 - c.f[1]) * (bz ? c.f[2] : (T)1 - c.f[2]);
-                    size_t X = ix[bx + 1], Y = iy[by + 1], Z = iz[bz + 1];
-                    T gx = __ldg(phi + ((size_t)ix[bx + 2] * N + Y) * N + Z) - __ldg(phi + ((size_t)ix[bx] * N + Y) * N + Z);
-                    T gy = __ldg(phi + (X * N + iy[by + 2]) * N + Z) - __ldg(phi + (X * N + iy[by]) * N + Z);
-                    T gz = __ldg(phi + (X * N + Y) * N + iz[bz + 2]) - __ldg(phi + (X * N + Y) * N + iz[bz]);
-                    a[0] += w * gx; a[1] += w * gy; a[2] += w * gz;
-                }
-        const T s = -(T)0.5 * inv_dx * kick_dt;
-#pragma unroll
-        for (int d = 0; d < 3; ++d) v[d] += a[d] * s;
-#pragma unroll
-        for (int d = 0; d < 3; ++d) vel[3 * i + d] = v[d];
+        for (int d = 0; d < 3; ++d) v[d] += a[d] * (g * kick_dt);
+        kicked = true;
     }
     if (drift_dt != (T)0) {
+        const T h = drift_dt / (T)nsub;
+        for (int j = 1; j <= nsub; ++j) {
 #pragma unroll
-        for (int d = 0; d < 3; ++d) pos[3 * i + d] = wrap_pos(x[d] + v[d] * drift_dt, L);
+            for (int d = 0; d < 3; ++d) x[d] = wrap_pos(x[d] + v[d] * h, L);
+            if (j < nsub) {
+                T a[3];
+                gather_grad<T>(phi, x, N, L, a);
+#pragma unroll
+                for (int d = 0; d < 3; ++d) v[d] += a[d] * (g * h);
+                kicked = true;
+            }
+        }
+#pragma unroll
+        for (int d = 0; d < 3; ++d) pos[3 * i + d] = x[d];
+    }
+    if (kicked) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) vel[3 * i + d] = v[d];
     }
 }
 
@@ -341,11 +367,12 @@ cudaError_t particle_set(ParticleState &ps, int N, double L, int dtype, long lon
 }
 
 cudaError_t particle_push(ParticleState &ps, int N, double L, int dtype, const void *phi, double kick_dt, double drift_dt,
-                          cudaStream_t s)
+                          int nsub, cudaStream_t s)
 {
     if (ps.n == 0) return cudaSuccess;
-    if (dtype == 0) k_push<float><<<blocks(ps.n, 128), 128, 0, s>>>((float *)ps.pos, (float *)ps.vel, (const float *)phi, ps.n, N, (float)L, (float)kick_dt, (float)drift_dt);
-    else k_push<double><<<blocks(ps.n, 128), 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt);
+    if (nsub < 1) nsub = 1;
+    if (dtype == 0) k_push<float><<<blocks(ps.n, 128), 128, 0, s>>>((float *)ps.pos, (float *)ps.vel, (const float *)phi, ps.n, N, (float)L, (float)kick_dt, (float)drift_dt, nsub);
+    else k_push<double><<<blocks(ps.n, 128), 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt, nsub);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (drift_dt != 0.0 && ++ps.steps_since_sort >= kResortInterval)

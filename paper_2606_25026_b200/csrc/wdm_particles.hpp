@@ -25,9 +25,10 @@ size_t particle_bytes(int N, int dtype, long long capacity);
 void particle_bind(ParticleState &ps, int N, int dtype, long long capacity, void *rho_p, void *pool);
 cudaError_t particle_set(ParticleState &ps, int N, double L, int dtype, long long n, const void *pos, const void *vel,
                          const void *mass, double mass_scalar, bool from_host, cudaStream_t s);
-// v += a(phi, x) * kick_dt ; x += v * drift_dt ; wrap into [-L/2, L/2)
+// v += a(phi, x) * kick_dt ; then nsub drifts of drift_dt / nsub (wrapped into [-L/2, L/2)) with a kick of that
+// size, gathered at the new position, between two drifts
 cudaError_t particle_push(ParticleState &ps, int N, double L, int dtype, const void *phi, double kick_dt,
-                          double drift_dt, cudaStream_t s);
+                          double drift_dt, int nsub, cudaStream_t s);
 // rho_p += CIC(x) (the caller zeroes rho_p)
 cudaError_t particle_deposit(ParticleState &ps, int N, double L, int dtype, cudaStream_t s);
 cudaError_t particle_get(ParticleState &ps, int dtype, void *pos_out, void *vel_out, bool to_host, cudaStream_t s);

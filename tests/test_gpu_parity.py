@@ -427,3 +427,24 @@ def test_diagnostics_match_oracle(wdm, dtype, N, rtol):
     for key in ("M", "max_rho", "max_phi", "V", "K", "Q", "dt_max"):
         assert abs(a[key] - b[key]) <= 100 * rtol * abs(b[key]), (key, a[key], b[key])
     sim.close()
+
+
+# ---------------------------------------------------------------- particle variants
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("mode", [dict(substeps=4), dict(static=True), dict(substeps=3, static=False)])
+def test_particle_modes_match_oracle(wdm, dtype, mode):
+    w = wl.small_coupled(32, dtype=dtype)
+    sim, o = pair(wdm, w, max_particles=len(w.pos))
+    sim.set_particle_mode(**mode)
+    o.set_particle_mode(**mode)
+    sim.step(3, w.dt); o.step(3, w.dt)
+    sim.step(1, w.dt); o.step(1, w.dt)          # a second call: closing / opening half kicks across calls
+    p, v = sim.particles()
+    po, vo = o.particles()
+    d = p.cpu().numpy() - po
+    d -= w.L * np.round(d / w.L)
+    assert np.abs(d).max() <= (POS_TOL if dtype == "c64" else 1e-12) * w.L
+    assert rel(v.cpu().numpy(), vo) <= (1e-4 if dtype == "c64" else 1e-11)
+    check_fields(sim, o, dtype, 4, str(mode))
+    sim.close()
