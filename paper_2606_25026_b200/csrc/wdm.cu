@@ -521,13 +521,13 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             pz.kick_extra = (c->kappa != 0.0 || pz.mask != nullptr) ? 1 : 0;
             py.data = (cx<T> *)c->psi;
             py.tmap = c->tm_psi_y;
-            if (c->lag_psi > 0) {
+            if (c->lag_psi > 0 && !pz.kick_extra) {
                 ChainCtl ctl{c->chain_done, ++c->epoch_psi * (unsigned int)(N / c->tab->fact.W), c->lag_psi};
                 pz.tag = S_PSI_ZY;
                 Timed t(c, S_PSI_ZY);
                 CU(c, c->tab->psi_zy(&pz, &py, kicks ? 1 : 0, &ctl, c->stream));
             } else {
-                { pz.tag = S_PSI_Z; Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? 1 : 0, c->stream)); }
+                { pz.tag = S_PSI_Z; Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? (pz.kick_extra ? 2 : 1) : 0, c->stream)); }
                 { py.tag = S_PSI_Y; Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
             }
         }

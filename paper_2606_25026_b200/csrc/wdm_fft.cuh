@@ -175,16 +175,15 @@ template <int R, typename T, class ST>
 WDM_HD void fwd_level_regs(cx<T> (&v)[R], int rowbase, int m, const cx<T> *tw, ST &&st)
 {
     constexpr bool PRE = R * sizeof(T) <= 64;
-    cx<T> w[PRE ? R : 1];
-    if constexpr (PRE) static_for<1, R>([&](auto s_) { constexpr int s = decltype(s_)::value; w[s] = tw[s * m]; });
+    constexpr int LOOK = PRE ? R : 4;          // too many to hold: a rolling window, each fetched LOOK outputs ahead of its use
+    cx<T> w[R];
+    static_for<1, (LOOK < R ? LOOK + 1 : R)>([&](auto s_) { constexpr int s = decltype(s_)::value; w[s] = tw[s * m]; });
     dif_fwd<R>(v);
     static_for<0, R>([&](auto s_) {
         constexpr int s = decltype(s_)::value;
+        if constexpr (s > 0 && s + LOOK < R) w[s + LOOK] = tw[(s + LOOK) * m];
         cx<T> y = v[brev(s, R)];
-        if constexpr (s > 0) {
-            if constexpr (PRE) y = cmul(y, w[s]);
-            else y = cmul(y, tw[s * m]);
-        }
+        if constexpr (s > 0) y = cmul(y, w[s]);
         st(rowbase + m * s, y);
     });
 }

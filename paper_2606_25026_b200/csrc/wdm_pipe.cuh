@@ -338,6 +338,25 @@ struct HalfSpec {
     }
 };
 
+// Packed tile of the real-data transforms: N rows x W/2 complex (two real lines per complex line).  With 64-byte
+// rows two rows share a 128-byte bank line; the middle level reads rows a multiple of RM apart from neighbouring
+// lanes, which would land in the same half.  Rows whose bit log2(RM) is set therefore swap places with their
+// neighbour (row ^ 1): every access pattern of the sweeps (level A: rows q, q + 1; middle: g RM + s, (g+1) RM + s;
+// the Hermitian split: consecutive rows) then touches both halves.
+// (Measured at 512^3: -2 % on the density sweep; the complex-to-real sweep is latency bound and loses more to the
+// extra index arithmetic than it gains, so it keeps the plain layout: ON = false.)
+template <class C, bool ON = true>
+struct Packed {
+    using T = typename C::T;
+    static constexpr int RSP = C::W / 2;
+    static constexpr bool SWZ = ON && RSP * sizeof(cx<T>) == 64 && C::RB == 1;
+    static __device__ __forceinline__ int idx(int row, int l)
+    {
+        if constexpr (SWZ) row ^= (row / C::RM) & 1;
+        return row * RSP + l;
+    }
+};
+
 struct NoPre {};
 
 constexpr size_t align128(size_t x) { return (x + 127) & ~(size_t)127; }
@@ -347,7 +366,9 @@ constexpr size_t align128(size_t x) { return (x + 127) & ~(size_t)127; }
 // leaves shared memory for the first butterfly (Eq. 18(a),(d)); the Phi values of the NEXT tile are fetched
 // into registers before the current tile's last stage.  RHO (x axis): rho - <rho> = |psi2|^2 (+ rho_p) - <rho>
 // formed from the outgoing registers, packed real-to-complex FFT along x in the same buffer -> H.
-template <class C_, int AX, bool KICK, bool RHO, bool DRIFT>
+// KICK: 0 none, 1 plain potential kick, 2 with the extra terms of SweepParams::kick_extra (a separate
+// instantiation, so the plain kernel carries none of their code or registers).
+template <class C_, int AX, int KICK, bool RHO, bool DRIFT>
 struct PsiK {
     using C = C_;
     using T = typename C::T;
@@ -420,8 +441,8 @@ struct PsiK {
                     split<AX, mA, W>(gt + it * NTG, q, l);
                     cx<T> v[RA];
                     static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = S[L::idx(q + mA * r, l)]; });
-                    if constexpr (KICK) {
-                        if (p.kick_extra) {
+                    if constexpr (KICK != 0) {
+                        if constexpr (KICK == 2) {
                             // self-interaction and / or absorbing layer: the pencil of line l is (x, y) = divmod(t W + l, N)
                             T mxy = (T)1;
                             if (p.mask) {
@@ -516,7 +537,7 @@ struct PsiK {
         }
         if constexpr (RHO) {
             // rho tile as N rows x W reals == N rows x W/2 packed complex lines (lines 2l', 2l'+1)
-            constexpr int WP = W / 2, RSP = W / 2;
+            constexpr int WP = W / 2;
             T *F = reinterpret_cast<T *>(buf);
             group_sync(grp, NTG);                       // every thread has finished reading the psi tile
             // rho - <rho> (Eq. 23).  <rho> is conserved, so it is measured once per refresh; k = 0 is
@@ -541,7 +562,7 @@ struct PsiK {
                 });
                 cx<T> w[RA];
                 twiddles(w);
-                fwd_level_regs_w<RA, T>(v, pq, mA, w, [&](int row, cx<T> y) { Sp[row * RSP + pl / 2] = y; });
+                fwd_level_regs_w<RA, T>(v, pq, mA, w, [&](int row, cx<T> y) { Sp[Packed<C>::idx(row, pl / 2)] = y; });
             } else {
                 static_for<0, ITER>([&](auto it_) {
                     constexpr int it = decltype(it_)::value;
@@ -553,28 +574,28 @@ struct PsiK {
                         int row = q + mA * r;
                         T v = rho[it][r];
                         if (gp) v += ldg(gp + (long long)(mA * r) * TL::RSTRIDE);
-                        F[row * W + l] = v - mean;
+                        F[2 * Packed<C>::idx(row, l / 2) + (l & 1)] = v - mean;
                     });
                 });
                 group_sync(grp, NTG);
                 for (int b = gt; b < mA * WP; b += NTG) {
                     int l = b % WP, q = b / WP;
-                    fwd_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; },
-                                     [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
+                    fwd_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[Packed<C>::idx(row, l)]; },
+                                     [&](int row, cx<T> v) { Sp[Packed<C>::idx(row, l)] = v; });
                 }
             }
             group_sync(grp, NTG);
-            g_fwd_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return row * RSP + l; });
+            g_fwd_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return Packed<C>::idx(row, l); });
             for (int b = gt; b < (N / RM) * WP; b += NTG) {
                 int l = b % WP, g = b / WP;
-                mid_fwd<RM, T>(g * RM, [&](int row) { return Sp[row * RSP + l]; },
-                               [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
+                mid_fwd<RM, T>(g * RM, [&](int row) { return Sp[Packed<C>::idx(row, l)]; },
+                               [&](int row, cx<T> v) { Sp[Packed<C>::idx(row, l)] = v; });
             }
             group_sync(grp, NTG);
             // Hermitian split of Z = FFT(a + i b):  A_k = (Z_k + conj Z_{N-k})/2,  B_k = (Z_k - conj Z_{N-k})/(2i)
             auto emit = [&](int k, int pk, int l) {
                 int pn = HalfSpec<C>::row_of((N - k) & (N - 1));
-                cx<T> zk = Sp[pk * RSP + l], zn = Sp[pn * RSP + l];
+                cx<T> zk = Sp[Packed<C>::idx(pk, l)], zn = Sp[Packed<C>::idx(pn, l)];
                 const T h = (T)0.5;
                 cx<T> A = mk<T>((zk.x + zn.x) * h, (zk.y - zn.y) * h);
                 cx<T> B = mk<T>((zk.y + zn.y) * h, (zn.x - zk.x) * h);
@@ -693,7 +714,8 @@ struct HK {
 
 // complex-to-real inverse along x: H[kx <= N/2][y][z] -> Phi[x][y][z]; lines (2l', 2l'+1) share one FFT.
 // Buffer = [packed tile: N rows x W/2 complex][raw tile: N/2+1 rows x W complex, filled by the async copies].
-template <class C_>
+// EXT: add the static external potential on the way out (SweepParams::phi_ext != nullptr), a separate instantiation
+template <class C_, bool EXT = false>
 struct C2RK {
     using C = C_;
     using T = typename C::T;
@@ -722,8 +744,8 @@ struct C2RK {
         auto place = [&](int k, int pk, int l) {
             cx<T> A, B;
             ld2(R + k * W + 2 * l, A, B);
-            Sp[pk * RSP + l] = mk<T>(A.x - B.y, A.y + B.x);
-            if (k > 0 && k < N / 2) Sp[HalfSpec<C>::row_of(N - k) * RSP + l] = mk<T>(A.x + B.y, B.x - A.y);
+            Sp[Packed<C, false>::idx(pk, l)] = mk<T>(A.x - B.y, A.y + B.x);
+            if (k > 0 && k < N / 2) Sp[Packed<C, false>::idx(HalfSpec<C>::row_of(N - k), l)] = mk<T>(A.x + B.y, B.x - A.y);
         };
         for (int b = gt; b < (N / 2) * WP; b += NTG) {
             int l = b % WP, k, pk;
@@ -734,26 +756,26 @@ struct C2RK {
         group_sync(grp, NTG);
         for (int b = gt; b < (N / RM) * WP; b += NTG) {
             int l = b % WP, g = b / WP;
-            mid_inv<RM, T>(g * RM, [&](int row) { return Sp[row * RSP + l]; },
-                           [&](int row, cx<T> v) { Sp[row * RSP + l] = v; });
+            mid_inv<RM, T>(g * RM, [&](int row) { return Sp[Packed<C, false>::idx(row, l)]; },
+                           [&](int row, cx<T> v) { Sp[Packed<C, false>::idx(row, l)] = v; });
         }
         group_sync(grp, NTG);
-        g_inv_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return row * RSP + l; });
+        g_inv_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return Packed<C, false>::idx(row, l); });
         for (int b = gt; b < mA * WP; b += NTG) {
             int l = b % WP, q = b / WP;
             T *gp = p.phi_out + tile.at(q, 2 * l);
-            const T *ge = p.phi_ext ? p.phi_ext + tile.at(q, 2 * l) : nullptr;     // Phi_total = Phi_DM + Phi_ext (Alg. 1 l.15)
+            const T *ge = EXT ? p.phi_ext + tile.at(q, 2 * l) : nullptr;           // Phi_total = Phi_DM + Phi_ext (Alg. 1 l.15)
             auto out = [&](int row, cx<T> v) {
                 // Re -> line 2l', Im -> line 2l'+1: one (re, im) pair is two adjacent reals of Phi
-                if (ge) {
+                if constexpr (EXT) {
                     cx<T> e = ldg(reinterpret_cast<const cx<T> *>(ge + (long long)(row - q) * TL::RSTRIDE));
                     v.x += e.x;
                     v.y += e.y;
                 }
                 stv(reinterpret_cast<cx<T> *>(gp + (long long)(row - q) * TL::RSTRIDE), v);
             };
-            if constexpr (PAIR) inv_level_w<RA, T>(q, mA, pers.w, [&](int row) { return Sp[row * RSP + l]; }, out);
-            else inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[row * RSP + l]; }, out);
+            if constexpr (PAIR) inv_level_w<RA, T>(q, mA, pers.w, [&](int row) { return Sp[Packed<C, false>::idx(row, l)]; }, out);
+            else inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[Packed<C, false>::idx(row, l)]; }, out);
         }
     }
 };

@@ -93,16 +93,18 @@ cudaError_t chain_launch(ChainParams<Real, (int)sizeof...(KS)> &cp, int planes, 
     return cudaLaunchCooperativeKernel((void *)k_chain<KS...>, dim3(grid), dim3(kThreads), args, ChainSmem<KS...>::TOTAL, s);
 }
 
-using PsiZKick = PsiK<C, AX_CONTIG, true, false, true>;
-using PsiZ = PsiK<C, AX_CONTIG, false, false, true>;
-using PsiS = PsiK<C, AX_Y, false, false, true>;
-using PsiX = PsiK<C, AX_X, false, false, true>;
-using PsiXRho = PsiK<C, AX_X, false, true, true>;
-using RhoOnly = PsiK<C, AX_X, false, true, false>;
+using PsiZKick = PsiK<C, AX_CONTIG, 1, false, true>;
+using PsiZKickX = PsiK<C, AX_CONTIG, 2, false, true>;
+using PsiZ = PsiK<C, AX_CONTIG, 0, false, true>;
+using PsiS = PsiK<C, AX_Y, 0, false, true>;
+using PsiX = PsiK<C, AX_X, 0, false, true>;
+using PsiXRho = PsiK<C, AX_X, 0, true, true>;
+using RhoOnly = PsiK<C, AX_X, 0, true, false>;
 using HYF = HK<C, H_Y_FWD>;
 using HZG = HK<C, H_Z_GREEN>;
 using HYI = HK<C, H_Y_INV>;
-using C2R = C2RK<C>;
+using C2R = C2RK<C, false>;
+using C2RExt = C2RK<C, true>;
 
 cudaError_t init()
 {
@@ -112,7 +114,7 @@ cudaError_t init()
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     g_ctas = sms * C::MINB;
 #define OPT(K) if ((e = optin<K>()) != cudaSuccess) return e;
-    OPT(PsiZKick) OPT(PsiZ) OPT(PsiS) OPT(PsiX) OPT(PsiXRho) OPT(RhoOnly) OPT(HYF) OPT(HZG) OPT(HYI) OPT(C2R)
+    OPT(PsiZKick) OPT(PsiZKickX) OPT(C2RExt) OPT(PsiZ) OPT(PsiS) OPT(PsiX) OPT(PsiXRho) OPT(RhoOnly) OPT(HYF) OPT(HZG) OPT(HYI) OPT(C2R)
 #undef OPT
     g_chain_ctas = g_ctas;
     if ((e = chain_optin<PsiZKick, PsiS>(sms)) != cudaSuccess) return e;
@@ -159,7 +161,7 @@ cudaError_t h_yzy(const void *py, const void *pz, const ChainCtl *ctl, cudaStrea
 
 cudaError_t psi_z(const void *pp, int kick, cudaStream_t s)
 {
-    return kick ? launch<PsiZKick>(pp, kTilesGrid, s) : launch<PsiZ>(pp, kTilesGrid, s);
+    return kick == 2 ? launch<PsiZKickX>(pp, kTilesGrid, s) : (kick ? launch<PsiZKick>(pp, kTilesGrid, s) : launch<PsiZ>(pp, kTilesGrid, s));
 }
 cudaError_t psi_strided(const void *pp, int along_x, cudaStream_t s)
 {
@@ -172,7 +174,10 @@ cudaError_t psi_x_rho(const void *pp, int drift, cudaStream_t s)
 cudaError_t h_y_fwd(const void *pp, cudaStream_t s) { return launch<HYF>(pp, kTilesHalf, s); }
 cudaError_t h_z_green(const void *pp, cudaStream_t s) { return launch<HZG>(pp, kTilesHalf, s); }
 cudaError_t h_y_inv(const void *pp, cudaStream_t s) { return launch<HYI>(pp, kTilesHalf, s); }
-cudaError_t c2r(const void *pp, cudaStream_t s) { return launch<C2R>(pp, kTilesGrid, s); }
+cudaError_t c2r(const void *pp, cudaStream_t s)
+{
+    return static_cast<const P *>(pp)->phi_ext ? launch<C2RExt>(pp, kTilesGrid, s) : launch<C2R>(pp, kTilesGrid, s);
+}
 
 const SweepTable kTable = {Fact{C::N, C::RA, C::RB, C::RM, C::W, C::NT, C::NG, C::MINB}, WDM_DTYPE, init, psi_z,
                            psi_strided, psi_x_rho, h_y_fwd, h_z_green, h_y_inv, c2r, chain_lag, psi_zy, h_yzy};

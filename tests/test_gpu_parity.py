@@ -301,6 +301,51 @@ def test_t512_sampled_properties(wdm):
     sim.close()
 
 
+def test_config4_1024_closed_forms(wdm):
+    """Config 4's size (1024^3 complex64; a float64 oracle run would need > 50 GB): properties that hold at any
+    size, evaluated on the device.  (1) plane wave with all three wavenumbers non-zero: Phi = 0 and
+    psi(t) = A exp(i(k.x - mu k^2 t/2)) exactly (P3) -- every twiddle, digit reversal and kinetic-phase index of
+    the 1024-point sweeps; (2) rho = r0 + r1 cos(k.x): Phi = -4 pi G r1 cos(k.x)/k^2 (P4) -- the real-to-complex,
+    Green and complex-to-real sweeps; (3) unitarity of two steps on a noisy field."""
+    import torch
+    N, L = 1024, 1.0
+    dt = (L / N) ** 2 / 6
+    x = (-0.5 * L + (L / N) * torch.arange(N, device="cuda", dtype=torch.float64))
+    n = (3, -7, 11)
+    k = [2 * math.pi * v / L for v in n]
+    sim = wdm.Sim(N, dtype="c64")
+    ph = (k[0] * x)[:, None, None] + (k[1] * x)[None, :, None] + (k[2] * x)[None, None, :]
+    A = 0.7
+    psi = torch.polar(torch.full_like(ph, A), ph).to(torch.complex64)
+    sim.set_psi(psi)
+    sim.step(3, dt)
+    k2 = sum(v * v for v in k)
+    exact = torch.polar(torch.full_like(ph, A), ph - 0.5 * k2 * 3 * dt)
+    out = sim.psi()
+    err = float(torch.linalg.vector_norm((out.to(torch.complex128) - exact).flatten()) / torch.linalg.vector_norm(exact.flatten()))
+    assert err <= 2e-5, err
+    assert float(sim.potential().abs().max()) < 1e-5
+    del psi, exact, out
+    r0, r1 = 2.0, 0.5
+    c = torch.cos(ph)
+    sim.set_psi(torch.sqrt(r0 + r1 * c).to(torch.complex64))
+    sim.step(0, 0.0)
+    phi = sim.potential().double()
+    ref = -r1 * c / k2                                  # 4 pi G = 1
+    assert float(torch.linalg.vector_norm((phi - ref).flatten()) / torch.linalg.vector_norm(ref.flatten())) <= 2e-5
+    del phi, ref, c, ph
+    g = torch.Generator(device="cuda"); g.manual_seed(4)
+    psi = torch.randn((N, N, N, 2), generator=g, device="cuda", dtype=torch.float32) * 0.3
+    psi[..., 0] += 1.0
+    psi = torch.view_as_complex(psi).contiguous()
+    n0 = float((psi.abs().double() ** 2).sum())
+    sim.set_psi(psi)
+    sim.step(2, dt)
+    n1 = float((sim.psi().abs().double() ** 2).sum())
+    assert abs(n1 / n0 - 1) < 1e-5
+    sim.close()
+
+
 # ---------------------------------------------------------------- L2-chained sweeps: same arithmetic, different schedule
 
 @pytest.mark.parametrize("dtype,N,G", [("c64", 128, 1.0), ("c128", 128, 1.0), ("c64", 256, 1.0), ("c128", 256, 0.0),
