@@ -124,7 +124,7 @@ int wdm_get_diagnostics(wdm_ctx *ctx, double *out_host);
  * kernel.  Bit 1 (2): the y-forward, z-Green, y-inverse sweeps of the Poisson solve (Eq. 18(c)
  * PAPER.md:194, Eq. 23) run as one kernel.  In a chained kernel the later stage trails
  * the earlier one by `lag` x-planes and reads them from L2 instead of HBM.  mode 0: one launch per
- * sweep.  Default: 2 for N >= 512, else 0.  lag <= 0 picks the lag automatically.  wdm_get_chain reports the lags in use
+ * sweep.  Default: 0.  lag <= 0 picks the lag automatically.  wdm_get_chain reports the lags in use
  * (0 = that chain runs as separate sweeps, e.g. because the grid is too small for it to be
  * meaningful).  The environment variables WDM_CHAIN=<mode> and WDM_CHAIN_LAG=<planes> set the
  * defaults of new contexts. */

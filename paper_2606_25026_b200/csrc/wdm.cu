@@ -193,6 +193,7 @@ struct wdm_ctx {
     unsigned int *chain_done = nullptr;       // [N] for psi z->y, then [2 (N/2+1)] for H y->z->y
     unsigned int epoch_psi = 0, epoch_h = 0;
     int lag_psi = 0, lag_h = 0;
+    int ticket_parity = 0;
     ParticleState part;
     long long max_particles = -1;   // -1: unbounded (cudaMalloc on demand)
     // instrumentation
@@ -390,6 +391,17 @@ static int ensure_mask(wdm_ctx *c, double dt)
     return WDM_OK;
 }
 
+// Tile-ticket counters of the sweeps: two words used by alternate launches (a launch draws from one and zeroes the
+// other for its successor on the stream).  Call once per sweep launch, right before it.
+template <typename T>
+static void take_ticket(wdm_ctx *c, SweepParams<T> &p)
+{
+    unsigned int *base = c->chain_done + 2 * c->N + 2;
+    p.ticket = base + c->ticket_parity;
+    p.ticket_next = base + (c->ticket_parity ^ 1);
+    c->ticket_parity ^= 1;
+}
+
 template <typename T>
 static SweepParams<T> base_params(wdm_ctx *c)
 {
@@ -407,7 +419,6 @@ static SweepParams<T> base_params(wdm_ctx *c)
     p.phi_out = (T *)c->phi;
     p.rho_p = c->part.n > 0 ? (const T *)c->part.rho_p : nullptr;
     p.rho_mean = (const T *)((const unsigned char *)c->rho_mean + 16);
-    p.ticket = c->chain_done + 2 * N + 2;
     p.phi_ext = (const T *)c->phi_ext;
     return p;
 }
@@ -424,6 +435,7 @@ static int density_poisson(wdm_ctx *c, bool drift)
         p.data = (cx<T> *)c->psi;
         p.tmap = c->tm_psi_x;
         p.tag = S_PSI_X_RHO;
+        take_ticket(c, p);
         Timed t(c, S_PSI_X_RHO);
         CU(c, c->tab->psi_x_rho(&p, drift ? 1 : 0, c->stream));
     }
@@ -436,13 +448,13 @@ static int density_poisson(wdm_ctx *c, bool drift)
         Timed t(c, S_H_YZY);
         CU(c, c->tab->h_yzy(&p, &p, &ctl, c->stream));
     } else {
-        { p.tag = S_H_Y_FWD; Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
-        { p.tag = S_H_Z_GREEN; Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
-        { p.tag = S_H_Y_INV; Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
+        { p.tag = S_H_Y_FWD; take_ticket(c, p); Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
+        { p.tag = S_H_Z_GREEN; take_ticket(c, p); Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
+        { p.tag = S_H_Y_INV; take_ticket(c, p); Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
     }
     p.tmap = c->tm_h_x;
     p.tmap2 = c->tm_h_x1;
-    { p.tag = S_C2R; Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, c->stream)); }
+    { p.tag = S_C2R; take_ticket(c, p); Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, c->stream)); }
     return WDM_OK;
 }
 
@@ -527,8 +539,8 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
                 Timed t(c, S_PSI_ZY);
                 CU(c, c->tab->psi_zy(&pz, &py, kicks ? 1 : 0, &ctl, c->stream));
             } else {
-                { pz.tag = S_PSI_Z; Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? (pz.kick_extra ? 2 : 1) : 0, c->stream)); }
-                { py.tag = S_PSI_Y; Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
+                { pz.tag = S_PSI_Z; take_ticket(c, pz); Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? (pz.kick_extra ? 2 : 1) : 0, c->stream)); }
+                { py.tag = S_PSI_Y; take_ticket(c, py); Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
             }
         }
         if (grav) {
@@ -538,6 +550,7 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             SweepParams<T> p = base_params<T>(c);
             p.data = (cx<T> *)c->psi;
             p.tmap = c->tm_psi_x;
+            take_ticket(c, p);
             Timed t(c, S_PSI_Y);
             CU(c, c->tab->psi_strided(&p, 1, c->stream));
         }
@@ -622,9 +635,10 @@ static int create_common(wdm_ctx **out, int N, double L, double mu, double G, in
         const char *env = getenv("WDM_CHAIN");             // bit mask as in wdm_set_chain
         const char *lag = getenv("WDM_CHAIN_LAG");
         int req = lag ? atoi(lag) : 0;
-        // default: chain the Poisson sweeps once the half spectrum is far larger than L2 (measured: -12 % on them at
-        // 512^3, a loss at 256^3 and below where the array is L2-resident anyway); never the psi pair (slower)
-        int mode = env ? atoi(env) : (N >= 512 ? 2 : 0);
+        // default: separate sweeps.  Measured at 512^3 (end of round 1): the chained Poisson kernel moves a third of
+        // the DRAM bytes of its three sweeps but takes 0.59 ms against their 0.57 ms (the y sweeps run at 93-95 % of
+        // the HBM floor on their own; the chain pays for its dependency waits), the psi pair is clearly slower
+        int mode = env ? atoi(env) : 0;
         if (mode & 1) c->lag_psi = c->tab->chain_lag(2, N, req);
         if (mode & 2) c->lag_h = c->tab->chain_lag(3, N / 2 + 1, req);
     }

@@ -216,7 +216,10 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
         unsigned char *buf = smem + (size_t)b * SM::TILE_BYTES;
         const TileRef r = chain_decode(cp, bid + j * stride);
         WDM_T(t_top);
-        while (issued[b] < j / NBUF + 1) __nanosleep(64);
+        // one warp polls for the start of this fill (the others would only burn issue slots the other group needs)
+        if (gt < 32)
+            while (issued[b] < j / NBUF + 1) __nanosleep(100);
+        group_sync(grp, NTG);
         mbar_wait(full + b, (j / NBUF) & 1);
         WDM_T(t_data);
         auto hook = [&]() { prefetch_for(j + NG); };

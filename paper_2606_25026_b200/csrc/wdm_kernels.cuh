@@ -121,7 +121,8 @@ struct SweepParams {
     // TMA descriptors of the array a strided sweep walks: boxes of (W elements along z) x (<= 256 rows along the
     // sweep axis); tmap2 is the one-row box that fetches row N/2 of the half spectrum in the complex-to-real sweep
     CUtensorMap tmap, tmap2;
-    unsigned int *ticket;      // [0] tile tickets drawn in this launch, [1] CTAs that have left (both 0 between launches)
+    unsigned int *ticket;      // tile tickets drawn in this launch (0 when the launch starts)
+    unsigned int *ticket_next; // the next launch's counter: this launch zeroes it (launches alternate between two words)
     int tag;                   // which launch of the step this is (kernel-stats slot; read by developer traces only)
 };
 

@@ -161,6 +161,7 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
     volatile int *tile_of = issued + NBUF;
     static_assert(NBUF * (sizeof(uint64_t) + 2 * sizeof(int)) <= 64, "control block");
     const int nstatic = NBUF * stride;
+    if (tid == 0 && bid == 0) *p.ticket_next = 0;               // the launch before this one has finished with it
     if (tid == 0)
         for (int b = 0; b < NBUF; ++b) {
             mbar_init(full + b, 1);
@@ -202,7 +203,10 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
         const int b = k % NBUF;
         unsigned char *buf = smem + (size_t)b * K::TILE_BYTES;
         WDM_T(t_top);
-        while (issued[b] < k / NBUF + 1) __nanosleep(64);
+        // one warp polls for the start of this fill (the others would only burn issue slots the other group needs)
+        if (gt < 32)
+            while (issued[b] < k / NBUF + 1) __nanosleep(100);
+        group_sync(grp, NTG);
         const int t = tile_of[b];
         if (t < 0) {
             // nothing left for this group: pass the end mark on to the tile that would have followed in this
@@ -241,12 +245,6 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
 #ifdef WDM_TRACE
         if (gt == 0) trace_put(p.tag, grp, NG, k / NG, 0, t_top, t_data, t_done, clock64());
 #endif
-    }
-    // the last CTA to leave rewinds the ticket counter for the next launch on this stream
-    __syncthreads();
-    if (tid == 0) {
-        const unsigned int left = atomicAdd(p.ticket + 1, 1u);
-        if (left == gridDim.x - 1) { p.ticket[0] = 0; p.ticket[1] = 0; }
     }
 }
 
