@@ -71,8 +71,11 @@ int wdm_set_particles_host(wdm_ctx *ctx, long long n, const void *pos_host, cons
 /* Advance nsteps kick-drift-kick steps of size dt (Eq. 17-18; Alg. 1 l.5-16
  * PAPER.md:247-267; particles: leapfrog KDK sharing dt, G14-G15).  nsteps >= 0; dt may be negative
  * (time reversal).  If Phi is stale it is first recomputed from the current (psi, x); nsteps = 0 does
- * only that.  On return (stream-ordered) psi, x, v are at the same time level and Phi / rho are the
- * ones consistent with them.  Asynchronous: no host synchronisation. */
+ * only that.  After the call psi, x, v are at the same time level and Phi / rho are the ones consistent
+ * with them -- as seen through every wdm_get_*: the closing half kicks of the last step (and its absorbing
+ * layer) are kept pending and folded into the opening kick of the next wdm_step with the same dt, or applied
+ * by the next call that reads the state, changes dt or changes a parameter (so a loop of wdm_step(1, dt)
+ * costs no extra pass over psi).  Asynchronous: no host synchronisation. */
 int wdm_step(wdm_ctx *ctx, int nsteps, double dt);
 
 /* Whole user call with HOST buffers: copy psi in, wdm_step(nsteps, dt), copy psi out, synchronise. */

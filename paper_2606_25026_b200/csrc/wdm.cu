@@ -194,6 +194,9 @@ struct wdm_ctx {
     unsigned int epoch_psi = 0, epoch_h = 0;
     int lag_psi = 0, lag_h = 0;
     int ticket_parity = 0;
+    // closing half kicks not applied yet (dt of the call that owes them; 0 = none): they merge with the opening
+    // half kick of the next wdm_step, or are applied when the state is read or a parameter changes
+    double pend_psi = 0, pend_part = 0;
     ParticleState part;
     long long max_particles = -1;   // -1: unbounded (cudaMalloc on demand)
     // instrumentation
@@ -501,11 +504,43 @@ static int refresh(wdm_ctx *c)
     return WDM_OK;
 }
 
+// Apply the closing half kick(s) a previous wdm_step left pending (psi: half kick with Phi, then the absorbing layer;
+// particles: v += a dt/(2 nsub)).  Phi and the kick parameters must still be the ones of that step.
+template <typename T>
+static int flush_pending(wdm_ctx *c, bool psi, bool part)
+{
+    const bool layer = c->alpha > 0;
+    if (psi && c->pend_psi != 0.0) {
+        const double dt = c->pend_psi;
+        int rc = ensure_mask<T>(c, dt);
+        if (rc) return rc;
+        Timed t(c, S_KICK);
+        if (c->kappa != 0.0 || layer)
+            k_kick_general<T><<<148 * 8, 256, 0, c->stream>>>((cx<T> *)c->psi, (const T *)c->phi, (T)(0.5 * dt / c->mu),
+                                                                (T)(c->kappa * 0.5 * dt / c->mu), (T)0, layer ? (const T *)c->mask : nullptr,
+                                                                c->N, c->n);
+        else
+            k_kick<T><<<148 * 8, 256, 0, c->stream>>>((cx<T> *)c->psi, (const T *)c->phi, (T)(0.5 * dt / c->mu), c->n);
+        CU(c, cudaGetLastError());
+        c->pend_psi = 0.0;
+    }
+    if (part && c->pend_part != 0.0) {
+        Timed t(c, S_PART_PUSH);
+        CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, 0.5 * c->pend_part / c->nsub, 0.0, 1, c->stream));
+        c->pend_part = 0.0;
+    }
+    return WDM_OK;
+}
+
 template <typename T>
 static int step_impl(wdm_ctx *c, int nsteps, double dt)
 {
     int rc = refresh<T>(c);
     if (rc || nsteps == 0) return rc;
+    // a pending closing kick merges with this call's opening kick only if both use the same dt (one table of
+    // absorbing-layer factors, one sub-step size)
+    if ((c->pend_psi != 0.0 && c->pend_psi != dt) || (c->pend_part != 0.0 && c->pend_part != dt))
+        if ((rc = flush_pending<T>(c, true, true))) return rc;
     rc = ensure_phase<T>(c, dt);
     if (rc) return rc;
     rc = ensure_mask<T>(c, dt);
@@ -516,11 +551,13 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
     const bool layer = c->alpha > 0;
     const bool kicks = have_phi || c->kappa != 0.0 || layer;
     for (int s = 0; s < nsteps; ++s) {
-        // merged closing (h_d, of the previous step) + opening (h_a) half kicks (G21); the layer sits between them
-        const double hd = s == 0 ? 0.0 : 0.5 * dt, ha = 0.5 * dt, kdt = hd + ha;
+        // merged closing (h_d, of the previous step -- possibly of the previous call) + opening (h_a) half kicks
+        // (G21); the absorbing layer sits between them
+        const double hd = s == 0 ? 0.5 * c->pend_psi : 0.5 * dt, ha = 0.5 * dt, kdt = hd + ha;
+        const double hd_p = s == 0 ? 0.5 * c->pend_part : 0.5 * dt;
         if (c->part.n > 0 && !c->pstatic) {
             // v += a(Phi^n, x^n) kdt/nsub ; nsub x { x += v dt/nsub ; wrap ; [kick] } ; then deposit x^{n+1}  (G14-G16, G29)
-            { Timed t(c, S_PART_PUSH); CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, have_phi ? kdt / c->nsub : 0.0, dt, c->nsub, c->stream)); }
+            { Timed t(c, S_PART_PUSH); CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, have_phi ? (hd_p + ha) / c->nsub : 0.0, dt, c->nsub, c->stream)); }
             if (grav) { rc = particles_deposit<T>(c); if (rc) return rc; }
         }
         {
@@ -529,7 +566,7 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             pz.kick = (T)(kdt / c->mu);
             pz.kself_d = (T)(c->kappa * hd / c->mu);
             pz.kself_a = (T)(c->kappa * ha / c->mu);
-            pz.mask = layer && s > 0 ? (const T *)c->mask : nullptr;
+            pz.mask = layer && hd != 0.0 ? (const T *)c->mask : nullptr;
             pz.kick_extra = (c->kappa != 0.0 || pz.mask != nullptr) ? 1 : 0;
             py.data = (cx<T> *)c->psi;
             py.tmap = c->tm_psi_y;
@@ -543,6 +580,8 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
                 { py.tag = S_PSI_Y; take_ticket(c, py); Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
             }
         }
+        c->pend_psi = 0.0;
+        c->pend_part = 0.0;
         if (grav) {
             rc = density_poisson<T>(c, true);
             if (rc) return rc;
@@ -555,22 +594,16 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             CU(c, c->tab->psi_strided(&p, 1, c->stream));
         }
     }
-    if (kicks) {
-        // closing half kick of the last step, then its absorbing layer
-        Timed t(c, S_KICK);
-        if (c->kappa != 0.0 || layer)
-            k_kick_general<T><<<148 * 8, 256, 0, c->stream>>>((cx<T> *)c->psi, (const T *)c->phi, (T)(0.5 * dt / c->mu),
-                                                                (T)(c->kappa * 0.5 * dt / c->mu), (T)0, layer ? (const T *)c->mask : nullptr,
-                                                                c->N, c->n);
-        else
-            k_kick<T><<<148 * 8, 256, 0, c->stream>>>((cx<T> *)c->psi, (const T *)c->phi, (T)(0.5 * dt / c->mu), c->n);
-        CU(c, cudaGetLastError());
-    }
-    if (have_phi && c->part.n > 0 && !c->pstatic) {
-        Timed t(c, S_PART_PUSH);
-        CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, 0.5 * dt / c->nsub, 0.0, 1, c->stream));
-    }
+    // the closing half kicks (and the last absorbing layer) stay pending: the next wdm_step merges them into its
+    // opening kick; a read of the state or a change of parameters applies them first (flush_pending)
+    c->pend_psi = kicks ? dt : 0.0;
+    c->pend_part = (have_phi && c->part.n > 0 && !c->pstatic) ? dt : 0.0;
     return WDM_OK;
+}
+
+static int do_flush(wdm_ctx *c, bool psi, bool part)
+{
+    return c->dtype == WDM_C64 ? flush_pending<float>(c, psi, part) : flush_pending<double>(c, psi, part);
 }
 
 // ---------------------------------------------------------------- C ABI
@@ -689,6 +722,10 @@ static int set_psi(wdm_ctx *c, const void *psi, cudaMemcpyKind kind)
 {
     if (!c) return WDM_EINVAL;
     if (!psi) return fail(c, WDM_EINVAL, "null psi");
+    // the particles still owe the closing half kick of the last step (with the old Phi); psi's is moot
+    int rcf = do_flush(c, false, true);
+    if (rcf) return rcf;
+    c->pend_psi = 0.0;
     CU(c, cudaMemcpyAsync(c->psi, psi, c->n * csize(c->dtype), kind, c->stream));
     c->have_psi = true;
     c->stale = true;
@@ -703,6 +740,11 @@ static int set_particles(wdm_ctx *c, long long n, const void *pos, const void *v
     if (!c) return WDM_EINVAL;
     if (n < 0 || (n > 0 && (!pos || !vel))) return fail(c, WDM_EINVAL, "bad particle arguments");
     if (c->max_particles >= 0 && n > c->max_particles) return fail(c, WDM_ENOMEM, "%lld particles > max_particles %lld of the workspace", n, c->max_particles);
+    {   // psi still owes the closing half kick of the last step (with the old Phi); the old particles' is moot
+        int rcf = do_flush(c, true, false);
+        if (rcf) return rcf;
+        c->pend_part = 0.0;
+    }
     if (c->owns && n > c->part.capacity) {
         size_t rs = rsize(c->dtype);
         void *rho_p = c->part.rho_p, *pm = nullptr;
@@ -740,6 +782,10 @@ static int get_grid(wdm_ctx *c, void *out, int what, cudaMemcpyKind kind)
     if (!c) return WDM_EINVAL;
     if (!out) return fail(c, WDM_EINVAL, "null output");
     if (!c->have_psi) return fail(c, WDM_ESTATE, "wdm_set_psi has not been called");
+    if (what != 1) {                 // psi, or the density (the absorbing layer of a pending kick changes |psi|)
+        int rcf = do_flush(c, true, false);
+        if (rcf) return rcf;
+    }
     if (what == 0) {
         CU(c, cudaMemcpyAsync(out, c->psi, c->n * csize(c->dtype), kind, c->stream));
     } else {
@@ -778,6 +824,10 @@ extern "C" int wdm_get_density_host(wdm_ctx *c, void *o) { return get_grid(c, o,
 static int get_particles(wdm_ctx *c, void *pos, void *vel, bool host)
 {
     if (!c) return WDM_EINVAL;
+    {
+        int rcf = do_flush(c, false, true);
+        if (rcf) return rcf;
+    }
     if (c->part.n > 0) {
         c->launches += 1;
         cudaError_t e = particle_get(c->part, c->dtype, pos, vel, host, c->stream);
@@ -808,6 +858,8 @@ extern "C" int wdm_set_particle_mode(wdm_ctx *c, int substeps, int is_static)
 {
     if (!c) return WDM_EINVAL;
     if (substeps < 1) return fail(c, WDM_EINVAL, "substeps must be >= 1");
+    int rcf = do_flush(c, true, true);
+    if (rcf) return rcf;
     c->nsub = substeps;
     c->pstatic = is_static != 0;
     return WDM_OK;
@@ -819,6 +871,7 @@ extern "C" int wdm_get_diagnostics(wdm_ctx *c, double *out_host)
     if (!out_host) return fail(c, WDM_EINVAL, "null output");
     int rc = do_refresh(c);
     if (rc) return rc;
+    if ((rc = do_flush(c, true, false))) return rc;
     // scratch: the 64-byte block of the <rho> accumulators is free between refreshes except for the mean at byte 16;
     // use the first 48 bytes of the head of H instead (H is dead outside a Poisson solve)
     double *acc = (double *)c->H;
@@ -853,6 +906,8 @@ extern "C" int wdm_set_kick_terms(wdm_ctx *c, double kappa, const void *phi_ext_
     if (!c) return WDM_EINVAL;
     if (kappa != kappa || !(absorb_alpha >= 0) || (absorb_alpha > 0 && absorb_nb < 1))
         return fail(c, WDM_EINVAL, "need a finite kappa, absorb_alpha >= 0 and absorb_nb >= 1");
+    int rcf = do_flush(c, true, true);           // pending closing kicks belong to the old terms
+    if (rcf) return rcf;
     c->kappa = kappa;
     c->phi_ext = phi_ext_dev;
     c->alpha = absorb_alpha;

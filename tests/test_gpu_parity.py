@@ -260,7 +260,13 @@ def test_state_semantics_and_errors(wdm):
     assert torch.equal(buf, psi)
     n0 = wdm.wdm_launch_count(h)
     wdm.wdm_step(h, 2, 1e-4)
-    assert wdm.wdm_launch_count(h) - n0 == 2 * 7 + 1    # 7 sweeps per step + the closing half kick
+    assert wdm.wdm_launch_count(h) - n0 == 2 * 7        # 7 sweeps per step; the closing half kick stays pending
+    wdm.wdm_step(h, 1, 1e-4)                             # ... and merges into the next call's opening kick
+    assert wdm.wdm_launch_count(h) - n0 == 3 * 7
+    wdm.wdm_get_psi(h, buf)                              # reading psi applies it (one elementwise kernel)
+    assert wdm.wdm_launch_count(h) - n0 == 3 * 7 + 1
+    wdm.wdm_get_psi(h, buf)
+    assert wdm.wdm_launch_count(h) - n0 == 3 * 7 + 1
     wdm.wdm_destroy(h)
 
 
@@ -492,4 +498,49 @@ def test_particle_modes_match_oracle(wdm, dtype, mode):
     assert np.abs(d).max() <= (POS_TOL if dtype == "c64" else 1e-12) * w.L
     assert rel(v.cpu().numpy(), vo) <= (1e-4 if dtype == "c64" else 1e-11)
     check_fields(sim, o, dtype, 4, str(mode))
+    sim.close()
+
+
+# ---------------------------------------------------------------- closing kicks deferred across wdm_step calls
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_deferred_closing_kick_call_patterns(wdm, dtype):
+    """The closing half kick of a call is merged into the next call's opening kick (same dt) or applied when the
+    state is read, dt changes, or a setter intervenes.  Every pattern must reproduce the oracle, which applies
+    both half kicks in every step."""
+    w = wl.small_coupled(32, dtype=dtype)
+    sim, o = pair(wdm, w, max_particles=len(w.pos))
+    kw = dict(kappa=2.0, absorb_alpha=0.05 / w.dt, absorb_nb=10)
+    sim.set_kick_terms(**kw); o.set_kick_terms(**kw)
+    pos_tol = (POS_TOL if dtype == "c64" else 1e-12) * w.L
+
+    def check(n, what):
+        p, v = sim.particles()
+        po, vo = o.particles()
+        d = p.cpu().numpy() - po
+        d -= w.L * np.round(d / w.L)
+        assert np.abs(d).max() <= pos_tol, what
+        assert rel(v.cpu().numpy(), vo) <= (1e-4 if dtype == "c64" else 1e-10), what
+        assert rel(sim.psi().cpu().numpy(), o.psi()) <= tol(dtype, n), what
+
+    for _ in range(3):                                   # same dt, nothing read in between: merged across calls
+        sim.step(1, w.dt); o.step(1, w.dt)
+    check(3, "three merged calls")
+    sim.step(2, w.dt); o.step(2, w.dt)
+    sim.step(2, 0.5 * w.dt); o.step(2, 0.5 * w.dt)        # dt changes: the pending kick is applied first
+    check(7, "dt change")
+    sim.step(1, w.dt); o.step(1, w.dt)
+    sim.set_kick_terms(kappa=-1.0); o.set_kick_terms(kappa=-1.0)     # parameters change with a kick pending
+    sim.step(2, w.dt); o.step(2, w.dt)
+    check(10, "terms change")
+    # new particles while psi's closing kick is pending, then new psi while the particles' is pending
+    sim.step(1, w.dt); o.step(1, w.dt)
+    p0, v0 = o.particles()
+    sim.set_particles(p0[::-1].copy(), v0[::-1].copy(), w.mass); o.set_particles(p0[::-1].copy(), v0[::-1].copy(), w.mass)
+    sim.step(1, w.dt); o.step(1, w.dt)
+    psi_now = o.psi().astype(np.complex64 if dtype == "c64" else np.complex128)
+    sim.set_psi(psi_now); o.set_psi(psi_now)
+    sim.step(2, w.dt); o.step(2, w.dt)
+    check(14, "setters with kicks pending")
+    check_fields(sim, o, dtype, 14, "fields at the end")
     sim.close()
