@@ -33,7 +33,6 @@ struct ChainParams {
     unsigned int *done;          // (NS - 1) x units completion counters, monotone across launches
     unsigned int target;         // value a complete plane's counter has reached in this launch
     int units, tpu_log2, lag, total, nseg;
-    int debug;                   // experiments only: 1 = do not wait for dependencies, 2 = do not signal either
     int seg_pos[2 * NS + 1], seg_slot[2 * NS], seg_lo[2 * NS], seg_v[2 * NS];
 };
 
@@ -182,7 +181,7 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
     // the planes the tile depends on, then the warp issues the bulk copies; the other warps go on to their next tile
     auto request = [&](int j, int b) {
         const TileRef r = chain_decode(cp, bid + j * stride);
-        if (r.stage > 0 && !(cp.debug & 1)) {
+        if (r.stage > 0) {
             if (gt == 0) {
                 const unsigned int *ctr = cp.done + (size_t)(r.stage - 1) * cp.units + r.unit;
                 while ((int)(ld_acquire(ctr) - cp.target) < 0) __nanosleep(100);
@@ -241,7 +240,7 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
         WDM_T(t_done);
         if (gt < 32) {
             // release: the group's stores (ordered before this thread by the barrier) are visible before the count
-            if (gt == 0 && r.stage < NS - 1 && !(cp.debug & 2)) red_release_add(cp.done + (size_t)r.stage * cp.units + r.unit, 1u);
+            if (gt == 0 && r.stage < NS - 1) red_release_add(cp.done + (size_t)r.stage * cp.units + r.unit, 1u);
             if (j < NG)
                 for (int jj = j + NG; jj < NBUF && jj < J; jj += NG) request(jj, jj);
             if (j + NBUF < J) {

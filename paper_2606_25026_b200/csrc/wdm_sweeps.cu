@@ -1,7 +1,5 @@
 // wdm_sweeps.cu -- __global__ wrappers of the pipelined sweeps for ONE (dtype, N), selected at compile time
 // with -DWDM_DTYPE={0,1} -DWDM_N=<N>.  build.py compiles this file once per supported size.
-#include <cstdlib>
-
 #include "wdm_internal.hpp"
 #include "wdm_chain.cuh"
 
@@ -85,7 +83,6 @@ cudaError_t chain_launch(ChainParams<Real, (int)sizeof...(KS)> &cp, int planes, 
 {
     chain_plan(cp, planes, kTilesPerPlane, ctl->lag);
     cp.done = ctl->done;
-    { const char *d = getenv("WDM_CHAIN_DEBUG"); cp.debug = d ? atoi(d) : 0; }
     cp.target = ctl->target;
     int grid = cp.total < g_chain_ctas ? cp.total : g_chain_ctas;
     if (grid <= 0 || chain_min_distance(kTilesPerPlane, ctl->lag < planes ? ctl->lag : planes) <= grid) return cudaErrorInvalidConfiguration;
