@@ -6,7 +6,8 @@
 //   psi sweep y
 //   psi sweep x + rho = |psi|^2 + rho_p + real-to-complex x-spectrum -> H
 //   H sweep y forward, H sweep z forward . Green . inverse, H sweep y inverse, x complex-to-real -> Phi
-// and once at the end the closing half kick.  Nothing synchronises with the host.
+// The closing half kick of the call stays pending: the next wdm_step folds it into its opening kick, a read of the
+// state applies it (flush_pending).  Nothing synchronises with the host.
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -174,7 +175,6 @@ struct wdm_ctx {
     void *psi = nullptr, *phi = nullptr, *H = nullptr;
     void *rho_mean = nullptr;   // [0..1] double accumulators, then the mean as T at byte offset 16
     void *twA = nullptr, *twB = nullptr, *phase = nullptr, *ksq_pos = nullptr, *ksq_nat = nullptr;
-    unsigned short *pos_of_k = nullptr;
     double phase_dt = 0;
     bool phase_valid = false, have_psi = false, stale = true;
     // L2-chained sweeps (wdm_chain.cuh): completion counters, launch epochs, lag per chain (0: separate sweeps)
@@ -356,7 +356,6 @@ static int upload_tables(wdm_ctx *c)
     CU(c, cudaMemcpyAsync(c->twB, t.twB.data(), t.twB.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(c->ksq_pos, t.ksq_pos.data(), t.ksq_pos.size() * sizeof(T), cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(c->ksq_nat, t.ksq_nat.data(), t.ksq_nat.size() * sizeof(T), cudaMemcpyHostToDevice, c->stream));
-    CU(c, cudaMemcpyAsync(c->pos_of_k, t.pos_of_k.data(), t.pos_of_k.size() * 2, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));   // host vectors die here
     return WDM_OK;
 }
@@ -413,7 +412,6 @@ static SweepParams<T> base_params(wdm_ctx *c)
     p.twA = (const cx<T> *)c->twA;
     p.twB = (const cx<T> *)c->twB;
     p.phase = (const cx<T> *)c->phase;
-    p.pos_of_k = c->pos_of_k;
     p.ksq_pos = (const T *)c->ksq_pos;
     p.ksq_nat = (const T *)c->ksq_nat;
     p.green = (T)(-4.0 * M_PI * c->G / ((double)N * N * N));
@@ -658,7 +656,7 @@ static int create_common(wdm_ctx **out, int N, double L, double mu, double G, in
         (rc = ctx_alloc(c, &c->H, c->nH * cs)) || (rc = ctx_alloc(c, &c->twA, N * cs)) ||
         (rc = ctx_alloc(c, &c->twB, N * cs)) || (rc = ctx_alloc(c, &c->phase, N * cs)) ||
         (rc = ctx_alloc(c, &c->ksq_pos, N * rs)) || (rc = ctx_alloc(c, &c->ksq_nat, N * rs)) ||
-        (rc = ctx_alloc(c, (void **)&c->pos_of_k, N * 2)) || (rc = ctx_alloc(c, &c->rho_mean, 64)) ||
+        (rc = ctx_alloc(c, &c->rho_mean, 64)) ||
         (rc = ctx_alloc(c, (void **)&c->chain_done, (size_t)(2 * N + 2 + 8) * sizeof(unsigned int))) ||
         (rc = ctx_alloc(c, &c->mask, (size_t)3 * N * rs)))
         return bail(rc);

@@ -13,7 +13,7 @@
 // ends are shorter slots), CTA c owns positions c, c + grid, ... and runs them through the same three-buffer
 // asynchronous pipeline as pipe_run.  A tile of stage s >= 1 is not requested before all TPU tiles of
 // (s - 1, same plane) have been stored: every finished tile bumps a per-(stage, plane) counter with release
-// semantics, the issuing group's thread 0 spins on it with acquire loads before the group's cp.async reads.
+// semantics; lane 0 of the requesting warp spins on it with acquire loads before the warp issues the TMA copies.
 //
 // Progress: dependencies always point to smaller positions; a group blocks only while REQUESTING position
 // g + (NBUF - NG) * grid, g its own next tile, and what it waits for lies more than (NBUF - NG) * grid
@@ -24,8 +24,6 @@
 #include "wdm_pipe.cuh"
 
 namespace wdm {
-
-constexpr int kChainMaxStages = 3;
 
 template <typename T, int NS>
 struct ChainParams {

@@ -114,7 +114,6 @@ struct SweepParams {
     const T *rho_mean;         // RHO: device scalar <rho>, subtracted before the transform (Eq. 23)
     cx<T> *H;                  // RHO / C2R: half spectrum
     T *phi_out;                // C2R: potential out
-    const unsigned short *pos_of_k;  // position holding frequency k after a forward transform
     const T *ksq_pos;          // Green: k^2 of the frequency held at a position
     const T *ksq_nat;          // Green: k^2 of frequency index k (natural)
     T green;                   // Green: -4 pi G / N^3

@@ -1,14 +1,18 @@
 // wdm_pipe.cuh -- persistent, software-pipelined form of the axis sweeps (sm_100a).
 //
-// One CTA per SM walks tiles t = blockIdx.x, blockIdx.x + gridDim.x, ...  The CTA is NG "compute groups" of
-// C::NT threads; tile j of the CTA is transformed by group j % NG inside shared-memory buffer j % (NG+1).
-// A tile is brought in by asynchronous copies (cp.async / LDGSTS -- no registers, no issue slots while in
-// flight) that signal an mbarrier, and the group that has just finished reading a buffer immediately
-// refills it with the tile NG+1 positions ahead, so every load has more than one whole tile-compute time of
-// lead and HBM latency never reaches the math.  Results leave through plain (fire-and-forget) global stores.
+// One CTA per SM.  The CTA is NG "compute groups" of C::NT threads over NG + 1 shared-memory tile buffers; the
+// k-th tile of the CTA is transformed by group k % NG inside buffer k % (NG + 1).  The first NG + 1 tiles are
+// blockIdx.x + k * gridDim.x, every later one is a ticket from a device-wide counter (fast SMs take more tiles).
+// A tile is brought in by TMA -- 3-D tensor boxes for strided tiles, one bulk copy per pencil for contiguous
+// tiles -- issued by the first warp of the group that has just finished with the buffer, for the tile NG + 1
+// positions ahead, so every load has more than one whole tile-compute time of lead and HBM latency never reaches
+// the math.  Results leave through 8 / 16-byte global stores.
 //
-//   full[b]  mbarrier, count = C::NT: every thread of the issuing group attaches its copies with
-//            cp.async.mbarrier.arrive.noinc; the consuming group waits on the phase parity (j / NBUF) & 1.
+//   full[b]   mbarrier, count 1: the issuing lane's arrive.expect_tx carries the tile's byte count, the copies
+//             complete_tx on it; the consuming group waits on the phase parity (k / NBUF) & 1.
+//   issued[b] fills of buffer b started so far; tile_of[b] the tile of the current fill (-1: nothing left).  A
+//             parity wait cannot tell a phase from the one two before it, so the consumer's first warp polls
+//             issued[b] before the group waits on full[b].
 //   group barrier: bar.sync (1 + group), C::NT -- the other group is never stalled by it.
 #pragma once
 
@@ -36,20 +40,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, int parity)
         "}\n" ::"r"(smem_u32(bar)), "r"(parity)
         : "memory");
 }
-__device__ __forceinline__ void cp_async_arrive(uint64_t *bar)
-{
-    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void cp_async16(void *dst, const void *src)
-{
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async8(void *dst, const void *src)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_elem(cx<float> *dst, const cx<float> *src) { cp_async8(dst, src); }
-__device__ __forceinline__ void cp_async_elem(cx<double> *dst, const cx<double> *src) { cp_async16(dst, src); }
 // TMA: the mbarrier of a tile buffer has ONE expected arrival -- the issuing thread's arrive.expect_tx with the
 // tile's byte count -- and completes when the bulk copies have delivered that many bytes.
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
@@ -379,10 +369,7 @@ struct PsiK {
     static constexpr size_t TILE_BYTES = align128(L::ELEMS * sizeof(cx<T>));
     static constexpr int AUX = DRIFT ? AUX_PHASE : AUX_NONE;
     struct Pre { T th[KICK ? ITER : 1][KICK ? RA : 1]; };
-#ifndef WDM_RHO_PAIR
-#define WDM_RHO_PAIR 1
-#endif
-    static constexpr bool PAIR = ax_strided(AX) && pair_ok<C>() && (!RHO || WDM_RHO_PAIR);
+    static constexpr bool PAIR = ax_strided(AX) && pair_ok<C>();
     // the density sweep is short of registers at the end of its last psi stage (two lines of outputs, their
     // |psi|^2 and the twiddles): it fetches the twiddles where it needs them instead of keeping them
     static constexpr bool KEEP_TW = PAIR && !RHO;

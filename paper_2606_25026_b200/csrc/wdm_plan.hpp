@@ -51,7 +51,6 @@ inline bool find_fact(int N, int dtype, Fact &f)
 template <typename T>
 struct Tables {
     std::vector<cx<T>> twA, twB;           // s-major twiddles of level A (N entries) and level B (MB entries)
-    std::vector<unsigned short> pos_of_k;  // N
     std::vector<T> ksq_pos, ksq_nat;       // N each
 };
 
@@ -82,12 +81,10 @@ inline Tables<T> build_tables(const Fact &f, double L)
     if (f.RB > 1)
         for (int s = 0; s < f.RB; ++s)
             for (int q = 0; q < mB; ++q) t.twB[s * mB + q] = unit_root<T>((long long)q * s, MB);
-    t.pos_of_k.resize(N);
     t.ksq_pos.resize(N);
     t.ksq_nat.resize(N);
     for (int p = 0; p < N; ++p) {
         int k = k_of_pos(p, f.RA, f.RB, f.RM);
-        t.pos_of_k[k] = (unsigned short)p;
         double kk = wavenumber(k, N, L);
         t.ksq_pos[p] = (T)(kk * kk);
     }
