@@ -151,7 +151,10 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
     volatile int *tile_of = issued + NBUF;
     static_assert(NBUF * (sizeof(uint64_t) + 2 * sizeof(int)) <= 64, "control block");
     const int nstatic = NBUF * stride;
-    if (tid == 0 && bid == 0) *p.ticket_next = 0;               // the launch before this one has finished with it
+    // Programmatic dependent launch: let the next sweep's CTAs take SMs as this grid's CTAs retire, and do everything
+    // that does not depend on the previous kernel (control block, lookup tables: written by the host before any
+    // launch) before waiting for it -- the launch latency and this prologue then hide behind the predecessor's tail.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (tid == 0)
         for (int b = 0; b < NBUF; ++b) {
             mbar_init(full + b, 1);
@@ -182,6 +185,8 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
         for (int i = tid; i < C::N; i += NTG * NG) a[i] = p.ksq_pos[i];
         tb.ksq_pos = a;
     }
+    asm volatile("griddepcontrol.wait;" ::: "memory");         // the previous kernel on the stream is complete and visible
+    if (tid == 0 && bid == 0) *p.ticket_next = 0;               // the launch before this one has finished with it
     __syncthreads();
     for (int k = 0; k < NBUF; ++k)
         if (k % NG == grp && gt < 32 && tile_of[k] >= 0) K::issue(p, tile_of[k], smem + (size_t)k * K::TILE_BYTES, full + k, gt);

@@ -58,8 +58,19 @@ template <class K>
 cudaError_t launch(const void *pp, int ntiles, cudaStream_t s)
 {
     int grid = ntiles < g_ctas ? ntiles : g_ctas;
-    k_pipe<K><<<grid, kThreads, smem_of<K>(), s>>>(*static_cast<const P *>(pp), ntiles);
-    return cudaGetLastError();
+    // programmatic stream serialization: the kernel may start while its predecessor drains; it orders itself with
+    // griddepcontrol.wait (pipe_run) before touching anything the predecessor wrote
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = smem_of<K>();
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_pipe<K>, *static_cast<const P *>(pp), ntiles);
 }
 
 constexpr int kTilesPerPlane = C::N / C::W;                     // every chained stage: N / W tiles per x-plane
