@@ -373,7 +373,11 @@ struct PsiK {
     static_assert(!RHO || AX == AX_X, "the density sweep runs along x");
     static constexpr size_t TILE_BYTES = align128(L::ELEMS * sizeof(cx<T>));
     static constexpr int AUX = DRIFT ? AUX_PHASE : AUX_NONE;
-    struct Pre { T th[KICK ? ITER : 1][KICK ? RA : 1]; };
+    // Potential values prefetched across tiles (into registers, during the previous tile's last stage): those of
+    // the thread's FIRST level-A butterfly only.  The rest are loaded at the top of the tile's first phase and
+    // arrive while the first butterfly computes -- half the registers held through the radix-32 middle level.
+    static constexpr int PF = 1;
+    struct Pre { T th[KICK ? PF : 1][KICK ? RA : 1]; };
     static constexpr bool PAIR = ax_strided(AX) && pair_ok<C>();
     // the density sweep is short of registers at the end of its last psi stage (two lines of outputs, their
     // |psi|^2 and the twiddles): it fetches the twiddles where it needs them instead of keeping them
@@ -389,7 +393,7 @@ struct PsiK {
     {
         if constexpr (KICK) {
             const TL tile(p, t);
-            static_for<0, ITER>([&](auto it_) {
+            static_for<0, (PF < ITER ? PF : ITER)>([&](auto it_) {
                 constexpr int it = decltype(it_)::value;
                 int q, l;
                 split<AX, mA, W>(gt + it * NTG, q, l);
@@ -425,12 +429,27 @@ struct PsiK {
                 fwd_level_pair<RA, T>(pq, mA, w, [&](int row, cx<T> &a, cx<T> &c) { ld2(S + L::idx(row, pl), a, c); },
                                       [&](int row, cx<T> a, cx<T> c) { st2(S + L::idx(row, pl), a, c); });
             } else {
+                T late[(KICK != 0 && ITER > PF) ? ITER - PF : 1][KICK != 0 ? RA : 1];
+                if constexpr (KICK != 0)
+                    static_for<PF, ITER>([&](auto it_) {
+                        constexpr int it = decltype(it_)::value;
+                        int q, l;
+                        split<AX, mA, W>(gt + it * NTG, q, l);
+                        const T *gp = p.phi + tile.at(q, l);
+                        static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; late[it - PF][r] = ldg(gp + (long long)(mA * r) * TL::RSTRIDE); });
+                    });
                 static_for<0, ITER>([&](auto it_) {
                     constexpr int it = decltype(it_)::value;
                     int q, l;
                     split<AX, mA, W>(gt + it * NTG, q, l);
                     cx<T> v[RA];
                     static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = S[L::idx(q + mA * r, l)]; });
+                    auto th = [&](auto r_) -> T {
+                        constexpr int r = decltype(r_)::value;
+                        if constexpr (KICK == 0) return (T)0;
+                        else if constexpr (it < PF) return pre.th[it][r];
+                        else return late[it - PF][r];
+                    };
                     if constexpr (KICK != 0) {
                         if constexpr (KICK == 2) {
                             // self-interaction and / or absorbing layer: the pencil of line l is (x, y) = divmod(t W + l, N)
@@ -442,10 +461,10 @@ struct PsiK {
                             static_for<0, RA>([&](auto r_) {
                                 constexpr int r = decltype(r_)::value;
                                 const T m = p.mask ? mxy * ldg(p.mask + 2 * N + q + mA * r) : (T)1;
-                                v[r] = kick_general(v[r], pre.th[it][r], m, p.kick, p.kself_d, p.kself_a);
+                                v[r] = kick_general(v[r], th(r_), m, p.kick, p.kself_d, p.kself_a);
                             });
                         } else {
-                            static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], pre.th[it][r] * p.kick); });
+                            static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], th(r_) * p.kick); });
                         }
                     }
                     fwd_level_regs<RA, T>(v, q, mA, tb.twA + q, [&](int row, cx<T> y) { S[L::idx(row, l)] = y; });
