@@ -38,6 +38,7 @@ def lib():
             "wdmo_fft3": [i, dp, dp, i], "wdmo_dft3_direct": [i, dp, dp, i],
             "wdmo_poisson": [i, d, d, dp, dp],
             "wdmo_cic_deposit": [i, d, ll, dp, dp, dp], "wdmo_cic_gather": [i, d, dp, ll, dp, dp],
+            "wdmo_tsc_deposit": [i, d, ll, dp, dp, dp], "wdmo_tsc_gather": [i, d, dp, ll, dp, dp], "wdmo_set_assignment": [vp, i],
             "wdmo_create": [C.POINTER(vp), i, d, d, d], "wdmo_destroy": [vp],
             "wdmo_set_psi": [vp, dp], "wdmo_set_particles": [vp, ll, dp, dp, dp, d],
             "wdmo_step": [vp, i, d], "wdmo_get_psi": [vp, dp], "wdmo_get_density": [vp, dp],
@@ -116,6 +117,20 @@ def cic_gather(phi, L, pos):
     return acc
 
 
+def tsc_deposit(N, L, pos, mass):
+    """Triangular-shaped-cloud deposit (27 nodes; reading G30)."""
+    pos = _f64(pos); mass = _f64(np.broadcast_to(mass, (pos.shape[0],)))
+    rho = np.zeros((N, N, N))
+    _check(lib().wdmo_tsc_deposit(N, L, pos.shape[0], _dp(pos), _dp(mass), _dp(rho)), "tsc_deposit")
+    return rho
+
+
+def tsc_gather(phi, L, pos):
+    phi = _f64(phi); pos = _f64(pos); acc = np.empty_like(pos)
+    _check(lib().wdmo_tsc_gather(phi.shape[0], L, _dp(phi), pos.shape[0], _dp(pos), _dp(acc)), "tsc_gather")
+    return acc
+
+
 class Oracle:
     """Same call sequence as the product's Sim (wdm_create / set / step / get), float64 on the host."""
 
@@ -179,6 +194,10 @@ class Oracle:
     def set_particle_mode(self, substeps=1, static=False):
         """Leapfrog sub-steps per SPE step; static: particles only source the potential."""
         _check(lib().wdmo_set_particle_mode(self._h, int(substeps), 1 if static else 0), "set_particle_mode")
+
+    def set_assignment(self, order=2):
+        """2 = cloud-in-cell (G12-G13), 3 = triangular-shaped cloud (G30), for deposit and gather alike."""
+        _check(lib().wdmo_set_assignment(self._h, int(order)), "set_assignment")
 
     def diagnostics(self):
         """dict(M, max_rho, max_phi, V, K, Q, dt_max) of the current state (Sect. 3.5-3.6; central differences)."""

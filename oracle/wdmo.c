@@ -25,6 +25,8 @@
  * Pins (tests/test_oracle_pins.py): P1 norm, P2 free Gaussian closed form, P3 plane wave,
  * P4 single-mode Poisson, P5 direct DFT, P6 O(dt^2) energy error, P7 time reversal, P8 CIC
  * momentum / mass / zero self force, P9 gather in a known field, P10 numpy.fft cross-check.
+ * P16 triangular-shaped cloud: hand-computed weights, mass / centre / second moment, exact gradient of a
+ * quadratic-free (single-mode) field, momentum conservation.
  * The coupled psi+particle trajectory over many steps has no closed form: "parity unpinned"
  * beyond P1, P7, P8 and second-order self-convergence.
  *
@@ -61,6 +63,7 @@ typedef struct wdmo_ctx {
     /* particle variants (reading G29) */
     int nsub;            /* leapfrog sub-steps per SPE step (>= 1)                              */
     int pstatic;         /* :particles_static -- particles never move, they only source Phi    */
+    int order;           /* mass assignment / force interpolation: 2 = cloud-in-cell, 3 = TSC   */
 } wdmo_ctx;
 
 static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
@@ -309,6 +312,92 @@ int wdmo_cic_gather(int N, double L, const double *phi, long long np, const doub
     return WDMO_OK;
 }
 
+/* ---------------------------------------------------------------- triangular-shaped cloud (reading G30)
+ *
+ * Second-order assignment (Hockney & Eastwood, "Computer Simulation Using Particles", sec. 5-2-4): with
+ * u = (x + L/2)/dx, j = floor(u + 1/2) the NEAREST node and d = u - j in [-1/2, 1/2), the particle's mass goes
+ * to the three nodes j-1, j, j+1 per axis with weights
+ *      w(-1) = (1/2 - d)^2 / 2,    w(0) = 3/4 - d^2,    w(+1) = (1/2 + d)^2 / 2
+ * (the overlap of a triangle of base 2 dx centred on the particle with each node's cell); 27 nodes in 3-D, the
+ * weight the product over axes.  The gather uses the same weights on the same central-difference gradient as G13. */
+
+static void tsc_weights(double x, double L, double dx, long long *j, double w[3])
+{
+    double u = (x + 0.5 * L) / dx;
+    double fl = floor(u + 0.5);
+    double d = u - fl;
+    *j = (long long)fl;
+    w[0] = 0.5 * (0.5 - d) * (0.5 - d);
+    w[1] = 0.75 - d * d;
+    w[2] = 0.5 * (0.5 + d) * (0.5 + d);
+}
+
+static void tsc_deposit(double *rho, int N, double L, long long np, const double *pos, const double *mass)
+{
+    double dx = L / N, inv_vol = 1.0 / (dx * dx * dx);
+    for (long long p = 0; p < np; ++p) {
+        long long j[3]; double w[3][3];
+        for (int a = 0; a < 3; ++a) tsc_weights(pos[3 * p + a], L, dx, &j[a], w[a]);
+        for (int ox = -1; ox <= 1; ++ox)
+            for (int oy = -1; oy <= 1; ++oy)
+                for (int oz = -1; oz <= 1; ++oz) {
+                    size_t idx = ((size_t)wrap_index(j[0] + ox, N) * N + wrap_index(j[1] + oy, N)) * N
+                                 + wrap_index(j[2] + oz, N);
+                    rho[idx] += mass[p] * w[0][ox + 1] * w[1][oy + 1] * w[2][oz + 1] * inv_vol;
+                }
+    }
+}
+
+static void tsc_gather(const double *phi, int N, double L, long long np, const double *pos, double *acc)
+{
+    double dx = L / N;
+#pragma omp parallel for schedule(static)
+    for (long long p = 0; p < np; ++p) {
+        long long j[3]; double w[3][3];
+        for (int a = 0; a < 3; ++a) tsc_weights(pos[3 * p + a], L, dx, &j[a], w[a]);
+        double ax = 0.0, ay = 0.0, az = 0.0;
+        for (int ox = -1; ox <= 1; ++ox)
+            for (int oy = -1; oy <= 1; ++oy)
+                for (int oz = -1; oz <= 1; ++oz) {
+                    double wt = w[0][ox + 1] * w[1][oy + 1] * w[2][oz + 1];
+                    long long ix = j[0] + ox, iy = j[1] + oy, iz = j[2] + oz;
+#define PHI(a, b, c_) phi[((size_t)wrap_index((a), N) * N + wrap_index((b), N)) * N + wrap_index((c_), N)]
+                    ax += wt * -(PHI(ix + 1, iy, iz) - PHI(ix - 1, iy, iz)) / (2.0 * dx);
+                    ay += wt * -(PHI(ix, iy + 1, iz) - PHI(ix, iy - 1, iz)) / (2.0 * dx);
+                    az += wt * -(PHI(ix, iy, iz + 1) - PHI(ix, iy, iz - 1)) / (2.0 * dx);
+#undef PHI
+                }
+        acc[3 * p] = ax; acc[3 * p + 1] = ay; acc[3 * p + 2] = az;
+    }
+}
+
+int wdmo_tsc_deposit(int N, double L, long long np, const double *pos, const double *mass, double *rho)
+{
+    if (N < 1 || L <= 0 || np < 0 || !rho || (np > 0 && (!pos || !mass))) return WDMO_EINVAL;
+    tsc_deposit(rho, N, L, np, pos, mass);
+    return WDMO_OK;
+}
+
+int wdmo_tsc_gather(int N, double L, const double *phi, long long np, const double *pos, double *acc)
+{
+    if (N < 1 || L <= 0 || np < 0 || !phi || (np > 0 && (!pos || !acc))) return WDMO_EINVAL;
+    tsc_gather(phi, N, L, np, pos, acc);
+    return WDMO_OK;
+}
+
+/* the context's scheme */
+static void assign_deposit(const wdmo_ctx *c, double *rho)
+{
+    if (c->order == 3) tsc_deposit(rho, c->N, c->L, c->np, c->pos, c->mass);
+    else cic_deposit(rho, c->N, c->L, c->np, c->pos, c->mass);
+}
+
+static void assign_gather(wdmo_ctx *c)
+{
+    if (c->order == 3) tsc_gather(c->phi, c->N, c->L, c->np, c->pos, c->acc);
+    else cic_gather(c->phi, c->N, c->L, c->np, c->pos, c->acc);
+}
+
 /* ---------------------------------------------------------------- context */
 
 int wdmo_create(wdmo_ctx **out, int N, double L, double hbar_over_m, double G)
@@ -321,6 +410,7 @@ int wdmo_create(wdmo_ctx **out, int N, double L, double hbar_over_m, double G)
     if (!c) return WDMO_ENOMEM;
     c->N = N; c->L = L; c->mu = hbar_over_m; c->G = G; c->dx = L / N;
     c->nsub = 1;
+    c->order = 2;
     c->n = (size_t)N * N * N;
     c->psi = (cplx *)malloc(sizeof(cplx) * c->n);
     c->work = (cplx *)malloc(sizeof(cplx) * c->n);
@@ -389,13 +479,13 @@ static int update_potential(wdmo_ctx *c)
         double re = creal(c->psi[i]), im = cimag(c->psi[i]);
         c->rho[i] = re * re + im * im;
     }
-    if (c->np > 0) cic_deposit(c->rho, c->N, c->L, c->np, c->pos, c->mass);
+    if (c->np > 0) assign_deposit(c, c->rho);
     int rc = poisson(c->rho, c->phi, c->work, c->N, c->L, c->G);
     if (rc) return rc;
     /* Phi_total = Phi_DM + Phi_ext (Alg. 1 l.15); particles feel the total as well (G27) */
     if (c->phi_ext)
         for (size_t i = 0; i < c->n; ++i) c->phi[i] += c->phi_ext[i];
-    if (c->np > 0) cic_gather(c->phi, c->N, c->L, c->np, c->pos, c->acc);
+    if (c->np > 0) assign_gather(c);
     return WDMO_OK;
 }
 
@@ -452,7 +542,7 @@ static int drift(wdmo_ctx *c, double dt)
         for (int j = 1; j <= c->nsub; ++j) {
             for (long long i = 0; i < 3 * c->np; ++i) c->pos[i] = wrap_pos(c->pos[i] + c->vel[i] * h, c->L);
             if (j < c->nsub) {
-                cic_gather(c->phi, c->N, c->L, c->np, c->pos, c->acc);
+                assign_gather(c);
                 for (long long i = 0; i < 3 * c->np; ++i) c->vel[i] += c->acc[i] * h;
             }
         }
@@ -478,6 +568,15 @@ static void absorb(wdmo_ctx *c, double dt)
                 double b = absorb_profile(x, c->L, c->nb) + absorb_profile(y, c->L, c->nb) + absorb_profile(z, c->L, c->nb);
                 c->psi[((size_t)ix * N + iy) * N + iz] *= exp(-c->alpha * b * dt);
             }
+}
+
+/* order 2: cloud-in-cell (G12, G13); order 3: triangular-shaped cloud (G30).  The potential becomes stale. */
+int wdmo_set_assignment(wdmo_ctx *c, int order)
+{
+    if (!c || (order != 2 && order != 3)) return WDMO_EINVAL;
+    c->order = order;
+    c->stale = 1;
+    return WDMO_OK;
 }
 
 /* nsub >= 1 leapfrog sub-steps per SPE step; pstatic != 0: particles are a fixed mass distribution */

@@ -524,3 +524,89 @@ def test_p15_static_particles_only_source_the_potential():
     # total mass in the source: sum rho dx^3 = M_psi + sum m_p
     dx3 = (w.L / w.N) ** 3
     assert abs(o.density().sum() * dx3 - (np.sum(np.abs(o.psi()) ** 2) * dx3 + np.sum(np.broadcast_to(w.mass, (len(w.pos),))))) < 1e-10
+
+
+# ---------------------------------------------------------------- P16: triangular-shaped cloud (reading G30)
+
+def test_p16_tsc_hand_computed_weights():
+    N, L = 8, 2.0
+    dx = L / N
+    # on a node: (1/8, 3/4, 1/8) per axis, across the periodic face for node 0
+    rho = oracle.tsc_deposit(N, L, np.array([[-L / 2 + 3 * dx, -L / 2, -L / 2 + 7 * dx]]), 1.0) * dx ** 3
+    assert rho[3, 0, 7] == pytest.approx(0.75 ** 3) and rho[2, 7, 6] == pytest.approx(0.125 ** 3)
+    assert rho[4, 1, 0] == pytest.approx(0.125 ** 3) and rho[3, 7, 0] == pytest.approx(0.75 * 0.125 ** 2)
+    assert np.count_nonzero(rho) == 27 and rho.sum() == pytest.approx(1.0, rel=1e-14)
+    # a quarter cell past node 5 along x (d = 1/4): 1/32, 11/16, 9/32; on nodes along y and z
+    rho = oracle.tsc_deposit(N, L, np.array([[-L / 2 + 5.25 * dx, -L / 2 + 2 * dx, -L / 2 + 2 * dx]]), 1.0) * dx ** 3
+    line = rho[:, 2, 2] / 0.75 ** 2
+    assert line[4] == pytest.approx(1 / 32) and line[5] == pytest.approx(11 / 16) and line[6] == pytest.approx(9 / 32)
+    assert np.count_nonzero(line) == 3
+    # exactly half way between nodes 5 and 6: the far node's weight vanishes, 1/2 each (the cloud is continuous there)
+    for eps in (0.0, -1e-9, 1e-9):
+        rho = oracle.tsc_deposit(N, L, np.array([[-L / 2 + (5.5 + eps) * dx, -L / 2 + 2 * dx, -L / 2 + 2 * dx]]), 1.0) * dx ** 3
+        line = rho[:, 2, 2] / 0.75 ** 2
+        assert abs(line[5] - 0.5) < 2e-9 and abs(line[6] - 0.5) < 2e-9 and abs(line[4]) < 1e-16 + 1e-17 and abs(line[7]) < 1e-16
+
+
+def test_p16_tsc_moments_mass_centre_and_constant_variance():
+    """Per axis: sum w = 1, sum w (i - u) = 0, sum w (i - u)^2 = 1/4 for every position (what defines the scheme
+    among three-point assignments)."""
+    N, L = 16, 1.0
+    dx = L / N
+    rng = np.random.default_rng(16)
+    idx = np.arange(N)
+    for x in rng.uniform(-L / 2, L / 2, size=(40, 3)):
+        rho = oracle.tsc_deposit(N, L, x[None, :], 3.0) * dx ** 3 / 3.0
+        assert rho.min() >= 0 and rho.sum() == pytest.approx(1.0, rel=1e-13)
+        for a in range(3):
+            marg = rho.sum(axis=tuple(b for b in range(3) if b != a))
+            u = (x[a] + L / 2) / dx
+            off = (idx - u + N / 2) % N - N / 2                    # minimum-image offset in cells
+            assert abs((marg * off).sum()) < 1e-12
+            assert (marg * off ** 2).sum() == pytest.approx(0.25, abs=1e-12)
+    p = rng.uniform(-L / 2, L / 2, size=(500, 3)); m = rng.uniform(0.1, 2.0, size=500)
+    assert oracle.tsc_deposit(N, L, p, m).sum() * dx ** 3 == pytest.approx(m.sum(), rel=1e-13)
+
+
+def test_p16_tsc_gather_closed_form():
+    """phi = A cos(k y): node gradient g_j = A sin(k y_j) sin(k dx)/dx; three-point interpolation with
+    w- + w+ = 1/4 + d^2 and w+ - w- = d gives sin(k y_j)[3/4 - d^2 + (1/4 + d^2) cos(k dx)] + d cos(k y_j) sin(k dx)."""
+    N, L = 16, 1.0
+    dx = L / N
+    X, Y, Z = grid(N, L)
+    kk = 2 * np.pi * 2 / L
+    A = 0.3
+    phi = A * np.cos(kk * Y)
+    rng = np.random.default_rng(17)
+    pos = rng.uniform(-0.5, 0.5, size=(64, 3))
+    acc = oracle.tsc_gather(phi, L, pos)
+    u = (pos[:, 1] + L / 2) / dx
+    j = np.floor(u + 0.5); d = u - j
+    yj = -L / 2 + dx * j
+    expect = A * np.sin(kk * dx) / dx * (np.sin(kk * yj) * (0.75 - d ** 2 + (0.25 + d ** 2) * np.cos(kk * dx))
+                                         + d * np.cos(kk * yj) * np.sin(kk * dx))
+    assert np.max(np.abs(acc[:, 1] - expect)) < 1e-13
+    assert np.max(np.abs(acc[:, 0])) < 1e-13 and np.max(np.abs(acc[:, 2])) < 1e-13
+    assert np.max(np.abs(acc - oracle.cic_gather(phi, L, pos))) > 1e-3          # and it is not the CIC value
+
+
+def test_p16_tsc_zero_self_force_momentum_and_context_switch():
+    N, L, G = 16, 1.0, 1.0
+    rng = np.random.default_rng(18)
+    o = oracle.Oracle(N, L, 1.0, G)
+    o.set_psi(np.zeros((N, N, N), complex))
+    o.set_assignment(3)
+    o.set_particles(rng.uniform(-0.5, 0.5, size=(1, 3)), np.zeros((1, 3)), 1.0)
+    assert np.max(np.abs(o.accel())) < 1e-12
+    p = rng.uniform(-0.5, 0.5, size=(200, 3)); m = rng.uniform(0.5, 1.5, size=200)
+    o.set_particles(p, np.zeros((200, 3)), m)
+    a3 = o.accel()
+    assert np.max(np.abs((m[:, None] * a3).sum(0))) < 1e-11 * np.abs(m[:, None] * a3).sum()
+    dx3 = (L / N) ** 3
+    assert np.allclose(o.density(), oracle.tsc_deposit(N, L, p, m), rtol=0, atol=1e-12 / dx3)
+    o.set_assignment(2)                                                        # back to CIC: the potential is refreshed
+    a2 = o.accel()
+    assert np.allclose(o.density(), oracle.cic_deposit(N, L, p, m), rtol=0, atol=1e-12 / dx3)
+    assert np.max(np.abs(a2 - a3)) > 1e-3 * np.max(np.abs(a2))
+    with pytest.raises(Exception):
+        o.set_assignment(4)
