@@ -112,6 +112,16 @@ int wdm_set_kick_terms(wdm_ctx *ctx, double kappa, const void *phi_ext_dev, doub
  * (":particles_static"): the particles never move; their mass stays in the Poisson source.  Default: 1, 0. */
 int wdm_set_particle_mode(wdm_ctx *ctx, int substeps, int is_static);
 
+/* Mass-assignment / force-interpolation scheme of the particles ("interpolated from the grid to particle
+ * positions", scheme not given; DESIGN reading G30).  order = 2: cloud-in-cell,
+ * 8 nodes, weights (1 - f, f) per axis (default).  order = 3: triangular-shaped cloud, 27 nodes: with j the node
+ * nearest to the particle and d in [-1/2, 1/2) its offset from it in cells, weights (1/2 - d)^2/2, 3/4 - d^2,
+ * (1/2 + d)^2/2 on nodes j-1, j, j+1 per axis.  The same weights deposit the mass into the Poisson source and gather
+ * the central-difference gradient of Eq. 21.  Any other order: WDM_EINVAL.  A change marks the
+ * potential stale (recomputed by the next step / get).  wdm_get_assignment writes the current order to *order. */
+int wdm_set_assignment(wdm_ctx *ctx, int order);
+int wdm_get_assignment(wdm_ctx *ctx, int *order);
+
 /* Diagnostics of the current state (Sect. 3.5-3.6) by one reduction pass on the device; the
  * gradients are the second-order central differences of Eq. 21.  Synchronises the stream.
  * out_host[0] M = sum |psi|^2 dx^3       [1] max |psi|^2       [2] max |Phi_total|

@@ -863,6 +863,26 @@ extern "C" int wdm_set_particle_mode(wdm_ctx *c, int substeps, int is_static)
     return WDM_OK;
 }
 
+extern "C" int wdm_set_assignment(wdm_ctx *c, int order)
+{
+    if (!c) return WDM_EINVAL;
+    if (order != 2 && order != 3) return fail(c, WDM_EINVAL, "assignment order must be 2 (cloud-in-cell) or 3 (triangular-shaped cloud)");
+    int rcf = do_flush(c, true, true);       // a pending closing half kick belongs to the scheme it was computed with
+    if (rcf) return rcf;
+    if (c->part.order != order) {
+        c->part.order = order;
+        c->stale = true;                     // the particles' share of the Poisson source changes
+    }
+    return WDM_OK;
+}
+
+extern "C" int wdm_get_assignment(wdm_ctx *c, int *order)
+{
+    if (!c || !order) return WDM_EINVAL;
+    *order = c->part.order;
+    return WDM_OK;
+}
+
 extern "C" int wdm_get_diagnostics(wdm_ctx *c, double *out_host)
 {
     if (!c) return WDM_EINVAL;

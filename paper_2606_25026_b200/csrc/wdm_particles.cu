@@ -42,6 +42,46 @@ __device__ __forceinline__ Cic<T> cic_of(const T *x, T half_L, T inv_dx, int N)
     return c;
 }
 
+// Assignment stencil of one particle: ORDER nodes per axis starting at `base` (wrapped), weights w[axis][0..ORDER).
+//   ORDER 2, cloud-in-cell (G12):        base = floor(u),           w = (1 - f, f),  f = u - floor(u)
+//   ORDER 3, triangular-shaped cloud (G30): base = floor(u + 1/2) - 1,  w = ((1/2 - d)^2 / 2, 3/4 - d^2, (1/2 + d)^2 / 2),
+//            d = u - floor(u + 1/2) in [-1/2, 1/2)
+template <typename T, int ORDER>
+struct Asg {
+    int base[3];
+    T w[3][ORDER];
+};
+
+template <typename T, int ORDER>
+__device__ __forceinline__ Asg<T, ORDER> asg_of(const T *x, T half_L, T inv_dx, int N)
+{
+    static_assert(ORDER == 2 || ORDER == 3, "cloud-in-cell or triangular-shaped cloud");
+    Asg<T, ORDER> s;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        T u = (x[a] + half_L) * inv_dx;
+        int i;
+        if constexpr (ORDER == 2) {
+            T fl = floor(u);
+            T f = u - fl;
+            i = (int)fl;
+            s.w[a][0] = (T)1 - f;
+            s.w[a][1] = f;
+        } else {
+            T fl = floor(u + (T)0.5);
+            T d = u - fl;
+            i = (int)fl - 1;
+            s.w[a][0] = (T)0.5 * ((T)0.5 - d) * ((T)0.5 - d);
+            s.w[a][1] = (T)0.75 - d * d;
+            s.w[a][2] = (T)0.5 * ((T)0.5 + d) * ((T)0.5 + d);
+        }
+        i %= N;
+        if (i < 0) i += N;
+        s.base[a] = i;
+    }
+    return s;
+}
+
 __device__ __forceinline__ int tile_key(const int *i0, int N)
 {
     int nt = ntiles1(N);
@@ -131,30 +171,30 @@ __global__ void k_scatter(const T *pos, const T *vel, const T *mass, const int *
     orig2[d] = orig[i];
 }
 
-// a = sum_corners w * (phi[node+e] - phi[node-e]) per axis (the caller scales by -1/(2 dx)): CIC gather of the
-// central-difference gradient (Eq. 21) with the deposit's weights (G13)
-template <typename T>
+// a = sum_nodes w * (phi[node+e] - phi[node-e]) per axis (the caller scales by -1/(2 dx)): gather of the
+// central-difference gradient (Eq. 21) with the deposit's weights (G13, G30)
+template <typename T, int ORDER>
 __device__ __forceinline__ void gather_grad(const T *__restrict__ phi, const T (&x)[3], int N, T L, T (&a)[3])
 {
     const T inv_dx = (T)N / L;
-    Cic<T> c = cic_of<T>(x, (T)0.5 * L, inv_dx, N);
+    Asg<T, ORDER> c = asg_of<T, ORDER>(x, (T)0.5 * L, inv_dx, N);
     const int M = N - 1;
-    // indices i0-1 .. i0+2 along each axis
-    int ix[4], iy[4], iz[4];
+    // indices base-1 .. base+ORDER along each axis
+    int ix[ORDER + 2], iy[ORDER + 2], iz[ORDER + 2];
 #pragma unroll
-    for (int d = 0; d < 4; ++d) {
-        ix[d] = (c.i0[0] + d - 1) & M;
-        iy[d] = (c.i0[1] + d - 1) & M;
-        iz[d] = (c.i0[2] + d - 1) & M;
+    for (int d = 0; d < ORDER + 2; ++d) {
+        ix[d] = (c.base[0] + d - 1) & M;
+        iy[d] = (c.base[1] + d - 1) & M;
+        iz[d] = (c.base[2] + d - 1) & M;
     }
     a[0] = a[1] = a[2] = (T)0;
 #pragma unroll
-    for (int bx = 0; bx < 2; ++bx)
+    for (int bx = 0; bx < ORDER; ++bx)
 #pragma unroll
-        for (int by = 0; by < 2; ++by)
+        for (int by = 0; by < ORDER; ++by)
 #pragma unroll
-            for (int bz = 0; bz < 2; ++bz) {
-                T w = (bx ? c.f[0] : (T)1 - c.f[0]) * (by ? c.f[1] : (T)1 - c.f[1]) * (bz ? c.f[2] : (T)1 - c.f[2]);
+            for (int bz = 0; bz < ORDER; ++bz) {
+                T w = c.w[0][bx] * c.w[1][by] * c.w[2][bz];
                 size_t X = ix[bx + 1], Y = iy[by + 1], Z = iz[bz + 1];
                 T gx = __ldg(phi + ((size_t)ix[bx + 2] * N + Y) * N + Z) - __ldg(phi + ((size_t)ix[bx] * N + Y) * N + Z);
                 T gy = __ldg(phi + (X * N + iy[by + 2]) * N + Z) - __ldg(phi + (X * N + iy[by]) * N + Z);
@@ -165,7 +205,7 @@ __device__ __forceinline__ void gather_grad(const T *__restrict__ phi, const T (
 
 // v += a(x) kick_dt ; then nsub drifts of drift_dt / nsub, wrapped, with a full kick of that size (gathered at the
 // new position, in the same potential) between two drifts (several N-body sub-steps per SPE step)
-template <typename T>
+template <typename T, int ORDER>
 __global__ void k_push(T *pos, T *vel, const T *__restrict__ phi, long long n, int N, T L, T kick_dt, T drift_dt, int nsub)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -176,7 +216,7 @@ __global__ void k_push(T *pos, T *vel, const T *__restrict__ phi, long long n, i
     bool kicked = false;
     if (kick_dt != (T)0) {
         T a[3];
-        gather_grad<T>(phi, x, N, L, a);
+        gather_grad<T, ORDER>(phi, x, N, L, a);
 #pragma unroll
         for (int d = 0; d < 3; ++d) v[d] += a[d] * (g * kick_dt);
         kicked = true;
@@ -188,7 +228,7 @@ __global__ void k_push(T *pos, T *vel, const T *__restrict__ phi, long long n, i
             for (int d = 0; d < 3; ++d) x[d] = wrap_pos(x[d] + v[d] * h, L);
             if (j < nsub) {
                 T a[3];
-                gather_grad<T>(phi, x, N, L, a);
+                gather_grad<T, ORDER>(phi, x, N, L, a);
 #pragma unroll
                 for (int d = 0; d < 3; ++d) v[d] += a[d] * (g * h);
                 kicked = true;
@@ -203,13 +243,15 @@ __global__ void k_push(T *pos, T *vel, const T *__restrict__ phi, long long n, i
     }
 }
 
-// CIC deposit: each CTA takes CHUNK consecutive (tile-sorted) particles and accumulates into a BOX^3-node
-// shared-memory box anchored at the tile of its first particle; nodes outside the box go straight to
-// global memory.  Equal cells inside a warp are combined first (warp-aggregated atomics).
-template <typename T>
+// Deposit: each CTA takes CHUNK consecutive (tile-sorted) particles and accumulates into a BOX^3-node
+// shared-memory box anchored at the tile of its first particle (one node lower for the three-point cloud, whose
+// stencil starts one node below the nearest node); nodes outside the box go straight to global memory.
+// Particles of a warp with the same stencil are combined first (warp-aggregated atomics).
+template <typename T, int ORDER>
 __global__ void __launch_bounds__(256) k_deposit(const T *__restrict__ pos, const T *__restrict__ mass, T mass_scalar,
                                                  T *rho, long long n, int N, T L)
 {
+    constexpr int NW = ORDER * ORDER * ORDER;
     __shared__ T box[BOX * BOX * BOX];
     __shared__ int org[3];
     const long long start = (long long)blockIdx.x * CHUNK;
@@ -220,36 +262,36 @@ __global__ void __launch_bounds__(256) k_deposit(const T *__restrict__ pos, cons
         T x[3] = {pos[3 * start], pos[3 * start + 1], pos[3 * start + 2]};
         Cic<T> c = cic_of<T>(x, half_L, inv_dx, N);
 #pragma unroll
-        for (int a = 0; a < 3; ++a) org[a] = (c.i0[a] / TS) * TS;
+        for (int a = 0; a < 3; ++a) org[a] = (c.i0[a] / TS) * TS - (ORDER - 2);
     }
     __syncthreads();
     const int M = N - 1;
     for (long long base = start; base < end; base += blockDim.x) {
         long long i = base + threadIdx.x;
         bool active = i < end;
-        Cic<T> c;
+        Asg<T, ORDER> c;
         T m = (T)0;
         int cell = -1;
         if (active) {
             T x[3] = {pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
-            c = cic_of<T>(x, half_L, inv_dx, N);
+            c = asg_of<T, ORDER>(x, half_L, inv_dx, N);
             m = (mass ? mass[i] : mass_scalar) * inv_vol;
-            cell = (c.i0[0] * N + c.i0[1]) * N + c.i0[2];
+            cell = (c.base[0] * N + c.base[1]) * N + c.base[2];
         }
-        // combine the lanes that sit in the same cell: the group leader deposits the summed weights
+        // combine the lanes whose stencils coincide: the group leader deposits the summed weights
         unsigned peers = __match_any_sync(0xffffffffu, cell);
         int leader = __ffs(peers) - 1;
         int lane = threadIdx.x & 31;
-        T w[8];
+        T w[NW];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            int bx = (q >> 2) & 1, by = (q >> 1) & 1, bz = q & 1;
-            w[q] = active ? m * (bx ? c.f[0] : (T)1 - c.f[0]) * (by ? c.f[1] : (T)1 - c.f[1]) * (bz ? c.f[2] : (T)1 - c.f[2]) : (T)0;
+        for (int q = 0; q < NW; ++q) {
+            int bx = q / (ORDER * ORDER), by = (q / ORDER) % ORDER, bz = q % ORDER;
+            w[q] = active ? m * c.w[0][bx] * c.w[1][by] * c.w[2][bz] : (T)0;
         }
         if (peers != (1u << lane)) {
             // tree-free reduction inside each peer group: walk the group mask
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
+            for (int q = 0; q < NW; ++q) {
                 T acc = (T)0;
                 unsigned rem = peers;
                 while (rem) {
@@ -261,13 +303,13 @@ __global__ void __launch_bounds__(256) k_deposit(const T *__restrict__ pos, cons
             }
         }
         if (active && lane == leader) {
-            int rx = (c.i0[0] - org[0]) & M, ry = (c.i0[1] - org[1]) & M, rz = (c.i0[2] - org[2]) & M;
-            bool inside = rx < BOX - 1 && ry < BOX - 1 && rz < BOX - 1;
+            int rx = (c.base[0] - org[0]) & M, ry = (c.base[1] - org[1]) & M, rz = (c.base[2] - org[2]) & M;
+            bool inside = rx <= BOX - ORDER && ry <= BOX - ORDER && rz <= BOX - ORDER;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                int bx = (q >> 2) & 1, by = (q >> 1) & 1, bz = q & 1;
+            for (int q = 0; q < NW; ++q) {
+                int bx = q / (ORDER * ORDER), by = (q / ORDER) % ORDER, bz = q % ORDER;
                 if (inside) atomicAdd(&box[((rx + bx) * BOX + ry + by) * BOX + rz + bz], w[q]);
-                else atomicAdd(rho + ((size_t)((c.i0[0] + bx) & M) * N + ((c.i0[1] + by) & M)) * N + ((c.i0[2] + bz) & M), w[q]);
+                else atomicAdd(rho + ((size_t)((c.base[0] + bx) & M) * N + ((c.base[1] + by) & M)) * N + ((c.base[2] + bz) & M), w[q]);
             }
         }
     }
@@ -371,8 +413,11 @@ cudaError_t particle_push(ParticleState &ps, int N, double L, int dtype, const v
 {
     if (ps.n == 0) return cudaSuccess;
     if (nsub < 1) nsub = 1;
-    if (dtype == 0) k_push<float><<<blocks(ps.n, 128), 128, 0, s>>>((float *)ps.pos, (float *)ps.vel, (const float *)phi, ps.n, N, (float)L, (float)kick_dt, (float)drift_dt, nsub);
-    else k_push<double><<<blocks(ps.n, 128), 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt, nsub);
+    const unsigned g = blocks(ps.n, 128);
+    if (dtype == 0 && ps.order == 2) k_push<float, 2><<<g, 128, 0, s>>>((float *)ps.pos, (float *)ps.vel, (const float *)phi, ps.n, N, (float)L, (float)kick_dt, (float)drift_dt, nsub);
+    else if (dtype == 0) k_push<float, 3><<<g, 128, 0, s>>>((float *)ps.pos, (float *)ps.vel, (const float *)phi, ps.n, N, (float)L, (float)kick_dt, (float)drift_dt, nsub);
+    else if (ps.order == 2) k_push<double, 2><<<g, 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt, nsub);
+    else k_push<double, 3><<<g, 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt, nsub);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (drift_dt != 0.0 && ++ps.steps_since_sort >= kResortInterval)
@@ -384,8 +429,12 @@ cudaError_t particle_deposit(ParticleState &ps, int N, double L, int dtype, cuda
 {
     if (ps.n == 0) return cudaSuccess;
     unsigned g = blocks(ps.n, CHUNK);
-    if (dtype == 0) k_deposit<float><<<g, 256, 0, s>>>((const float *)ps.pos, ps.has_mass ? (const float *)ps.mass : nullptr, (float)ps.mass_scalar, (float *)ps.rho_p, ps.n, N, (float)L);
-    else k_deposit<double><<<g, 256, 0, s>>>((const double *)ps.pos, ps.has_mass ? (const double *)ps.mass : nullptr, ps.mass_scalar, (double *)ps.rho_p, ps.n, N, L);
+    const float *mf = ps.has_mass ? (const float *)ps.mass : nullptr;
+    const double *md = ps.has_mass ? (const double *)ps.mass : nullptr;
+    if (dtype == 0 && ps.order == 2) k_deposit<float, 2><<<g, 256, 0, s>>>((const float *)ps.pos, mf, (float)ps.mass_scalar, (float *)ps.rho_p, ps.n, N, (float)L);
+    else if (dtype == 0) k_deposit<float, 3><<<g, 256, 0, s>>>((const float *)ps.pos, mf, (float)ps.mass_scalar, (float *)ps.rho_p, ps.n, N, (float)L);
+    else if (ps.order == 2) k_deposit<double, 2><<<g, 256, 0, s>>>((const double *)ps.pos, md, ps.mass_scalar, (double *)ps.rho_p, ps.n, N, L);
+    else k_deposit<double, 3><<<g, 256, 0, s>>>((const double *)ps.pos, md, ps.mass_scalar, (double *)ps.rho_p, ps.n, N, L);
     return cudaGetLastError();
 }
 

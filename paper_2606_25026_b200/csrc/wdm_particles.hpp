@@ -19,6 +19,7 @@ struct ParticleState {
     bool has_mass = false;
     double mass_scalar = 0.0;
     int steps_since_sort = 0;
+    int order = 2;                           // 2: cloud-in-cell (G12-G13), 3: triangular-shaped cloud (G30)
 };
 
 size_t particle_bytes(int N, int dtype, long long capacity);
@@ -29,7 +30,7 @@ cudaError_t particle_set(ParticleState &ps, int N, double L, int dtype, long lon
 // size, gathered at the new position, between two drifts
 cudaError_t particle_push(ParticleState &ps, int N, double L, int dtype, const void *phi, double kick_dt,
                           double drift_dt, int nsub, cudaStream_t s);
-// rho_p += CIC(x) (the caller zeroes rho_p)
+// rho_p += deposit of the particles' mass with the scheme ps.order (the caller zeroes rho_p)
 cudaError_t particle_deposit(ParticleState &ps, int N, double L, int dtype, cudaStream_t s);
 cudaError_t particle_get(ParticleState &ps, int dtype, void *pos_out, void *vel_out, bool to_host, cudaStream_t s);
 

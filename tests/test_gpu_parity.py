@@ -501,6 +501,69 @@ def test_particle_modes_match_oracle(wdm, dtype, mode):
     sim.close()
 
 
+# ---------------------------------------------------------------- triangular-shaped cloud (G30)
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_tsc_assignment_matches_oracle(wdm, dtype):
+    """27-node deposit and gather: density, potential, psi and the particle trajectory against the oracle's TSC,
+    every element; then back to cloud-in-cell in the same context."""
+    w = wl.small_coupled(32, dtype=dtype, n_particles=2000)
+    rng = np.random.default_rng(31)
+    m = w.mass * rng.uniform(0.2, 3.0, size=len(w.pos))
+    sim = wdm.Sim(w.N, w.L, w.hbar_over_m, w.G, dtype, max_particles=len(w.pos))
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    sim.set_psi(w.psi); o.set_psi(w.psi)
+    sim.set_particles(w.pos, w.vel, m); o.set_particles(w.pos, w.vel, m)
+    assert sim.assignment() == 2
+    sim.set_assignment(3); o.set_assignment(3)
+    assert sim.assignment() == 3
+    check_fields(sim, o, dtype, 0, "tsc initial")
+    # the particles' share of the source, on its own: the library's density minus |psi|^2 against the oracle's deposit
+    dep = sim.density().cpu().numpy().astype(np.float64) - np.abs(w.psi.astype(np.complex128)) ** 2
+    ref = oracle.tsc_deposit(w.N, w.L, w.pos, m)
+    assert np.abs(dep - ref).max() <= (2e-5 if dtype == "c64" else 1e-12) * max(np.abs(ref).max(), o.density().max())
+    sim.step(3, w.dt); o.step(3, w.dt)
+    sim.step(2, w.dt); o.step(2, w.dt)
+    check_fields(sim, o, dtype, 5, "tsc")
+    check_particles(sim, o, w.L, 5, dtype)
+    sim.set_assignment(2); o.set_assignment(2)             # flushes the pending half kick, marks the potential stale
+    check_fields(sim, o, dtype, 5, "back to cic")
+    sim.step(2, w.dt); o.step(2, w.dt)
+    check_fields(sim, o, dtype, 7, "cic after tsc")
+    check_particles(sim, o, w.L, 7, dtype)
+    with pytest.raises(Exception):
+        sim.set_assignment(4)
+    sim.close()
+
+
+def test_tsc_differs_from_cic_and_conserves_mass(wdm):
+    w = wl.small_coupled(32, dtype="c128", n_particles=500)
+    sim, o = pair(wdm, w, len(w.pos))
+    rho2 = sim.density().cpu().numpy()
+    sim.set_assignment(3)
+    rho3 = sim.density().cpu().numpy()
+    dx3 = (w.L / w.N) ** 3
+    assert abs(rho2.sum() - rho3.sum()) * dx3 < 1e-12 * rho2.sum() * dx3          # the same mass, spread differently
+    assert np.abs(rho2 - rho3).max() > 1e-3 * np.abs(rho2).max()
+    sim.close()
+
+
+def test_tsc_thin_disc_substeps(wdm):
+    """Config-5 disc at reduced size under TSC with two sub-steps: contention in the shared-memory box (one node
+    lower than the tile), warp-combined stencils, and the sort."""
+    w = wl.config5(N=64, n_particles=1 << 14, nsteps=6)
+    sim, o = pair(wdm, w, len(w.pos))
+    for x in (sim, o):
+        x.set_assignment(3)
+        x.set_particle_mode(substeps=2)
+    sim.step(0, 0.0); o.step(0, 0.0)
+    dt = wl.cfl_dt(w, float(np.abs(o.potential()).max())) if w.dt is None else w.dt
+    sim.step(6, dt); o.step(6, dt)
+    check_fields(sim, o, "c64", 6, "tsc disc")
+    check_particles(sim, o, w.L, 6, "c64")
+    sim.close()
+
+
 # ---------------------------------------------------------------- closing kicks deferred across wdm_step calls
 
 @pytest.mark.parametrize("dtype", ["c128", "c64"])
