@@ -300,10 +300,10 @@ def main():
 
         # ---- CPU oracle on the host cores, bounded sample (rank 0, N = 1 only)
         if rank == 0 and world == 1 and not args.no_cpu_baseline:
-            n_ref = 256
-            ws, rate, el, thr = oracle_rate(f"sample{n_ref}", 8, 1)
+            n_ref, CPU_STEPS = 256, 40         # about 13 s on 16 host cores (bounded sample: 10-30 s of CPU work)
+            ws, rate, el, thr = oracle_rate(f"sample{n_ref}", CPU_STEPS, 1)
             out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": thr, "kind": "oracle",
-                                   "sample": f"float64 CPU oracle, soliton+halo at {n_ref}^3, 8 timed KDK steps ({el:.1f} s)"}
+                                   "sample": f"float64 CPU oracle, soliton+halo at {n_ref}^3, {CPU_STEPS} timed KDK steps ({el:.1f} s)"}
     sim.close()
     if rank == 0:
         print(json.dumps(out))

@@ -78,6 +78,35 @@ WDM_DEV cx<double> rotate_neg(cx<double> v, double th)
     sincos(th, &s, &c);
     return mk<double>(v.x * c + v.y * s, v.y * c - v.x * s);
 }
+// R elements at once (the level-A butterfly of one thread).  Single precision: ONE test on the largest phase of the
+// butterfly instead of one per element -- the common path (every phase small) is straight-line code.
+template <int R>
+WDM_DEV void rotate_neg_all(cx<float> (&v)[R], const float (&th)[R])
+{
+    float mx = 0.0f;
+#pragma unroll
+    for (int r = 0; r < R; ++r) mx = fmaxf(mx, fabsf(th[r]));
+    if (mx < 0.25f) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            float s, c;
+            sincos_small(th[r], s, c);
+            v[r] = mk<float>(v[r].x * c + v[r].y * s, v[r].y * c - v[r].x * s);
+        }
+    } else {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            float2 sc = sincos_large(th[r]);
+            v[r] = mk<float>(v[r].x * sc.y + v[r].y * sc.x, v[r].y * sc.y - v[r].x * sc.x);
+        }
+    }
+}
+template <int R>
+WDM_DEV void rotate_neg_all(cx<double> (&v)[R], const double (&th)[R])
+{
+#pragma unroll
+    for (int r = 0; r < R; ++r) v[r] = rotate_neg(v[r], th[r]);
+}
 // the general kick of one element (see SweepParams::kick_extra); m = product of the three axis factors or 1
 template <typename T>
 WDM_DEV cx<T> kick_general(cx<T> v, T phi, T m, T kick, T kd, T ka)

@@ -350,6 +350,41 @@ struct Packed {
     }
 };
 
+// The frequencies k < N/2 of the packed lines, spread over a group's threads: item b = gt + i NT is packed line
+// b % WP, frequency number b / WP (HalfSpec::nth).  f(k, e, en, l): e / en = shared-memory element (PK::idx) of
+// frequency k / of its mirror N - k in line l.  When the group's stride NT / WP is an even multiple DA of RM/2 (and
+// RB == 1), item i of a thread is frequency k0 + DA i, at rows a fixed distance apart, and so is its mirror from
+// i = 1 on (an even DA also keeps the swizzle bit of Packed the same): the indices are formed once per tile and
+// every later item is an immediate offset -- the index arithmetic was 40 % of the complex-to-real sweep's
+// instructions (ncu, profiles/r1e).
+template <class C, int WP, class PK, class F>
+__device__ __forceinline__ void half_spectrum_items(int gt, F &&f)
+{
+    constexpr int NT = C::NT, HM = C::RM / 2, ITEMS = (C::N / 2) * WP;
+    constexpr bool FAST = C::RB == 1 && NT % WP == 0 && (NT / WP) % (2 * HM) == 0 && ITEMS % NT == 0 && ITEMS / NT <= 16;
+    if constexpr (FAST) {
+        constexpr int DA = NT / WP / HM, ITERS = ITEMS / NT, STEP = DA * C::RM * WP;
+        static_assert(ITERS * DA == C::RA && PK::RSP == WP, "item i of a thread is frequency k0 + DA i");
+        const int l = gt % WP, kk0 = gt / WP, sM = kk0 % HM, sA0 = kk0 / HM;
+        const int k0 = sA0 + C::RA * sM;
+        const int e0 = PK::idx(sA0 * C::RM + sM, l);
+        const int en0 = PK::idx(HalfSpec<C>::row_of((C::N - k0) & (C::N - 1)), l);
+        // k = sA + RA sM with sA > 0:  N - k = (RA - sA) + RA (RM - 1 - sM)
+        const int en1 = PK::idx((C::RA - sA0 - DA) * C::RM + (C::RM - 1 - sM), l);
+        f(k0, e0, en0, l);
+        static_for<1, ITERS>([&](auto i_) {
+            constexpr int i = decltype(i_)::value;
+            f(k0 + DA * i, e0 + i * STEP, en1 - (i - 1) * STEP, l);
+        });
+    } else {
+        for (int b = gt; b < ITEMS; b += NT) {
+            int l = b % WP, k, pk;
+            HalfSpec<C>::nth(b / WP, k, pk);
+            f(k, PK::idx(pk, l), PK::idx(HalfSpec<C>::row_of((C::N - k) & (C::N - 1)), l), l);
+        }
+    }
+}
+
 struct NoPre {};
 
 constexpr size_t align128(size_t x) { return (x + 127) & ~(size_t)127; }
@@ -464,7 +499,9 @@ struct PsiK {
                                 v[r] = kick_general(v[r], th(r_), m, p.kick, p.kself_d, p.kself_a);
                             });
                         } else {
-                            static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; v[r] = rotate_neg(v[r], th(r_) * p.kick); });
+                            T ph[RA];
+                            static_for<0, RA>([&](auto r_) { constexpr int r = decltype(r_)::value; ph[r] = th(r_) * p.kick; });
+                            rotate_neg_all<RA>(v, ph);
                         }
                     }
                     fwd_level_regs<RA, T>(v, q, mA, tb.twA + q, [&](int row, cx<T> y) { S[L::idx(row, l)] = y; });
@@ -602,20 +639,18 @@ struct PsiK {
             }
             group_sync(grp, NTG);
             // Hermitian split of Z = FFT(a + i b):  A_k = (Z_k + conj Z_{N-k})/2,  B_k = (Z_k - conj Z_{N-k})/(2i)
-            auto emit = [&](int k, int pk, int l) {
-                int pn = HalfSpec<C>::row_of((N - k) & (N - 1));
-                cx<T> zk = Sp[Packed<C>::idx(pk, l)], zn = Sp[Packed<C>::idx(pn, l)];
+            auto emit = [&](int k, int e, int en, int l) {
+                cx<T> zk = Sp[e], zn = Sp[en];
                 const T h = (T)0.5;
                 cx<T> A = mk<T>((zk.x + zn.x) * h, (zk.y - zn.y) * h);
                 cx<T> B = mk<T>((zk.y + zn.y) * h, (zn.x - zk.x) * h);
                 st2(p.H + tile.at(k, 2 * l), A, B);
             };
-            for (int b = gt; b < (N / 2) * WP; b += NTG) {
-                int l = b % WP, k, pk;
-                HalfSpec<C>::nth(b / WP, k, pk);
-                emit(k, pk, l);
+            half_spectrum_items<C, WP, Packed<C>>(gt, emit);
+            if (gt < WP) {
+                const int e = Packed<C>::idx(HalfSpec<C>::row_of(N / 2), gt);
+                emit(N / 2, e, e, gt);
             }
-            if (gt < WP) emit(N / 2, HalfSpec<C>::row_of(N / 2), gt);
         }
     }
 };
@@ -750,18 +785,17 @@ struct C2RK {
         const cx<T> *R = reinterpret_cast<const cx<T> *>(buf + PACKED_BYTES);
         const TL tile(p, t);
         // Z_k = A_k + i B_k,  Z_{N-k} = conj(A_k) + i conj(B_k)
-        auto place = [&](int k, int pk, int l) {
+        auto place = [&](int k, int e, int en, int l) {
             cx<T> A, B;
             ld2(R + k * W + 2 * l, A, B);
-            Sp[Packed<C, false>::idx(pk, l)] = mk<T>(A.x - B.y, A.y + B.x);
-            if (k > 0 && k < N / 2) Sp[Packed<C, false>::idx(HalfSpec<C>::row_of(N - k), l)] = mk<T>(A.x + B.y, B.x - A.y);
+            Sp[e] = mk<T>(A.x - B.y, A.y + B.x);
+            if (k > 0 && k < N / 2) Sp[en] = mk<T>(A.x + B.y, B.x - A.y);
         };
-        for (int b = gt; b < (N / 2) * WP; b += NTG) {
-            int l = b % WP, k, pk;
-            HalfSpec<C>::nth(b / WP, k, pk);
-            place(k, pk, l);
+        half_spectrum_items<C, WP, Packed<C, false>>(gt, place);
+        if (gt < WP) {
+            const int e = Packed<C, false>::idx(HalfSpec<C>::row_of(N / 2), gt);
+            place(N / 2, e, e, gt);
         }
-        if (gt < WP) place(N / 2, HalfSpec<C>::row_of(N / 2), gt);
         group_sync(grp, NTG);
         for (int b = gt; b < (N / RM) * WP; b += NTG) {
             int l = b % WP, g = b / WP;
