@@ -336,8 +336,9 @@ struct HalfSpec {
 // lanes, which would land in the same half.  Rows whose bit log2(RM) is set therefore swap places with their
 // neighbour (row ^ 1): every access pattern of the sweeps (level A: rows q, q + 1; middle: g RM + s, (g+1) RM + s;
 // the Hermitian split: consecutive rows) then touches both halves.
-// (Measured at 512^3: -2 % on the density sweep; the complex-to-real sweep is latency bound and loses more to the
-// extra index arithmetic than it gains, so it keeps the plain layout: ON = false.)
+// (Measured at 512^3: -2 % on the density sweep.  Through idx() the swizzle costs three integer instructions per
+// access, which the latency-bound complex-to-real sweep lost more to than it gained; with idxA / idxM it is free,
+// and that sweep's middle level drops its 2-way conflicts: 8.4 M of 29.6 M wavefronts per launch, -5 %.)
 template <class C, bool ON = true>
 struct Packed {
     using T = typename C::T;
@@ -347,6 +348,22 @@ struct Packed {
     {
         if constexpr (SWZ) row ^= (row / C::RM) & 1;
         return row * RSP + l;
+    }
+    // The same index for the two access patterns of the stages, written so that the swizzle costs nothing per
+    // access once the stage is unrolled (d a compile-time constant): two base addresses per thread, the rest
+    // immediates.  idxA: row q + d of a level-A butterfly (q < RM, d a multiple of RM; RB == 1 so mA == RM).
+    // idxM: row row0 + d of a middle-level butterfly (row0 a multiple of RM, d < RM).
+    static __device__ __forceinline__ int idxA(int q, int d, int l)
+    {
+        if constexpr (SWZ) return ((q ^ ((d / C::RM) & 1)) + d) * RSP + l;
+        else return (q + d) * RSP + l;
+    }
+    static __device__ __forceinline__ int idxM(int row0, int d, int l)
+    {
+        if constexpr (SWZ) {
+            const int b = ((row0 / C::RM) & 1) * RSP;
+            return (row0 + d) * RSP + l + ((d & 1) ? -b : b);
+        } else return (row0 + d) * RSP + l;
     }
 };
 
@@ -608,7 +625,7 @@ struct PsiK {
                 });
                 cx<T> w[RA];
                 twiddles(w);
-                fwd_level_regs_w<RA, T>(v, pq, mA, w, [&](int row, cx<T> y) { Sp[Packed<C>::idx(row, pl / 2)] = y; });
+                fwd_level_regs_w<RA, T>(v, pq, mA, w, [&](int row, cx<T> y) { Sp[Packed<C>::idxA(pq, row - pq, pl / 2)] = y; });
             } else {
                 static_for<0, ITER>([&](auto it_) {
                     constexpr int it = decltype(it_)::value;
@@ -620,22 +637,22 @@ struct PsiK {
                         int row = q + mA * r;
                         T v = rho[it][r];
                         if (gp) v += ldg(gp + (long long)(mA * r) * TL::RSTRIDE);
-                        F[2 * Packed<C>::idx(row, l / 2) + (l & 1)] = v - mean;
+                        F[2 * Packed<C>::idxA(q, mA * r, l / 2) + (l & 1)] = v - mean;
                     });
                 });
                 group_sync(grp, NTG);
                 for (int b = gt; b < mA * WP; b += NTG) {
                     int l = b % WP, q = b / WP;
-                    fwd_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[Packed<C>::idx(row, l)]; },
-                                     [&](int row, cx<T> v) { Sp[Packed<C>::idx(row, l)] = v; });
+                    fwd_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[Packed<C>::idxA(q, row - q, l)]; },
+                                     [&](int row, cx<T> v) { Sp[Packed<C>::idxA(q, row - q, l)] = v; });
                 }
             }
             group_sync(grp, NTG);
             g_fwd_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return Packed<C>::idx(row, l); });
             for (int b = gt; b < (N / RM) * WP; b += NTG) {
                 int l = b % WP, g = b / WP;
-                mid_fwd<RM, T>(g * RM, [&](int row) { return Sp[Packed<C>::idx(row, l)]; },
-                               [&](int row, cx<T> v) { Sp[Packed<C>::idx(row, l)] = v; });
+                mid_fwd<RM, T>(g * RM, [&](int row) { return Sp[Packed<C>::idxM(g * RM, row - g * RM, l)]; },
+                               [&](int row, cx<T> v) { Sp[Packed<C>::idxM(g * RM, row - g * RM, l)] = v; });
             }
             group_sync(grp, NTG);
             // Hermitian split of Z = FFT(a + i b):  A_k = (Z_k + conj Z_{N-k})/2,  B_k = (Z_k - conj Z_{N-k})/(2i)
@@ -766,6 +783,7 @@ struct C2RK {
     using TL = Tile<C, AX_X>;
     static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA;
     static constexpr int WP = W / 2, RSP = W / 2;
+    using PK = Packed<C, true>;
     static constexpr size_t PACKED_BYTES = align128((size_t)N * RSP * sizeof(cx<T>));
     static constexpr size_t TILE_BYTES = PACKED_BYTES + align128((size_t)(N / 2 + 1) * W * sizeof(cx<T>));
     static constexpr int AUX = AUX_NONE;
@@ -791,19 +809,19 @@ struct C2RK {
             Sp[e] = mk<T>(A.x - B.y, A.y + B.x);
             if (k > 0 && k < N / 2) Sp[en] = mk<T>(A.x + B.y, B.x - A.y);
         };
-        half_spectrum_items<C, WP, Packed<C, false>>(gt, place);
+        half_spectrum_items<C, WP, PK>(gt, place);
         if (gt < WP) {
-            const int e = Packed<C, false>::idx(HalfSpec<C>::row_of(N / 2), gt);
+            const int e = PK::idx(HalfSpec<C>::row_of(N / 2), gt);
             place(N / 2, e, e, gt);
         }
         group_sync(grp, NTG);
         for (int b = gt; b < (N / RM) * WP; b += NTG) {
             int l = b % WP, g = b / WP;
-            mid_inv<RM, T>(g * RM, [&](int row) { return Sp[Packed<C, false>::idx(row, l)]; },
-                           [&](int row, cx<T> v) { Sp[Packed<C, false>::idx(row, l)] = v; });
+            mid_inv<RM, T>(g * RM, [&](int row) { return Sp[PK::idxM(g * RM, row - g * RM, l)]; },
+                           [&](int row, cx<T> v) { Sp[PK::idxM(g * RM, row - g * RM, l)] = v; });
         }
         group_sync(grp, NTG);
-        g_inv_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return Packed<C, false>::idx(row, l); });
+        g_inv_B<C, WP>(Sp, tb.twB, gt, grp, [](int row, int l) { return PK::idx(row, l); });
         for (int b = gt; b < mA * WP; b += NTG) {
             int l = b % WP, q = b / WP;
             T *gp = p.phi_out + tile.at(q, 2 * l);
@@ -817,8 +835,8 @@ struct C2RK {
                 }
                 stv(reinterpret_cast<cx<T> *>(gp + (long long)(row - q) * TL::RSTRIDE), v);
             };
-            if constexpr (PAIR) inv_level_w<RA, T>(q, mA, pers.w, [&](int row) { return Sp[Packed<C, false>::idx(row, l)]; }, out);
-            else inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[Packed<C, false>::idx(row, l)]; }, out);
+            if constexpr (PAIR) inv_level_w<RA, T>(q, mA, pers.w, [&](int row) { return Sp[PK::idxA(q, row - q, l)]; }, out);
+            else inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[PK::idxA(q, row - q, l)]; }, out);
         }
     }
 };
