@@ -44,6 +44,13 @@ ALG_BYTES_PER_CELL_C = {
     # read from L2 (first stage's read + last stage's write)
     "psi_chain_z_kick_y": 4.5, "poisson_chain_y_zgreen_y": 3.0,
 }
+# The CPU oracle is timed on ONE sample, in the reference arm and in the cpu_baseline leg alike: the soliton + halo
+# recipe of the bench workload at 256^3 (float64, 0.3 s per KDK step on 16 host cores; 512^3 would need 6.5 GB and
+# 3 s per step).
+REF_SAMPLE_N = 256
+# algorithmic HBM bytes per particle of the particle kernels (pos, vel read + write in the push,
+# pos read in the deposit; the gathered Phi nodes and the deposited rho_p nodes go through L2)
+PARTICLE_BYTES = {"particle_gather_kick_drift": 48, "particle_cic_deposit": 12}
 HBM_MIN_PER_CELL_C = dict(ALG_BYTES_PER_CELL_C, psi_chain_z_kick_y=2.5, poisson_chain_y_zgreen_y=1.0)
 
 
@@ -160,7 +167,7 @@ def oracle_rate(sample_name: str, steps: int, warmup: int):
 def run_reference(args, rank, world):
     if rank != 0:
         return
-    n_ref = 256 if (args.steps + args.warmup) <= 12 else 128
+    n_ref = REF_SAMPLE_N
     w, rate, el, thr = oracle_rate(f"sample{n_ref}", args.steps, args.warmup)
     sample = (f"float64 CPU oracle, soliton+halo workload at {n_ref}^3 instead of 512^3 "
               f"({args.steps} timed KDK steps, {el:.1f} s)")
@@ -284,6 +291,25 @@ def main():
                                           "hbm_min_bytes_per_step": step_min,
                                           "hbm_min_frac": step_min / (ms / K * 1e-3) / 1e9 / peak}}
         out["kernels"] = kern
+        if npart:
+            # particle kernels against their own HBM count; the rho_p clear (one real per cell, "particle_mesh_clear")
+            # and rho_p's read inside the density sweep are per-cell costs of the coupled step (96 B/cell instead of 88)
+            rsize = csize // 2
+            pk = {}
+            for name, b in PARTICLE_BYTES.items():
+                if name in kern:
+                    g = b * (rsize // 4) * npart / (kern[name]["avg_ms"] * 1e-3) / 1e9
+                    pk[name] = {"avg_ms": kern[name]["avg_ms"], "launches_per_step": kern[name]["launches"] / kp,
+                                "alg_bytes_per_particle": b * (rsize // 4), "achieved_GBs": g, "frac": g / peak}
+            for name in ("particle_mesh_clear", "particle_cell_sort"):
+                if name in kern:
+                    pk[name] = {"avg_ms": kern[name]["avg_ms"], "launches_per_step": kern[name]["launches"] / kp}
+            if "particle_mesh_clear" in pk:
+                g = rsize * N ** 3 / (pk["particle_mesh_clear"]["avg_ms"] * 1e-3) / 1e9
+                pk["particle_mesh_clear"].update({"alg_bytes": rsize * N ** 3, "achieved_GBs": g, "frac": g / peak})
+            pk["ms_per_step_all_particle_kernels"] = sum(kern[k]["avg_ms"] * kern[k]["launches"] for k in kern if k.startswith("particle_")) / kp
+            pk["share_of_step"] = sum(kern[k]["share"] for k in kern if k.startswith("particle_"))
+            out["particles"] = pk
 
         # ---- end to end through the C ABI with HOST buffers: copy in + K steps + copy out, wall clock
         out_host = torch.empty_like(psi_host).pin_memory()
@@ -300,7 +326,7 @@ def main():
 
         # ---- CPU oracle on the host cores, bounded sample (rank 0, N = 1 only)
         if rank == 0 and world == 1 and not args.no_cpu_baseline:
-            n_ref, CPU_STEPS = 256, 40         # about 13 s on 16 host cores (bounded sample: 10-30 s of CPU work)
+            n_ref, CPU_STEPS = REF_SAMPLE_N, 40         # about 13 s on 16 host cores (bounded sample: 10-30 s of CPU work)
             ws, rate, el, thr = oracle_rate(f"sample{n_ref}", CPU_STEPS, 1)
             out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": thr, "kind": "oracle",
                                    "sample": f"float64 CPU oracle, soliton+halo at {n_ref}^3, {CPU_STEPS} timed KDK steps ({el:.1f} s)"}

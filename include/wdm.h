@@ -28,7 +28,7 @@ typedef struct wdm_ctx wdm_ctx; /* opaque, owned by the library */
 enum { WDM_C64 = 0, WDM_C128 = 1 };
 enum {
     WDM_OK = 0,
-    WDM_EINVAL = 1,       /* null pointer, L <= 0, hbar_over_m <= 0, G < 0, n < 0, nsteps < 0, bad dtype */
+    WDM_EINVAL = 1,       /* null pointer, L <= 0, hbar_over_m <= 0, G < 0, n < 0, nsteps < 0, non-finite dt, bad dtype */
     WDM_EUNSUPPORTED = 2, /* N not a power of two or outside [8, 1024] (powers of two)  */
     WDM_ENOMEM = 3,       /* device allocation failed / caller workspace too small                     */
     WDM_ECUDA = 4,        /* a CUDA call failed; text in wdm_last_error                                */
@@ -51,7 +51,8 @@ int wdm_create_ws(wdm_ctx **out, int N, double L, double hbar_over_m, double G, 
 int wdm_destroy(wdm_ctx *ctx);
 
 /* All later work of this context is enqueued on `cuda_stream` (a cudaStream_t, e.g.
- * torch.cuda.current_stream().cuda_stream; NULL = the legacy default stream). */
+ * torch.cuda.current_stream().cuda_stream; NULL = the legacy default stream).  The new stream is first made to
+ * wait (event) for everything the context has already enqueued on the old one, so a change is always safe. */
 int wdm_set_stream(wdm_ctx *ctx, void *cuda_stream);
 
 /* Copy in the wave function, N^3 interleaved complex of the context dtype.  Marks Phi stale (G8). */
@@ -97,8 +98,10 @@ int wdm_get_particles_host(wdm_ctx *ctx, void *pos_out_host, void *vel_out_host)
 /* Extra terms of the potential kick (generalised equation, Eq. 13-14) and the absorbing
  * layer (Eq. 22; Alg. 1 l.15-18).  All act inside the fused kick: no extra pass over psi.
  *   kappa        local self-interaction, V += kappa |psi|^2 (potential units, like Phi; any sign)
- *   phi_ext_dev  static external potential, N^3 reals in the layout of Phi, or NULL.  NOT copied: the
- *                buffer must stay valid and unchanged while it is set.  It is added to the Poisson
+ *   phi_ext_dev  static external potential, N^3 reals in the layout of Phi, or NULL.  COPIED (stream-ordered) into
+ *                library-owned memory (one cudaMalloc of N^3 reals on first use, also for wdm_create_ws contexts;
+ *                WDM_ENOMEM if it fails): the caller may free or change its buffer once the stream has passed
+ *                the call.  It is added to the Poisson
  *                potential (Phi_total = Phi_DM + Phi_ext): psi and the particles feel the sum, and
  *                wdm_get_potential returns the sum.
  *   absorb_alpha, absorb_nb   after every step psi *= exp(-alpha (b(x) + b(y) + b(z)) dt) with

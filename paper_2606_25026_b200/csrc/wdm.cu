@@ -151,11 +151,11 @@ __global__ void __launch_bounds__(256) k_diag(const cx<T> *__restrict__ psi, con
 }
 
 enum Slot { S_PSI_Z, S_PSI_Y, S_PSI_X_RHO, S_H_Y_FWD, S_H_Z_GREEN, S_H_Y_INV, S_C2R, S_KICK, S_PART_PUSH,
-            S_PART_DEPOSIT, S_PART_SORT, S_MISC, S_PSI_ZY, S_H_YZY, S_COUNT };
+            S_PART_DEPOSIT, S_PART_SORT, S_MISC, S_PSI_ZY, S_H_YZY, S_PART_CLEAR, S_COUNT };
 static const char *kSlotNames[S_COUNT] = {"psi_sweep_z_kick", "psi_sweep_y", "psi_sweep_x_rho_r2c", "poisson_y_fwd",
                                           "poisson_z_green", "poisson_y_inv", "poisson_x_c2r", "kick_elementwise",
                                           "particle_gather_kick_drift", "particle_cic_deposit", "particle_cell_sort",
-                                          "misc", "psi_chain_z_kick_y", "poisson_chain_y_zgreen_y"};
+                                          "misc", "psi_chain_z_kick_y", "poisson_chain_y_zgreen_y", "particle_mesh_clear"};
 
 }  // namespace wdm
 
@@ -184,7 +184,8 @@ struct wdm_ctx {
     // extra kick terms (wdm_set_kick_terms; readings G26-G28)
     double kappa = 0, alpha = 0;
     int absorb_nb = 50;
-    const void *phi_ext = nullptr;            // caller-owned N^3 reals or nullptr
+    const void *phi_ext = nullptr;            // library-owned copy of the caller's N^3 reals (phi_ext_buf) or nullptr
+    void *phi_ext_buf = nullptr;              // cudaMalloc'ed on the first wdm_set_kick_terms with an external potential
     void *mask = nullptr;                     // 3 N axis factors exp(-alpha b dt) for mask_dt
     double mask_dt = 0;
     bool mask_valid = false;
@@ -277,28 +278,40 @@ static int prof_flush(wdm_ctx *c)
     return WDM_OK;
 }
 
+// Brackets one launch with events when profiling is on.  A failing event call switches profiling off for the
+// context and leaves the text in wdm_last_error (the launch itself is unaffected; its own status is checked by CU).
 struct Timed {
     wdm_ctx *c;
     int slot;
     bool on;
     size_t idx = 0;
+    static bool ok(wdm_ctx *c, cudaError_t e, const char *what)
+    {
+        if (e == cudaSuccess) return true;
+        fail(c, WDM_ECUDA, "profiling switched off: %s: %s", what, cudaGetErrorString(e));
+        c->profiling = false;
+        c->ev_used = 0;
+        return false;
+    }
     Timed(wdm_ctx *c_, int slot_) : c(c_), slot(slot_), on(c_->profiling)
     {
         c->launches++;
         if (!on) return;
         if (c->ev_used * 2 >= c->ev.size()) {
-            if (c->ev.size() >= 2 * 8192) { prof_flush(c); }
-            else {
-                cudaEvent_t a, b;
-                cudaEventCreate(&a); cudaEventCreate(&b);
+            if (c->ev.size() >= 2 * 8192) {
+                if (prof_flush(c) != WDM_OK) { c->profiling = on = false; return; }
+            } else {
+                cudaEvent_t a = nullptr, b = nullptr;
+                if (!ok(c, cudaEventCreate(&a), "cudaEventCreate")) { on = false; return; }
+                if (!ok(c, cudaEventCreate(&b), "cudaEventCreate")) { cudaEventDestroy(a); on = false; return; }
                 c->ev.push_back(a); c->ev.push_back(b); c->ev_slot.push_back(0);
             }
         }
         idx = c->ev_used++;
         c->ev_slot[idx] = slot;
-        cudaEventRecord(c->ev[2 * idx], c->stream);
+        if (!ok(c, cudaEventRecord(c->ev[2 * idx], c->stream), "cudaEventRecord")) on = false;
     }
-    ~Timed() { if (on) cudaEventRecord(c->ev[2 * idx + 1], c->stream); }
+    ~Timed() { if (on) ok(c, cudaEventRecord(c->ev[2 * idx + 1], c->stream), "cudaEventRecord"); }
 };
 
 // ---------------------------------------------------------------- TMA descriptors
@@ -435,7 +448,6 @@ static int density_poisson(wdm_ctx *c, bool drift)
         SweepParams<T> p = base_params<T>(c);
         p.data = (cx<T> *)c->psi;
         p.tmap = c->tm_psi_x;
-        p.tag = S_PSI_X_RHO;
         take_ticket(c, p);
         Timed t(c, S_PSI_X_RHO);
         CU(c, c->tab->psi_x_rho(&p, drift ? 1 : 0, c->stream));
@@ -445,17 +457,16 @@ static int density_poisson(wdm_ctx *c, bool drift)
     p.tmap = c->tm_h_y;
     if (c->lag_h > 0) {
         ChainCtl ctl{c->chain_done + N, ++c->epoch_h * (unsigned int)(N / c->tab->fact.W), c->lag_h};
-        p.tag = S_H_YZY;
         Timed t(c, S_H_YZY);
         CU(c, c->tab->h_yzy(&p, &p, &ctl, c->stream));
     } else {
-        { p.tag = S_H_Y_FWD; take_ticket(c, p); Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
-        { p.tag = S_H_Z_GREEN; take_ticket(c, p); Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
-        { p.tag = S_H_Y_INV; take_ticket(c, p); Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
+        { take_ticket(c, p); Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
+        { take_ticket(c, p); Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
+        { take_ticket(c, p); Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
     }
     p.tmap = c->tm_h_x;
     p.tmap2 = c->tm_h_x1;
-    { p.tag = S_C2R; take_ticket(c, p); Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, c->stream)); }
+    { take_ticket(c, p); Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, c->stream)); }
     return WDM_OK;
 }
 
@@ -463,7 +474,7 @@ template <typename T>
 static int particles_deposit(wdm_ctx *c)
 {
     if (c->part.n == 0) return WDM_OK;
-    { Timed t(c, S_MISC); CU(c, cudaMemsetAsync(c->part.rho_p, 0, c->n * sizeof(T), c->stream)); }
+    { Timed t(c, S_PART_CLEAR); CU(c, cudaMemsetAsync(c->part.rho_p, 0, c->n * sizeof(T), c->stream)); }
     Timed t(c, S_PART_DEPOSIT);
     CU(c, particle_deposit(c->part, c->N, c->L, c->dtype, c->stream));
     return WDM_OK;
@@ -556,6 +567,7 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
         if (c->part.n > 0 && !c->pstatic) {
             // v += a(Phi^n, x^n) kdt/nsub ; nsub x { x += v dt/nsub ; wrap ; [kick] } ; then deposit x^{n+1}  (G14-G16, G29)
             { Timed t(c, S_PART_PUSH); CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, have_phi ? (hd_p + ha) / c->nsub : 0.0, dt, c->nsub, c->stream)); }
+            if (particle_sort_due(c->part)) { Timed t(c, S_PART_SORT); c->launches += 2; CU(c, particle_resort(c->part, c->N, c->L, c->dtype, c->stream)); }
             if (grav) { rc = particles_deposit<T>(c); if (rc) return rc; }
         }
         {
@@ -570,12 +582,11 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             py.tmap = c->tm_psi_y;
             if (c->lag_psi > 0 && !pz.kick_extra) {
                 ChainCtl ctl{c->chain_done, ++c->epoch_psi * (unsigned int)(N / c->tab->fact.W), c->lag_psi};
-                pz.tag = S_PSI_ZY;
                 Timed t(c, S_PSI_ZY);
                 CU(c, c->tab->psi_zy(&pz, &py, kicks ? 1 : 0, &ctl, c->stream));
             } else {
-                { pz.tag = S_PSI_Z; take_ticket(c, pz); Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? (pz.kick_extra ? 2 : 1) : 0, c->stream)); }
-                { py.tag = S_PSI_Y; take_ticket(c, py); Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
+                { take_ticket(c, pz); Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? (pz.kick_extra ? 2 : 1) : 0, c->stream)); }
+                { take_ticket(c, py); Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
             }
         }
         c->pend_psi = 0.0;
@@ -703,6 +714,7 @@ extern "C" int wdm_destroy(wdm_ctx *c)
     cudaStreamSynchronize(c->stream);
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     for (void *p : c->owned) cudaFree(p);
+    if (c->phi_ext_buf) cudaFree(c->phi_ext_buf);
     delete c;
     return WDM_OK;
 }
@@ -712,6 +724,14 @@ extern "C" int wdm_set_stream(wdm_ctx *c, void *s)
     if (!c) return WDM_EINVAL;
     int rc = prof_flush(c);
     if (rc) return rc;
+    if ((cudaStream_t)s != c->stream) {
+        // work already enqueued on the old stream (wdm_step is asynchronous) must precede anything on the new one
+        cudaEvent_t e;
+        CU(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        cudaError_t e1 = cudaEventRecord(e, c->stream), e2 = e1 == cudaSuccess ? cudaStreamWaitEvent((cudaStream_t)s, e, 0) : e1;
+        cudaEventDestroy(e);
+        if (e2 != cudaSuccess) return fail(c, WDM_ECUDA, "ordering the new stream after the old one: %s", cudaGetErrorString(e2));
+    }
     c->stream = (cudaStream_t)s;
     return WDM_OK;
 }
@@ -769,7 +789,7 @@ extern "C" int wdm_set_particles_host(wdm_ctx *c, long long n, const void *pos, 
 extern "C" int wdm_step(wdm_ctx *c, int nsteps, double dt)
 {
     if (!c) return WDM_EINVAL;
-    if (nsteps < 0 || dt != dt) return fail(c, WDM_EINVAL, "nsteps must be >= 0 and dt finite");
+    if (nsteps < 0 || !std::isfinite(dt)) return fail(c, WDM_EINVAL, "nsteps must be >= 0 and dt finite");
     return c->dtype == WDM_C64 ? step_impl<float>(c, nsteps, dt) : step_impl<double>(c, nsteps, dt);
 }
 
@@ -922,12 +942,20 @@ extern "C" int wdm_get_diagnostics(wdm_ctx *c, double *out_host)
 extern "C" int wdm_set_kick_terms(wdm_ctx *c, double kappa, const void *phi_ext_dev, double absorb_alpha, int absorb_nb)
 {
     if (!c) return WDM_EINVAL;
-    if (kappa != kappa || !(absorb_alpha >= 0) || (absorb_alpha > 0 && absorb_nb < 1))
+    if (!std::isfinite(kappa) || !std::isfinite(absorb_alpha) || !(absorb_alpha >= 0) || (absorb_alpha > 0 && absorb_nb < 1))
         return fail(c, WDM_EINVAL, "need a finite kappa, absorb_alpha >= 0 and absorb_nb >= 1");
     int rcf = do_flush(c, true, true);           // pending closing kicks belong to the old terms
     if (rcf) return rcf;
+    if (phi_ext_dev) {
+        // copied: the caller's buffer may be freed or changed after this call returns (stream-ordered copy)
+        if (!c->phi_ext_buf) {
+            cudaError_t e = cudaMalloc(&c->phi_ext_buf, c->n * rsize(c->dtype));
+            if (e != cudaSuccess) { cudaGetLastError(); c->phi_ext_buf = nullptr; return fail(c, WDM_ENOMEM, "cudaMalloc of the external potential copy (%zu bytes): %s", c->n * rsize(c->dtype), cudaGetErrorString(e)); }
+        }
+        CU(c, cudaMemcpyAsync(c->phi_ext_buf, phi_ext_dev, c->n * rsize(c->dtype), cudaMemcpyDeviceToDevice, c->stream));
+    }
     c->kappa = kappa;
-    c->phi_ext = phi_ext_dev;
+    c->phi_ext = phi_ext_dev ? c->phi_ext_buf : nullptr;
     c->alpha = absorb_alpha;
     c->absorb_nb = absorb_nb;
     c->mask_valid = false;

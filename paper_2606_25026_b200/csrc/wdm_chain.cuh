@@ -212,13 +212,11 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
         const int b = j % NBUF;
         unsigned char *buf = smem + (size_t)b * SM::TILE_BYTES;
         const TileRef r = chain_decode(cp, bid + j * stride);
-        WDM_T(t_top);
         // one warp polls for the start of this fill (the others would only burn issue slots the other group needs)
         if (gt < 32)
             while (issued[b] < j / NBUF + 1) __nanosleep(100);
         group_sync(grp, NTG);
         mbar_wait(full + b, (j / NBUF) & 1);
-        WDM_T(t_data);
         auto hook = [&]() { prefetch_for(j + NG); };
         auto go = [&](auto i_) {
             constexpr int I = decltype(i_)::value;
@@ -235,7 +233,6 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
         chain_dispatch<0, NS>(r.stage, go);
         fence_proxy_async();
         group_sync(grp, NTG);                                   // buffer free; every store of the tile issued
-        WDM_T(t_done);
         if (gt < 32) {
             // release: the group's stores (ordered before this thread by the barrier) are visible before the count
             if (gt == 0 && r.stage < NS - 1) red_release_add(cp.done + (size_t)r.stage * cp.units + r.unit, 1u);
@@ -246,9 +243,6 @@ __device__ __forceinline__ void chain_run(const ChainParams<typename StageAt<0, 
                 request(j + NBUF, b);
             }
         }
-#ifdef WDM_TRACE
-        if (gt == 0) trace_put(cp.p[0].tag, grp, NG, j / NG, r.stage, t_top, t_data, t_done, clock64());
-#endif
     }
 }
 

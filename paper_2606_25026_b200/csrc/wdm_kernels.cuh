@@ -151,7 +151,6 @@ struct SweepParams {
     CUtensorMap tmap, tmap2;
     unsigned int *ticket;      // tile tickets drawn in this launch (0 when the launch starts)
     unsigned int *ticket_next; // the next launch's counter: this launch zeroes it (launches alternate between two words)
-    int tag;                   // which launch of the step this is (kernel-stats slot; read by developer traces only)
 };
 
 // Axis of a sweep over an array [x][y][z] (z contiguous).  The strides are compile-time constants of the

@@ -418,11 +418,16 @@ cudaError_t particle_push(ParticleState &ps, int N, double L, int dtype, const v
     else if (dtype == 0) k_push<float, 3><<<g, 128, 0, s>>>((float *)ps.pos, (float *)ps.vel, (const float *)phi, ps.n, N, (float)L, (float)kick_dt, (float)drift_dt, nsub);
     else if (ps.order == 2) k_push<double, 2><<<g, 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt, nsub);
     else k_push<double, 3><<<g, 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt, nsub);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    if (drift_dt != 0.0 && ++ps.steps_since_sort >= kResortInterval)
-        return dtype == 0 ? resort<float>(ps, N, L, s) : resort<double>(ps, N, L, s);
-    return cudaSuccess;
+    if (drift_dt != 0.0) ++ps.steps_since_sort;
+    return cudaGetLastError();
+}
+
+bool particle_sort_due(const ParticleState &ps) { return ps.n > 0 && ps.steps_since_sort >= kResortInterval; }
+
+cudaError_t particle_resort(ParticleState &ps, int N, double L, int dtype, cudaStream_t s)
+{
+    if (ps.n == 0) return cudaSuccess;
+    return dtype == 0 ? resort<float>(ps, N, L, s) : resort<double>(ps, N, L, s);
 }
 
 cudaError_t particle_deposit(ParticleState &ps, int N, double L, int dtype, cudaStream_t s)

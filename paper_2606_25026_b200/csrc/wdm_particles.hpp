@@ -30,6 +30,9 @@ cudaError_t particle_set(ParticleState &ps, int N, double L, int dtype, long lon
 // size, gathered at the new position, between two drifts
 cudaError_t particle_push(ParticleState &ps, int N, double L, int dtype, const void *phi, double kick_dt,
                           double drift_dt, int nsub, cudaStream_t s);
+// the tile order is kResortInterval drifts old: re-sort (counting sort by mesh tile) before the next deposit
+bool particle_sort_due(const ParticleState &ps);
+cudaError_t particle_resort(ParticleState &ps, int N, double L, int dtype, cudaStream_t s);
 // rho_p += deposit of the particles' mass with the scheme ps.order (the caller zeroes rho_p)
 cudaError_t particle_deposit(ParticleState &ps, int N, double L, int dtype, cudaStream_t s);
 cudaError_t particle_get(ParticleState &ps, int dtype, void *pos_out, void *vel_out, bool to_host, cudaStream_t s);

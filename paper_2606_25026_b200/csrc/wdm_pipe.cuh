@@ -66,23 +66,6 @@ __device__ __forceinline__ void group_sync(int group, int nthreads)
     asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "r"(nthreads) : "memory");
 }
 
-// ---------------------------------------------------------------- per-tile timeline (developer builds only, -DWDM_TRACE)
-#ifdef WDM_TRACE
-__device__ long long *g_wdm_trace;          // [cta][group][tile slot][8]: stage, t_top, t_data, t_done, t_requested
-__device__ int g_wdm_trace_tag;             // only launches with this SweepParams::tag write
-constexpr int kTraceSlots = 640;
-__device__ __forceinline__ void trace_put(int tag, int grp, int ng, int slot, int stage, long long t0, long long t1, long long t2, long long t3)
-{
-    if (g_wdm_trace && tag == g_wdm_trace_tag && slot < kTraceSlots) {
-        long long *r = g_wdm_trace + (((size_t)blockIdx.x * ng + grp) * kTraceSlots + slot) * 8;
-        r[0] = stage; r[1] = t0; r[2] = t1; r[3] = t2; r[4] = t3;
-    }
-}
-#define WDM_T(x) long long x = clock64()
-#else
-#define WDM_T(x)
-#endif
-
 // ---------------------------------------------------------------- the pipeline driver
 // K provides:  using C;  TILE_BYTES;  AUX;  struct Pre;  issue(p, tile, buf, gt);  prefetch(p, tile, gt, pre);
 //              compute(p, tabs, tile, next_tile, buf, gt, grp, pre)
@@ -197,7 +180,6 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
     for (int k = grp;; k += NG) {
         const int b = k % NBUF;
         unsigned char *buf = smem + (size_t)b * K::TILE_BYTES;
-        WDM_T(t_top);
         // one warp polls for the start of this fill (the others would only burn issue slots the other group needs)
         if (gt < 32)
             while (issued[b] < k / NBUF + 1) __nanosleep(100);
@@ -212,7 +194,6 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
         unsigned int ticket = 0;
         if (gt == 0) ticket = (unsigned int)nstatic + atomicAdd(p.ticket, 1u);   // consumed after the compute: latency hidden
         mbar_wait(full + b, (k / NBUF) & 1);
-        WDM_T(t_data);
         if (pre_tile != t) K::prefetch(p, t, gt, pre);
         // called by compute() before its last stage: fetch what the group's NEXT tile needs into registers, if
         // that tile has been assigned by now
@@ -226,7 +207,6 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
         K::compute(p, tb, t, buf, gt, grp, pre, pers, hook);
         fence_proxy_async();                                    // this thread's accesses to the buffer, before its refill
         group_sync(grp, NTG);                                   // every read of this buffer is done
-        WDM_T(t_done);
         if (gt < 32) {
             int tn = (int)__shfl_sync(0xffffffffu, ticket, 0);
             if (tn >= ntiles) tn = -1;
@@ -237,9 +217,6 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
             }
             if (tn >= 0) K::issue(p, tn, buf, full + b, gt);
         }
-#ifdef WDM_TRACE
-        if (gt == 0) trace_put(p.tag, grp, NG, k / NG, 0, t_top, t_data, t_done, clock64());
-#endif
     }
 }
 

@@ -192,14 +192,6 @@ const SweepTable kTable = {Fact{C::N, C::RA, C::RB, C::RM, C::W, C::NT, C::NG, C
 
 }  // namespace
 
-#ifdef WDM_TRACE
-extern "C" int wdm_trace_set(long long *buf_dev, int tag)
-{
-    cudaMemcpyToSymbol(g_wdm_trace_tag, &tag, sizeof tag);
-    return (int)cudaMemcpyToSymbol(g_wdm_trace, &buf_dev, sizeof buf_dev);
-}
-#endif
-
 #define WDM_CAT3(a, b, c) a##b##_##c
 #define WDM_TABLE_NAME(d, n) WDM_CAT3(sweep_table_, d, n)
 const SweepTable *WDM_TABLE_NAME(WDM_DTYPE, WDM_N)() { return &kTable; }

@@ -46,15 +46,34 @@ def pair(wdm, w, max_particles=0):
     return sim, o
 
 
+MAXABS = 50.0      # max-abs bound = MAXABS x the rel-L2 tolerance x max|field| (one bad tile cannot hide in a norm)
+
+
+def maxabs(a, b):
+    """max |a - b| / max |b|"""
+    b = np.asarray(b)
+    a = np.asarray(a, dtype=np.complex128 if np.iscomplexobj(a) else np.float64)
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
 def check_fields(sim, o, dtype, nsteps, what=""):
+    """rel-L2 within the north_star tolerance (the pass criterion BASELINE.json states) AND, element by element,
+    max|gpu - oracle| <= MAXABS x that tolerance x max|oracle|: at 512^3 a single wrong tile (8192 cells) at the 1 %
+    level reads 7.8e-5 in the norm but 1e-2 in the maximum."""
     t = tol(dtype, nsteps)
-    e_psi = rel(sim.psi().cpu().numpy(), o.psi())
-    e_phi = rel(sim.potential().cpu().numpy(), o.potential())
-    e_rho = rel(sim.density().cpu().numpy(), o.density())
-    assert e_psi <= t, f"{what} psi {e_psi} > {t}"
-    assert e_phi <= t, f"{what} Phi {e_phi} > {t}"
-    assert e_rho <= 2 * t, f"{what} rho {e_rho} > {2 * t}"
-    return e_psi, e_phi
+    got = {"psi": sim.psi().cpu().numpy(), "Phi": sim.potential().cpu().numpy(), "rho": sim.density().cpu().numpy()}
+    ref = {"psi": o.psi(), "Phi": o.potential(), "rho": o.density()}
+    err = {}
+    for key, f in (("psi", 1), ("Phi", 1), ("rho", 2)):
+        if key == "Phi" and not np.any(ref[key]):
+            assert not np.any(got[key]), f"{what} Phi must vanish"
+            err[key] = 0.0
+            continue
+        err[key] = rel(got[key], ref[key])
+        assert err[key] <= f * t, f"{what} {key} rel-L2 {err[key]} > {f * t}"
+        m = maxabs(got[key], ref[key])
+        assert m <= MAXABS * f * t, f"{what} {key} max-abs {m} > {MAXABS * f * t}"
+    return err["psi"], err["Phi"]
 
 
 # ---------------------------------------------------------------- config 1: exactness, checked after every step
@@ -90,7 +109,7 @@ def test_white_noise_all_modes(wdm, N, dtype):
     sim.close()
 
 
-@pytest.mark.parametrize("dtype,N", [("c64", 256), ("c128", 256), ("c64", 512)])
+@pytest.mark.parametrize("dtype,N", [("c64", 256), ("c128", 256), ("c64", 512), ("c128", 512)])
 def test_large_sizes_two_steps(wdm, dtype, N):
     psi0 = (0.3 * wl.random_field(N, dtype, 7) + 1.0).astype(np.complex64 if dtype == "c64" else np.complex128)
     w = wl.Workload(f"noise{N}", N, dtype, 2, psi=psi0)
@@ -98,7 +117,7 @@ def test_large_sizes_two_steps(wdm, dtype, N):
     sim, o = pair(wdm, w)
     sim.step(2, w.dt)
     o.step(2, w.dt)
-    check_fields(sim, o, dtype, 2, f"N={N}")
+    check_fields(sim, o, dtype, 2, f"N={N}")      # c128-512: the three-level (RB > 1) transforms, 8 x 8 x 8
     sim.close()
 
 
@@ -307,48 +326,241 @@ def test_t512_sampled_properties(wdm):
     sim.close()
 
 
-def test_config4_1024_closed_forms(wdm):
-    """Config 4's size (1024^3 complex64; a float64 oracle run would need > 50 GB): properties that hold at any
-    size, evaluated on the device.  (1) plane wave with all three wavenumbers non-zero: Phi = 0 and
-    psi(t) = A exp(i(k.x - mu k^2 t/2)) exactly (P3) -- every twiddle, digit reversal and kinetic-phase index of
-    the 1024-point sweeps; (2) rho = r0 + r1 cos(k.x): Phi = -4 pi G r1 cos(k.x)/k^2 (P4) -- the real-to-complex,
-    Green and complex-to-real sweeps; (3) unitarity of two steps on a noisy field."""
+class ModeSum:
+    """sum_j amp_j exp(i k_j . x) on the N^3 lattice x_i = -L/2 + i L/N, k_j = 2 pi n_j / L with integer n_j, built on
+    the device in float64 by x-chunks (one complex GEMM per chunk).  The angles are 2 pi (n (i - N/2) mod N)/N with
+    the product reduced in integers, so every factor is exact to double rounding.  Also the projections
+    <field, exp(i k_j . x)> / N^3 of a given field onto the same modes."""
+
+    def __init__(self, N, n, chunk=32):
+        import torch
+        self.torch, self.N, self.chunk = torch, N, chunk
+        self.n = torch.as_tensor(np.asarray(n), device="cuda", dtype=torch.int64)          # (J, 3)
+        i = torch.arange(N, device="cuda", dtype=torch.int64) - N // 2
+        def E(col):
+            m = (self.n[:, col][None, :] * i[:, None]) % N
+            ang = (2.0 * math.pi / N) * m.to(torch.float64)
+            return torch.polar(torch.ones_like(ang), ang)                                  # (N, J) complex128
+        self.Ex = E(0)
+        Ey, Ez = E(1), E(2)
+        self.YZ = (Ey.T[:, :, None] * Ez.T[:, None, :]).reshape(self.n.shape[0], N * N)     # (J, N^2)
+
+    def chunks(self):
+        return [(x0, min(x0 + self.chunk, self.N)) for x0 in range(0, self.N, self.chunk)]
+
+    def slab(self, amp, x0, x1):
+        """(x1 - x0, N, N) complex128 slab of the sum"""
+        return ((self.Ex[x0:x1] * amp[None, :]) @ self.YZ).view(x1 - x0, self.N, self.N)
+
+    def fill(self, amp, out, real_sqrt_offset=None):
+        """out[...] = the sum (cast to out's dtype); with real_sqrt_offset = r0: out = sqrt(r0 + Re(sum))"""
+        for x0, x1 in self.chunks():
+            v = self.slab(amp, x0, x1)
+            out[x0:x1] = (self.torch.sqrt(real_sqrt_offset + v.real) if real_sqrt_offset is not None else v).to(out.dtype)
+        return out
+
+    def compare(self, amp, field, real=False):
+        """(rel-L2, max-abs / max|ref|) of `field` against the sum (its real part if real)"""
+        t = self.torch
+        num = den = 0.0
+        mx = mref = 0.0
+        for x0, x1 in self.chunks():
+            ref = self.slab(amp, x0, x1)
+            if real:
+                ref = ref.real
+                d = field[x0:x1].to(t.float64) - ref
+            else:
+                d = field[x0:x1].to(t.complex128) - ref
+            num += float((d.abs() ** 2).sum()); den += float((ref.abs() ** 2).sum())
+            mx = max(mx, float(d.abs().max())); mref = max(mref, float(ref.abs().max()))
+        return math.sqrt(num / den), mx / mref
+
+    def project(self, field):
+        """c_j = sum_x field(x) exp(-i k_j . x) / N^3 for every mode j (complex128, (J,))"""
+        t = self.torch
+        acc = t.zeros(self.n.shape[0], device="cuda", dtype=t.complex128)
+        YZc = self.YZ.conj().T.contiguous()                                                 # (N^2, J)
+        for x0, x1 in self.chunks():
+            f = field[x0:x1].reshape(x1 - x0, self.N * self.N).to(t.complex128)
+            acc += ((f @ YZc) * self.Ex[x0:x1].conj()).sum(dim=0)
+        return acc / float(self.N) ** 3
+
+
+def lattice_modes(N, J, seed):
+    """J distinct integer wave vectors: every axis reaches -(N/2 - 1), N/2 - 1 and the Nyquist index N/2, the
+    lowest modes are present (they dominate Phi ~ rho_k / k^2), the rest uniform in the whole spectrum."""
+    rng = np.random.default_rng(seed)
+    h = N // 2
+    forced = [(h - 1, -(h - 1), h), (-(h - 1), h, h - 1), (h, h - 1, -(h - 1)), (h, h, h), (h - 1, h - 1, h - 1),
+              (0, 0, 1), (0, 1, 0), (1, 0, 0), (-1, 1, 0), (0, -1, -1), (1, 1, 1), (3, -7, 11), (0, 0, h), (0, h, 0), (h, 0, 0),
+              (0, 0, -(h - 1)), (0, h - 1, 0), (-(h - 1), 0, 0)]
+    seen = set(forced)
+    while len(seen) < J:
+        seen.add(tuple(int(v) for v in rng.integers(-(h - 1), h + 1, size=3)))
+    seen.discard((0, 0, 0))
+    return np.array(sorted(seen), dtype=np.int64)
+
+
+BIG = [("c64", 1024), ("c128", 1024), ("c128", 512), ("c64", 512)]
+
+
+@pytest.mark.parametrize("dtype,N", BIG)
+def test_multimode_free_evolution_closed_form(wdm, dtype, N):
+    """G = 0: psi0 = sum_j A_j exp(i k_j . x) over ~256 seeded lattice modes that reach +-(N/2 - 1) and N/2 on every
+    axis evolves to sum_j A_j exp(i (k_j . x - mu |k_j|^2 t / 2)) EXACTLY for any dt ("exact solution to the dispersion
+    term"; Eq. 18(b)): every twiddle, digit reversal and kinetic-phase entry those modes
+    visit along each axis, at the sizes the CPU oracle cannot hold (1024^3) and for the three-level complex128
+    factorisations (512 = 8.8.8, 1024 = 8.8.16).  Evaluated on the device in float64; rel-L2 and max-abs."""
     import torch
-    N, L = 1024, 1.0
-    dt = (L / N) ** 2 / 6
-    x = (-0.5 * L + (L / N) * torch.arange(N, device="cuda", dtype=torch.float64))
-    n = (3, -7, 11)
-    k = [2 * math.pi * v / L for v in n]
-    sim = wdm.Sim(N, dtype="c64")
-    ph = (k[0] * x)[:, None, None] + (k[1] * x)[None, :, None] + (k[2] * x)[None, None, :]
-    A = 0.7
-    psi = torch.polar(torch.full_like(ph, A), ph).to(torch.complex64)
+    L, mu = 1.3, 0.8
+    n = lattice_modes(N, 256, 1000 + N)
+    ms = ModeSum(N, n)
+    rng = np.random.default_rng(7)
+    amp = torch.as_tensor(rng.uniform(0.2, 1.0, len(n)) * np.exp(2j * np.pi * rng.uniform(size=len(n))), device="cuda")
+    cdt = torch.complex64 if dtype == "c64" else torch.complex128
+    psi = torch.empty((N, N, N), dtype=cdt, device="cuda")
+    ms.fill(amp, psi)
+    sim = wdm.Sim(N, L, mu, 0.0, dtype)
     sim.set_psi(psi)
-    sim.step(3, dt)
-    k2 = sum(v * v for v in k)
-    exact = torch.polar(torch.full_like(ph, A), ph - 0.5 * k2 * 3 * dt)
+    del psi
+    nsteps, dt = 3, 0.37 * (L / N) ** 2
+    sim.step(nsteps, dt)
+    k2 = torch.as_tensor((2 * math.pi / L) ** 2 * (n.astype(np.float64) ** 2).sum(axis=1), device="cuda")
+    amp_t = amp * torch.polar(torch.ones_like(k2), -0.5 * mu * k2 * nsteps * dt)
     out = sim.psi()
-    err = float(torch.linalg.vector_norm((out.to(torch.complex128) - exact).flatten()) / torch.linalg.vector_norm(exact.flatten()))
-    assert err <= 2e-5, err
-    assert float(sim.potential().abs().max()) < 1e-5
-    del psi, exact, out
-    r0, r1 = 2.0, 0.5
-    c = torch.cos(ph)
-    sim.set_psi(torch.sqrt(r0 + r1 * c).to(torch.complex64))
-    sim.step(0, 0.0)
-    phi = sim.potential().double()
-    ref = -r1 * c / k2                                  # 4 pi G = 1
-    assert float(torch.linalg.vector_norm((phi - ref).flatten()) / torch.linalg.vector_norm(ref.flatten())) <= 2e-5
-    del phi, ref, c, ph
-    g = torch.Generator(device="cuda"); g.manual_seed(4)
-    psi = torch.randn((N, N, N, 2), generator=g, device="cuda", dtype=torch.float32) * 0.3
-    psi[..., 0] += 1.0
-    psi = torch.view_as_complex(psi).contiguous()
-    n0 = float((psi.abs().double() ** 2).sum())
+    e, m = ms.compare(amp_t, out)
+    t = tol(dtype, nsteps)
+    assert e <= t and m <= MAXABS * t, (e, m)
+    # and back: the drift is unitary and exactly reversible
+    sim.step(nsteps, -dt)
+    e, m = ms.compare(amp, sim.psi())
+    assert e <= 2 * t and m <= 2 * MAXABS * t, (e, m)
+    sim.close()
+
+
+@pytest.mark.parametrize("dtype,N", BIG)
+def test_multimode_poisson_closed_form(wdm, dtype, N):
+    """rho = r0 + sum_j r_j cos(k_j . x + phi_j)  =>  Phi = -4 pi G sum_j r_j cos(k_j . x + phi_j) / |k_j|^2
+    (Eq. 23; Eq. 18(c)) over the same ~256 lattice modes: the density, real-to-complex,
+    y, z-Green, y and complex-to-real sweeps.  Checked (1) as a field, rel-L2 and max-abs -- dominated by the lowest
+    modes, as Phi is -- and (2) mode by mode: the projection of the library's Phi onto each exp(i k_j . x) against
+    -4 pi G r_j e^{i phi_j} / (2 |k_j|^2), relative to that coefficient, so a wrong Green's-function or Hermitian
+    index at high k cannot hide under the low modes.  complex64 inputs carry the rounding of sqrt(rho) to float32
+    (white, 1.4e-7 per cell): per mode that is 4.5e-12 against r_j >= 2e-4, far below the tolerance."""
+    import torch
+    L, G = 1.3, 30.0
+    n = lattice_modes(N, 256, 2000 + N)
+    # cos needs k and -k: keep one of each +-pair (Nyquist components are their own mirror on the lattice)
+    h = N // 2
+    canon = {}
+    for v in n:
+        key = tuple(int(c) % N for c in v)
+        neg = tuple((-int(c)) % N for c in v)
+        if neg not in canon:
+            canon[key] = v
+    n = np.array(list(canon.values()), dtype=np.int64)
+    # drop modes that equal their own mirror on the lattice (all components 0 or N/2): cos(k.x + phi) then loses its
+    # phase information (it is +-cos(phi) on every node) -- keep the closed form simple
+    n = n[~np.all((n % h) == 0, axis=1)]
+    J = len(n)
+    ms = ModeSum(N, n)
+    rng = np.random.default_rng(9)
+    r = rng.uniform(0.2, 1.0, J) / J
+    ph = rng.uniform(0, 2 * np.pi, J)
+    amp = torch.as_tensor(r * np.exp(1j * ph), device="cuda")
+    cdt = torch.complex64 if dtype == "c64" else torch.complex128
+    psi = torch.empty((N, N, N), dtype=cdt, device="cuda")
+    ms.fill(amp, psi, real_sqrt_offset=2.0)
+    sim = wdm.Sim(N, L, 1.0, G, dtype)
     sim.set_psi(psi)
-    sim.step(2, dt)
-    n1 = float((sim.psi().abs().double() ** 2).sum())
-    assert abs(n1 / n0 - 1) < 1e-5
+    del psi
+    sim.step(0, 0.0)
+    phi = sim.potential()
+    k2 = (2 * math.pi / L) ** 2 * (n.astype(np.float64) ** 2).sum(axis=1)
+    coef = torch.as_tensor(-4 * math.pi * G * r * np.exp(1j * ph) / k2, device="cuda")
+    e, m = ms.compare(coef, phi, real=True)
+    t = tol(dtype, 0)
+    assert e <= t and m <= MAXABS * t, (e, m)
+    c = ms.project(phi)                                   # = coef / 2 for a real field
+    # bound per mode: 2 t of the coefficient itself + the share of white rounding noise at the rel-L2 tolerance that
+    # falls on one of the N^3 modes (t Phi_rms / sqrt(N^3); x4 for the largest of ~250 Rayleigh draws).  float32
+    # rounding of a red spectrum is white, so the highest modes (|coef| ~ 1e-6 of the lowest) sit on that floor.
+    phi_rms = math.sqrt(float((phi.double() ** 2).mean()))
+    bound = 2 * t * (0.5 * coef).abs() + 4 * t * phi_rms / math.sqrt(float(N) ** 3)
+    worst = float(((c - 0.5 * coef).abs() / bound).max())
+    assert worst <= 1.0, worst
+    assert float((4 * t * phi_rms / math.sqrt(float(N) ** 3)) / (0.5 * coef).abs().min()) < 0.05   # the floor stays a small fraction of every coefficient
+    assert abs(float(phi.double().mean())) <= 1e-6 * float(phi.abs().max())
+    sim.close()
+
+
+def test_config4_1024_c64_against_c128(wdm):
+    """BASELINE config 4 itself (1024^3 soliton + 65 536-mode halo, 20 steps, dt = dx^2/6): the float64 oracle would need
+    > 50 GB, so -- SURVEY.md 8(d) (iii) -- the complex64 run is compared with the complex128 run of the same library,
+    whose 1024-point sweeps are pinned by the closed forms above and whose smaller sizes match the oracle to 1e-13.
+    Tolerance: the complex64 budget for 20 steps."""
+    import torch
+    w = wl.config4()
+    N, nsteps = w.N, w.nsteps
+    psi0 = torch.from_numpy(w.psi).cuda()
+    out = {}
+    for dtype in ("c64", "c128"):
+        sim = wdm.Sim(N, w.L, w.hbar_over_m, w.G, dtype)
+        sim.set_psi(psi0)                                   # the complex64 array, upcast exactly for complex128
+        sim.step(nsteps, w.dt)
+        out[dtype] = (sim.psi(), sim.potential())
+        if dtype == "c64":
+            n1 = float((out[dtype][0].abs().double() ** 2).sum())
+            n0 = float((psi0.abs().double() ** 2).sum())
+            assert abs(n1 / n0 - 1) < 1e-5
+        sim.close()
+        del sim
+        torch.cuda.empty_cache()
+    t = tol("c64", nsteps)
+    for i, name in enumerate(("psi", "Phi")):
+        a, b = out["c64"][i], out["c128"][i]
+        num = den = 0.0
+        mx = mb = 0.0
+        for x0 in range(0, N, 64):
+            bb = b[x0:x0 + 64]
+            d = a[x0:x0 + 64].to(bb.dtype) - bb
+            num += float((d.abs() ** 2).sum()); den += float((bb.abs() ** 2).sum())
+            mx = max(mx, float(d.abs().max())); mb = max(mb, float(bb.abs().max()))
+        e = math.sqrt(num / den)
+        assert e <= t, (name, e)
+        assert mx / mb <= MAXABS * t, (name, mx / mb)
+
+
+# ---------------------------------------------------------------- large kick phases (reading G25)
+
+@pytest.mark.parametrize("terms", ["plain", "kappa_layer"])
+@pytest.mark.parametrize("target", [0.2, 0.3, 1.0, 3.0])
+def test_large_phase_kicks_c64(wdm, target, terms):
+    """The float32 kick takes a Taylor pair for |theta| < 1/4 and sincosf above (reading G25; in the fused z sweep the
+    choice is made once per 16-element butterfly).  dt is chosen so that the largest merged-kick phase
+    max|Phi| dt / mu is `target` rad: 0.2 (every butterfly small), 0.3 (butterflies below, above and straddling the
+    threshold), 1 and 3 (mostly sincosf; half kicks of the first step below / above).  Eq. 18(a),(d) PAPER.md:188, 197
+    hold for any dt, and so does the oracle.  One call of 3 steps (fused kicks), then single steps with psi read in
+    between (the elementwise closing half kick, k_kick / k_kick_general)."""
+    N = 64
+    psi0 = (0.3 * wl.random_field(N, "c64", 91) + 1.0).astype(np.complex64)
+    w = wl.Workload(f"bigphase{target}", N, "c64", 3, L=1.3, hbar_over_m=0.8, G=30.0, psi=psi0)
+    sim, o = pair(wdm, w)
+    phimax = float(np.abs(o.potential()).max())
+    dt = target * w.hbar_over_m / phimax
+    # self-interaction phase 30 % of the potential's, a layer that removes a few per cent per step
+    kw = {} if terms == "plain" else dict(kappa=0.3 * phimax / float(np.abs(psi0).max()) ** 2, absorb_alpha=0.05 / dt, absorb_nb=12)
+    sim.set_kick_terms(**kw); o.set_kick_terms(**kw)
+    sim.step(3, dt); o.step(3, dt)
+    check_fields(sim, o, "c64", 3, f"phase {target}")
+    sim.close()
+    sim, o = pair(wdm, w)                                   # fresh start: the map is strongly nonlinear at 3 rad per kick
+    sim.set_kick_terms(**kw); o.set_kick_terms(**kw)
+    for s in range(2):
+        sim.step(1, dt); o.step(1, dt)
+        e = rel(sim.psi().cpu().numpy(), o.psi())          # reading psi applies the pending half kick elementwise
+        assert e <= tol("c64", 1 + s), (s, e)
+    check_fields(sim, o, "c64", 2, f"phase {target}, single steps")
     sim.close()
 
 
@@ -470,11 +682,13 @@ def test_diagnostics_match_oracle(wdm, dtype, N, rtol):
         sim.set_kick_terms(kappa=kappa)
         o.set_kick_terms(kappa=kappa)
         a, b = sim.diagnostics(), o.diagnostics()
+        print("DIAG0", dtype, N, kappa, {k: abs(a[k] - b[k]) / max(abs(b[k]), 1e-300) for k in b})
         for key in ("M", "max_rho", "max_phi", "V", "K", "Q", "dt_max"):
             assert abs(a[key] - b[key]) <= rtol * max(abs(b[key]), 1e-300) * (50 if key in ("max_phi", "V") and dtype == "c64" else 1), (key, a[key], b[key])
     sim.set_kick_terms(); o.set_kick_terms()
     sim.step(2, dt); o.step(2, dt)
     a, b = sim.diagnostics(), o.diagnostics()
+    print("DIAG2", dtype, N, {k: abs(a[k] - b[k]) / max(abs(b[k]), 1e-300) for k in b})
     for key in ("M", "max_rho", "max_phi", "V", "K", "Q", "dt_max"):
         assert abs(a[key] - b[key]) <= 100 * rtol * abs(b[key]), (key, a[key], b[key])
     sim.close()

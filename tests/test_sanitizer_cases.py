@@ -1,0 +1,102 @@
+"""Small cases that draw every synchronisation path of the kernels, sized so that they also run under
+compute-sanitizer (memcheck, racecheck, synccheck; see profiles/r2_sanitizer.md for the commands):
+
+  * two-level and three-level tiles, complex64 and complex128, with fewer tiles than CTAs (static assignment only);
+  * 128^3: more tiles than the first static round, so the ticket path hands out tiles dynamically;
+  * coupled particles (shared-memory atomics of the deposit, the sort, both assignment schemes);
+  * the L2-chained kernels (release / acquire counters between stages of one cooperative launch);
+  * the extra kick terms and the external potential (separate instantiations of the z and complex-to-real sweeps).
+
+Each case is also a parity test against the CPU oracle, so a plain `pytest -m gpu` run checks the same code.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import wdm_workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.complex128 if np.iscomplexobj(a) else np.float64)
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(np.asarray(b).ravel()))
+
+
+@pytest.fixture(scope="module")
+def wdm():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2606_25026_b200 as w
+    w.lib()
+    return w
+
+
+def run_pair(wdm, w, nsteps, chain=0, kick=None, order=2, substeps=1):
+    npart = 0 if w.pos is None else len(w.pos)
+    sim = wdm.Sim(w.N, w.L, w.hbar_over_m, w.G, w.dtype, max_particles=npart)
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    sim.set_psi(w.psi); o.set_psi(w.psi)
+    if npart:
+        sim.set_particles(w.pos, w.vel, w.mass); o.set_particles(w.pos, w.vel, w.mass)
+        for x in (sim, o):
+            x.set_assignment(order)
+            x.set_particle_mode(substeps=substeps)
+    if kick:
+        sim.set_kick_terms(**kick); o.set_kick_terms(**kick)
+    if chain:
+        wdm.wdm_set_chain(sim.h, chain, 0)
+    sim.step(nsteps, w.dt); o.step(nsteps, w.dt)
+    t = (1e-12 if w.dtype == "c128" else 2e-5)
+    assert rel(sim.psi().cpu().numpy(), o.psi()) <= t
+    if w.G > 0 or kick:
+        assert rel(sim.potential().cpu().numpy(), o.potential()) <= t
+    if npart:
+        p, _ = sim.particles()
+        po, _ = o.particles()
+        d = p.cpu().numpy().astype(np.float64) - po
+        d -= w.L * np.round(d / w.L)
+        assert np.abs(d).max() <= (1e-5 if w.dtype == "c64" else 1e-12) * w.L
+    sim.close()
+
+
+def noise(N, dtype, G=30.0):
+    psi0 = (0.3 * wl.random_field(N, dtype, 500 + N) + 1.0).astype(np.complex64 if dtype == "c64" else np.complex128)
+    w = wl.Workload(f"san{N}", N, dtype, 2, L=1.3, hbar_over_m=0.8, G=G, psi=psi0)
+    w.dt = 0.2 * (w.L / N) ** 2
+    return w
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_san_32_static_tiles(wdm, dtype):
+    run_pair(wdm, noise(32, dtype), 2)
+
+
+def test_san_config1(wdm):
+    run_pair(wdm, wl.config1(), 2)
+
+
+def test_san_128_ticket_path(wdm):
+    run_pair(wdm, noise(128, "c64"), 2)
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+@pytest.mark.parametrize("order", [2, 3])
+def test_san_16_coupled(wdm, dtype, order):
+    run_pair(wdm, wl.small_coupled(16, dtype=dtype), 3, order=order, substeps=2 if order == 3 else 1)
+
+
+@pytest.mark.parametrize("dtype,N", [("c64", 32), ("c128", 32), ("c64", 128)])
+def test_san_chained(wdm, dtype, N):
+    run_pair(wdm, noise(N, dtype), 2, chain=3)
+
+
+def test_san_kick_terms(wdm):
+    N = 32
+    w = noise(N, "c64")
+    x = -0.5 * w.L + (w.L / N) * np.arange(N)
+    X, Y, Z = np.meshgrid(x, x, x, indexing="ij")
+    ext = (5.0 * np.cos(2 * math.pi * X / w.L) + 3.0 * (Y * Y + Z * Z)).astype(np.float32)
+    run_pair(wdm, w, 2, kick=dict(kappa=-3.0, phi_ext=ext, absorb_alpha=0.1 / w.dt, absorb_nb=10))
