@@ -45,6 +45,7 @@ def lib():
             "wdmo_get_potential": [vp, dp], "wdmo_get_particles": [vp, dp, dp],
             "wdmo_get_accel": [vp, dp], "wdmo_threads": [],
             "wdmo_set_kick_terms": [vp, d, dp, d, i], "wdmo_diagnostics": [vp, dp], "wdmo_set_particle_mode": [vp, i, i],
+            "wdmo_set_step_diagnostics": [vp, i], "wdmo_step_diagnostics": [vp, dp],
         }
         for name, args in sig.items():
             fn = getattr(_lib, name)
@@ -200,10 +201,21 @@ class Oracle:
         _check(lib().wdmo_set_assignment(self._h, int(order)), "set_assignment")
 
     def diagnostics(self):
-        """dict(M, max_rho, max_phi, V, K, Q, dt_max) of the current state (Sect. 3.5-3.6; central differences)."""
-        out = np.zeros(8)
+        """dict(M, max_rho, max_phi, V, K, Q, dt_max, T, W, E) of the current state (Sect. 3.5-3.6): K, Q by central
+        differences, T spectral, W = V/2, E = T + W."""
+        out = np.zeros(12)
         _check(lib().wdmo_diagnostics(self._h, _dp(out)), "diagnostics")
-        return dict(zip(("M", "max_rho", "max_phi", "V", "K", "Q", "dt_max"), out[:7]))
+        return dict(zip(("M", "max_rho", "max_phi", "V", "K", "Q", "dt_max", "T", "W", "E"), out[:10]))
+
+    def set_step_diagnostics(self, on=True):
+        _check(lib().wdmo_set_step_diagnostics(self._h, 1 if on else 0), "set_step_diagnostics")
+
+    def step_diagnostics(self):
+        """dict(M, max_rho, max_phi, T, W, Tx, Ty, Tz) of the field between the drift and the closing half kick of the
+        last step (recorded while set_step_diagnostics is on)."""
+        out = np.zeros(8)
+        _check(lib().wdmo_step_diagnostics(self._h, _dp(out)), "step_diagnostics")
+        return dict(zip(("M", "max_rho", "max_phi", "T", "W", "Tx", "Ty", "Tz"), out))
 
     def particles(self):
         pos = np.empty((self.np_, 3)); vel = np.empty((self.np_, 3))

@@ -64,6 +64,10 @@ typedef struct wdmo_ctx {
     int nsub;            /* leapfrog sub-steps per SPE step (>= 1)                              */
     int pstatic;         /* :particles_static -- particles never move, they only source Phi    */
     int order;           /* mass assignment / force interpolation: 2 = cloud-in-cell, 3 = TSC   */
+    /* per-step diagnostics, recorded between (c) and (d) of the last step when switched on */
+    int step_diag_on, step_diag_valid;
+    double step_diag[8];
+    double *phi_grav;    /* Poisson potential before Phi_ext is added (only kept while step_diag_on)          */
 } wdmo_ctx;
 
 static int is_pow2(int n) { return n >= 1 && (n & (n - 1)) == 0; }
@@ -430,7 +434,7 @@ int wdmo_destroy(wdmo_ctx *c)
     if (!c) return WDMO_OK;
     free(c->psi); free(c->work); free(c->rho); free(c->phi);
     free(c->pos); free(c->vel); free(c->acc); free(c->mass);
-    free(c->phi_ext);
+    free(c->phi_ext); free(c->phi_grav);
     free(c);
     return WDMO_OK;
 }
@@ -482,6 +486,7 @@ static int update_potential(wdmo_ctx *c)
     if (c->np > 0) assign_deposit(c, c->rho);
     int rc = poisson(c->rho, c->phi, c->work, c->N, c->L, c->G);
     if (rc) return rc;
+    if (c->step_diag_on) memcpy(c->phi_grav, c->phi, c->n * sizeof(double));
     /* Phi_total = Phi_DM + Phi_ext (Alg. 1 l.15); particles feel the total as well (G27) */
     if (c->phi_ext)
         for (size_t i = 0; i < c->n; ++i) c->phi[i] += c->phi_ext[i];
@@ -606,6 +611,83 @@ int wdmo_set_kick_terms(wdmo_ctx *c, double kappa, const double *phi_ext, double
     return WDMO_OK;
 }
 
+/* Spectral kinetic energy of the field in c->psi, per axis (Sect. 2.3: the kinetic term of Eq. 1 is
+ * -(mu^2/2) psi* lap psi per unit m; in Fourier space lap -> -k^2, pseudo-spectral as in Eq. 18(b)):
+ *   T_a = (mu^2/2) sum_k k_a^2 |psi~_k|^2 dV / N^3,   psi~ = DFT3(psi) unnormalised (Parseval: sum_x |psi|^2 = sum_k |psi~|^2 / N^3)
+ * T = T_x + T_y + T_z equals K + Q of wdmo_diagnostics in the continuum limit (Eq. 11-12).
+ * Uses c->work as scratch (free outside poisson()). */
+static int spectral_kinetic(wdmo_ctx *c, double T[3])
+{
+    int N = c->N;
+    memcpy(c->work, c->psi, sizeof(cplx) * c->n);
+    int rc = fft3_inplace(c->work, N, -1);
+    if (rc) return rc;
+    double t[3] = {0, 0, 0};
+    for (int ix = 0; ix < N; ++ix) {
+        double kx = wavenumber(ix, N, c->L);
+        for (int iy = 0; iy < N; ++iy) {
+            double ky = wavenumber(iy, N, c->L);
+            for (int iz = 0; iz < N; ++iz) {
+                double kz = wavenumber(iz, N, c->L);
+                cplx v = c->work[((size_t)ix * N + iy) * N + iz];
+                double a2 = creal(v) * creal(v) + cimag(v) * cimag(v);
+                t[0] += kx * kx * a2; t[1] += ky * ky * a2; t[2] += kz * kz * a2;
+            }
+        }
+    }
+    double f = 0.5 * c->mu * c->mu * c->dx * c->dx * c->dx / ((double)N * N * N);
+    for (int a = 0; a < 3; ++a) T[a] = f * t[a];
+    return WDMO_OK;
+}
+
+/* Diagnostics of the state between steps (c) and (d) of Eq. 18: psi_2 (after the drift, before the
+ * closing half kick), the source rho = |psi_2|^2 + particles and the potential just solved from it.  These are the
+ * quantities a fused GPU step has in hand without another pass over the grid:
+ *   [0] M = sum |psi_2|^2 dV      [1] max |psi_2|^2      [2] max |Phi_total|   (Eq. 26 PAPER.md:364-368 needs both maxima)
+ *   [3] T = T_x + T_y + T_z of psi_2 (spectral; the drift multiplies psi~ by unit-modulus factors, so T is the same
+ *       before and after step (b))     [4] W = 1/2 sum rho Phi_grav dV, rho the whole Poisson source, Phi_grav the
+ *       Poisson potential of Eq. 23 (without Phi_ext)     [5..7] T_x, T_y, T_z
+ * E = T + W is the conserved energy of the pure SPE (the 1/2 in W is what makes it conserved, P6). */
+static int record_step_diag(wdmo_ctx *c)
+{
+    double T[3], M = 0, W = 0, maxrho = 0, maxphi = 0, dV = c->dx * c->dx * c->dx;
+    int rc = spectral_kinetic(c, T);
+    if (rc) return rc;
+    for (size_t i = 0; i < c->n; ++i) {
+        double re = creal(c->psi[i]), im = cimag(c->psi[i]), r = re * re + im * im;
+        M += r;
+        if (r > maxrho) maxrho = r;
+        if (fabs(c->phi[i]) > maxphi) maxphi = fabs(c->phi[i]);
+        W += 0.5 * c->rho[i] * c->phi_grav[i];
+    }
+    c->step_diag[0] = M * dV; c->step_diag[1] = maxrho; c->step_diag[2] = maxphi;
+    c->step_diag[3] = T[0] + T[1] + T[2]; c->step_diag[4] = W * dV;
+    c->step_diag[5] = T[0]; c->step_diag[6] = T[1]; c->step_diag[7] = T[2];
+    c->step_diag_valid = 1;
+    return WDMO_OK;
+}
+
+int wdmo_set_step_diagnostics(wdmo_ctx *c, int on)
+{
+    if (!c) return WDMO_EINVAL;
+    c->step_diag_on = on != 0;
+    c->step_diag_valid = 0;
+    if (on && !c->phi_grav) {
+        c->phi_grav = (double *)malloc(c->n * sizeof(double));
+        if (!c->phi_grav) return WDMO_ENOMEM;
+    }
+    return WDMO_OK;
+}
+
+/* WDMO_ESTATE until a step has run with the recording switched on */
+int wdmo_step_diagnostics(wdmo_ctx *c, double *out)
+{
+    if (!c || !out) return WDMO_EINVAL;
+    if (!c->step_diag_valid) return WDMO_ESTATE;
+    memcpy(out, c->step_diag, sizeof c->step_diag);
+    return WDMO_OK;
+}
+
 int wdmo_step(wdmo_ctx *c, int nsteps, double dt)
 {
     if (!c || nsteps < 0) return WDMO_EINVAL;
@@ -617,6 +699,7 @@ int wdmo_step(wdmo_ctx *c, int nsteps, double dt)
         if (rc) return rc;
         rc = update_potential(c);               /* (c) rho, Phi^{n+1}, a^{n+1}               */
         if (rc) return rc;
+        if (c->step_diag_on && s == nsteps - 1 && (rc = record_step_diag(c))) return rc;
         half_kick(c, 0.5 * dt);                 /* (d) with the new Phi + closing half kick  */
         if (c->alpha > 0) absorb(c, dt);        /* Alg. 1 l.17-18                            */
     }
@@ -675,6 +758,14 @@ int wdmo_get_accel(wdmo_ctx *c, double *acc)
  *   out[5] Q     = mu^2/2 sum |grad sqrt(rho)|^2 dx^3              (Eq. 12 with its hbar^2/2m prefactor, per unit m)
  *   out[6] dt_max of Eq. 26 without the safety factor:
  *          0.5 min{ 4/(3 pi) dx^2/mu, 2 pi mu / max|Phi|, 2 pi mu / (|kappa| max|psi|^2) }
+ *   out[7] T     = mu^2/2 sum_k k^2 |psi~_k|^2 dx^3 / N^3          (spectral kinetic energy; = K + Q in the continuum)
+ *   out[8] W     = 1/2 sum rho Phi dx^3 = V/2                      (the 1/2 that makes E conserved, reading G31)
+ *   out[9] E     = T + W                                           (conserved by the pure SPE)
+ *   out[10], out[11] reserved (0)
+ * Which virial identity the numbers satisfy: the paper prints 2K + 2Q + V = 0 with Q = int |grad sqrt(rho)|^2 and
+ * V = int rho Phi; with the hbar^2/2m of Eq. 12 kept in Q and the self-energy counted once
+ * (W = V/2) the stationary-state identity of the SPE reads 2 (K + Q) + W = 2 T + W = 0 for the returned K, Q, W
+ * (reading G31 in DESIGN.md).
  * Phi is refreshed first if stale. */
 int wdmo_diagnostics(wdmo_ctx *c, double *out)
 {
@@ -713,7 +804,13 @@ int wdmo_diagnostics(wdmo_ctx *c, double *out)
     if (maxphi > 0 && 2.0 * M_PI * mu / maxphi < dtm) dtm = 2.0 * M_PI * mu / maxphi;
     if (c->kappa != 0 && maxrho > 0 && 2.0 * M_PI * mu / (fabs(c->kappa) * maxrho) < dtm) dtm = 2.0 * M_PI * mu / (fabs(c->kappa) * maxrho);
     out[6] = 0.5 * dtm;
-    out[7] = 0;
+    double T[3];
+    rc = spectral_kinetic(c, T);
+    if (rc) return rc;
+    out[7] = T[0] + T[1] + T[2];
+    out[8] = 0.5 * out[3];
+    out[9] = out[7] + out[8];
+    out[10] = out[11] = 0;
     return WDMO_OK;
 }
 

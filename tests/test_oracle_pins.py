@@ -610,3 +610,95 @@ def test_p16_tsc_zero_self_force_momentum_and_context_switch():
     assert np.max(np.abs(a2 - a3)) > 1e-3 * np.max(np.abs(a2))
     with pytest.raises(Exception):
         o.set_assignment(4)
+
+
+# ---------------------------------------------------------------- P17: spectral kinetic energy, W, E, per-step diagnostics
+
+def test_p17_spectral_kinetic_energy_plane_waves_closed_form():
+    """psi = sum_j A_j e^{i k_j . x}, distinct lattice k_j: T_a = (mu^2/2) sum_j k_ja^2 |A_j|^2 L^3 exactly (orthogonality),
+    including a Nyquist component (index N/2 <-> s = -N/2, reading G4: k^2 is sign-blind)."""
+    N, L, mu = 16, 1.3, 0.7
+    X, Y, Z = grid(N, L)
+    ns = np.array([[2, -1, 3], [0, 5, -4], [-7, 0, 8], [1, 1, 0]])
+    A = np.array([0.8, 0.5 - 0.2j, 0.3j, 1.1])
+    k = 2 * np.pi * ns / L
+    psi = sum(a * np.exp(1j * (kk[0] * X + kk[1] * Y + kk[2] * Z)) for a, kk in zip(A, k))
+    o = oracle.Oracle(N, L, mu, 0.0)
+    o.set_psi(psi)
+    d = o.diagnostics()
+    Ta = 0.5 * mu * mu * (np.abs(A)[:, None] ** 2 * k ** 2).sum(axis=0) * L ** 3
+    assert abs(d["T"] - Ta.sum()) < 1e-10 * Ta.sum()
+    assert d["W"] == 0.5 * d["V"] and abs(d["E"] - (d["T"] + d["W"])) < 1e-15 * abs(d["E"])
+    # per axis, and unchanged by a drift (G = 0: the step is Eq. 18(b) alone, unit-modulus factors in k-space)
+    o.set_step_diagnostics(True)
+    o.step(1, 0.37 * (L / N) ** 2)
+    s = o.step_diagnostics()
+    for a, key in enumerate(("Tx", "Ty", "Tz")):
+        assert abs(s[key] - Ta[a]) < 1e-10 * Ta.sum()
+    assert abs(s["T"] - Ta.sum()) < 1e-10 * Ta.sum() and abs(o.diagnostics()["T"] - Ta.sum()) < 1e-10 * Ta.sum()
+    assert abs(s["M"] - (np.abs(A) ** 2).sum() * L ** 3) < 1e-10
+
+
+def test_p17_T_equals_K_plus_Q_in_the_continuum_limit():
+    """T (spectral) and K + Q (central differences, Eq. 21) are the same integral (Eq. 11-12 PAPER.md:118-128 with the
+    hbar^2/2m prefactors): for a smooth moving Gaussian the difference falls by 4 per halving of dx, and
+    T -> (mu^2/2) (|k0|^2 + 3/(4 s^2)) M for psi = exp(-r^2/(4 s^2) + i k0 . x)."""
+    L, mu, s = 1.0, 0.9, 0.07
+    k0 = 2 * np.pi * np.array([2, -1, 1]) / L
+    diffs = []
+    for N in (16, 32, 64):
+        X, Y, Z = grid(N, L)
+        psi = np.exp(-(X ** 2 + Y ** 2 + Z ** 2) / (4 * s * s) + 1j * (k0[0] * X + k0[1] * Y + k0[2] * Z))
+        o = oracle.Oracle(N, L, mu, 0.0)
+        o.set_psi(psi)
+        d = o.diagnostics()
+        diffs.append(abs(d["T"] - (d["K"] + d["Q"])) / d["T"])
+    assert diffs[2] < 0.02 and 3.3 < diffs[1] / diffs[2] < 4.7, diffs
+    M = (2 * np.pi * s * s) ** 1.5
+    assert abs(d["T"] - 0.5 * mu * mu * (k0 @ k0 + 3 / (4 * s * s)) * M) < 1e-6 * d["T"]     # spectral: exact up to the periodic images
+
+
+def test_p17_energy_from_diagnostics_matches_numpy_and_is_second_order():
+    """E = T + W of wdmo_diagnostics against the numpy.fft evaluation of P6 (a library routine used as a check OF
+    the oracle), and its drift over a fixed time falls by 4 per halving of dt."""
+    N, L, mu, G = 16, 1.0, 1.0, 200.0 / FOUR_PI
+    X, Y, Z = grid(N, L)
+    psi0 = (2.0 + np.exp(2j * np.pi * X) + 0.7 * np.exp(2j * np.pi * (Y - Z)) + 0.4 * np.cos(2 * np.pi * Z)).astype(complex)
+    Tend, drifts = 0.02, []
+    for ns in (8, 16, 32):
+        o = oracle.Oracle(N, L, mu, G); o.set_psi(psi0)
+        e0 = o.diagnostics()["E"]
+        assert abs(e0 - total_energy(o.psi(), o.potential(), L, mu)) < 1e-12 * abs(e0)
+        o.step(ns, Tend / ns)
+        drifts.append(abs(o.diagnostics()["E"] - e0) / abs(e0))
+    assert 3.5 < drifts[0] / drifts[1] < 4.5 and 3.5 < drifts[1] / drifts[2] < 4.5, drifts
+
+
+def test_p17_step_diagnostics_are_those_of_psi2():
+    """The per-step record belongs to psi_2 = the field between Eq. 18(c) and (d).  Undo the closing half kick of the
+    last step by hand (psi_2 = psi exp(+i Phi dt / 2 mu), |psi| unchanged, so rho and Phi are those of the end state)
+    and hand psi_2 to a fresh oracle: its diagnostics must be the record."""
+    N, L, mu, G = 16, 1.3, 0.8, 60.0 / FOUR_PI
+    X, Y, Z = grid(N, L)
+    psi0 = (1.5 + np.exp(2j * np.pi * X / L) + 0.6 * np.exp(2j * np.pi * (2 * Y - Z) / L)).astype(complex)
+    dt = 0.3 * (L / N) ** 2
+    o = oracle.Oracle(N, L, mu, G); o.set_psi(psi0)
+    with pytest.raises(RuntimeError):
+        o.step_diagnostics()                              # nothing recorded yet
+    o.set_step_diagnostics(True)
+    o.step(3, dt)
+    s = o.step_diagnostics()
+    psi2 = o.psi() * np.exp(1j * o.potential() * dt / (2 * mu))
+    o2 = oracle.Oracle(N, L, mu, G); o2.set_psi(psi2)
+    d = o2.diagnostics()
+    for key in ("M", "max_rho", "max_phi", "T", "W"):
+        assert abs(s[key] - d[key]) <= 1e-11 * abs(d[key]), (key, s[key], d[key])
+    assert abs(s["Tx"] + s["Ty"] + s["Tz"] - s["T"]) < 1e-12 * s["T"]
+    # with particles W counts the whole source: 1/2 sum (|psi|^2 + rho_p) Phi
+    w = wl.small_coupled(16)
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G); o.set_psi(w.psi); o.set_particles(w.pos, w.vel, w.mass)
+    o.set_step_diagnostics(True)
+    o.step(2, w.dt)
+    s = o.step_diagnostics()
+    W = 0.5 * float(np.sum(o.density() * o.potential())) * (w.L / w.N) ** 3
+    assert abs(s["W"] - W) < 1e-12 * abs(W)
