@@ -719,7 +719,14 @@ int wdmo_get_density(wdmo_ctx *c, double *out)
     if (!c || !out) return WDMO_EINVAL;
     int rc = refresh(c);
     if (rc) return rc;
-    memcpy(out, c->rho, sizeof(double) * c->n);
+    /* |psi|^2 of the psi that wdmo_get_psi returns, plus the particles (reading G22).  Without an absorbing layer this
+     * is the source of the last Poisson solve (a kick leaves |psi| unchanged); with one (Alg. 1 l.17-18 masks psi AFTER
+     * the potential of l.13 was solved) it is the density of the attenuated field, while Phi stays the one of l.13. */
+    for (size_t i = 0; i < c->n; ++i) {
+        double re = creal(c->psi[i]), im = cimag(c->psi[i]);
+        out[i] = re * re + im * im;
+    }
+    if (c->np > 0) assign_deposit(c, out);
     return WDMO_OK;
 }
 

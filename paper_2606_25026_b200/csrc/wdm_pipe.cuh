@@ -780,9 +780,15 @@ struct C2RK {
         const cx<T> *R = reinterpret_cast<const cx<T> *>(buf + PACKED_BYTES);
         const TL tile(p, t);
         // Z_k = A_k + i B_k,  Z_{N-k} = conj(A_k) + i conj(B_k)
+        // Rows kx = 0 and kx = N/2 are the x-spectrum of REAL lines at a self-mirrored frequency: real in exact
+        // arithmetic.  What rounding leaves in their imaginary parts (Hermitian asymmetry of the y, z transforms,
+        // amplified by 1/k^2 at low k) must not enter: B's would land on line 2l', A's on line 2l'+1 -- with opposite
+        // signs on adjacent z, i.e. folded onto the mode at the z-Nyquist mirror (measured at 512^3 complex64: 2e-3 of
+        // the coefficient of (0, 0, 255), N^2-growing).  As in any complex-to-real transform they are ignored.
         auto place = [&](int k, int e, int en, int l) {
             cx<T> A, B;
             ld2(R + k * W + 2 * l, A, B);
+            if (k == 0 || k == N / 2) A.y = B.y = (T)0;
             Sp[e] = mk<T>(A.x - B.y, A.y + B.x);
             if (k > 0 && k < N / 2) Sp[en] = mk<T>(A.x + B.y, B.x - A.y);
         };

@@ -702,3 +702,18 @@ def test_p17_step_diagnostics_are_those_of_psi2():
     s = o.step_diagnostics()
     W = 0.5 * float(np.sum(o.density() * o.potential())) * (w.L / w.N) ** 3
     assert abs(s["W"] - W) < 1e-12 * abs(W)
+
+
+def test_density_getter_is_that_of_the_returned_psi_with_a_layer():
+    """Reading G22: wdmo_get_density = |psi|^2 of the psi the getter returns (+ particles).  With the absorbing layer of
+    Alg. 1 l.17-18 that is the attenuated field; Phi stays the potential solved at l.13 from the un-attenuated one."""
+    w = wl.small_coupled(16)
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    o.set_psi(w.psi); o.set_particles(w.pos, w.vel, w.mass)
+    o.set_kick_terms(absorb_alpha=0.2 / w.dt, absorb_nb=8)
+    o.step(2, w.dt)
+    pos, _ = o.particles()
+    want = np.abs(o.psi()) ** 2 + oracle.cic_deposit(w.N, w.L, pos, w.mass)
+    assert relerr(o.density(), want) < 1e-14
+    # the potential is NOT that of the attenuated field
+    assert relerr(o.potential(), oracle.poisson(want, w.L, w.G)) > 1e-4
