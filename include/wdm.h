@@ -125,6 +125,15 @@ int wdm_set_particle_mode(wdm_ctx *ctx, int substeps, int is_static);
 int wdm_set_assignment(wdm_ctx *ctx, int order);
 int wdm_get_assignment(wdm_ctx *ctx, int *order);
 
+/* Arithmetic of the particle deposit.  0 (default): floating-point atomics in shared and global memory -- the sum over
+ * the particles of a node depends on their order, so the coupled result is reproducible only to rounding (1e-7
+ * relative in complex64).  1: every weight is rounded once to 64-bit fixed point (a power-of-two scale chosen from the
+ * total particle mass) and accumulated with integer atomics: the mesh, hence the whole coupled run, is bit-identical from
+ * run to run (a debugging mode: 8 bytes per cell of extra device memory, cudaMalloc'ed on first use -- WDM_ENOMEM if that
+ * fails -- a conversion pass per step, and one host synchronisation per particle set).  Either way the deposit is the
+ * cloud-in-cell / triangular-shaped-cloud sum of PAPER.md:314 (readings G12, G30).  Marks the potential stale. */
+int wdm_set_deposit_mode(wdm_ctx *ctx, int deterministic);
+
 /* Diagnostics of the current state (Sect. 3.5-3.6) by one reduction pass on the device; the
  * gradients are the second-order central differences of Eq. 21.  Synchronises the stream.
  * out_host[0] M = sum |psi|^2 dx^3       [1] max |psi|^2       [2] max |Phi_total|

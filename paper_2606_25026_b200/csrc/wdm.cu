@@ -8,6 +8,7 @@
 //   H sweep y forward, H sweep z forward . Green . inverse, H sweep y inverse, x complex-to-real -> Phi
 // The closing half kick of the call stays pending: the next wdm_step folds it into its opening kick, a read of the
 // state applies it (flush_pending).  Nothing synchronises with the host.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -75,26 +76,52 @@ __global__ void k_density(const cx<T> *psi, const T *rho_p, T *out, size_t n)
     }
 }
 
-// <rho> = (sum |psi|^2)/N^3 + (sum m_p)/L^3, accumulated in double: acc[0] grid sum, acc[1] particle mass
+// <rho> = (sum |psi|^2)/N^3 + (sum m_p)/L^3 in double, in a FIXED order (per-thread strided sums, warp shuffles, one
+// partial per block, then one block over the partials): no atomics, so the mean -- and with it every bit of a pure SPE
+// run -- is reproducible from run to run.
+constexpr int kSumBlocks = 148 * 4;
+
+__device__ __forceinline__ double block_sum_256(double s)
+{
+    __shared__ double part[8];
+    for (int d = 16; d; d >>= 1) s += __shfl_down_sync(0xffffffffu, s, d);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __syncthreads();
+    double t = 0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < 8; ++w) t += part[w];
+    __syncthreads();
+    return t;          // valid in thread 0
+}
+
 template <typename T>
-__global__ void k_sum_density(const cx<T> *psi, size_t n, double *acc)
+__global__ void __launch_bounds__(256) k_sum_density(const cx<T> *psi, size_t n, double *partial)
 {
     double s = 0;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         cx<T> v = ldv(psi + i);
         s += (double)v.x * v.x + (double)v.y * v.y;
     }
-    for (int d = 16; d; d >>= 1) s += __shfl_down_sync(0xffffffffu, s, d);
-    if ((threadIdx.x & 31) == 0) atomicAdd(acc, s);
+    s = block_sum_256(s);
+    if (threadIdx.x == 0) partial[blockIdx.x] = s;
 }
 
 template <typename T>
-__global__ void k_sum_mass(const T *mass, long long n, double *acc)
+__global__ void __launch_bounds__(256) k_sum_mass(const T *mass, long long n, double *partial)
 {
     double s = 0;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) s += mass[i];
-    for (int d = 16; d; d >>= 1) s += __shfl_down_sync(0xffffffffu, s, d);
-    if ((threadIdx.x & 31) == 0) atomicAdd(acc + 1, s);
+    s = block_sum_256(s);
+    if (threadIdx.x == 0) partial[blockIdx.x] = s;
+}
+
+// acc[slot] = sum of partial[0 .. nb) (one block of 256 threads)
+__global__ void __launch_bounds__(256) k_sum_partials(const double *partial, int nb, double *acc, int slot)
+{
+    double s = 0;
+    for (int i = threadIdx.x; i < nb; i += 256) s += partial[i];
+    s = block_sum_256(s);
+    if (threadIdx.x == 0) acc[slot] = s;
 }
 
 template <typename T>
@@ -186,6 +213,11 @@ struct wdm_ctx {
     int absorb_nb = 50;
     const void *phi_ext = nullptr;            // library-owned copy of the caller's N^3 reals (phi_ext_buf) or nullptr
     void *phi_ext_buf = nullptr;              // cudaMalloc'ed on the first wdm_set_kick_terms with an external potential
+    // deterministic deposit (wdm_set_deposit_mode): N^3 64-bit accumulators, cudaMalloc'ed on first use; upper bound of
+    // the total particle mass (0 = not measured for the current particle set)
+    bool deposit_fixed = false;
+    unsigned long long *deposit_acc = nullptr;
+    double deposit_mass = 0;
     void *mask = nullptr;                     // 3 N axis factors exp(-alpha b dt) for mask_dt
     double mask_dt = 0;
     bool mask_valid = false;
@@ -432,6 +464,7 @@ static SweepParams<T> base_params(wdm_ctx *c)
     p.phi = (const T *)c->phi;
     p.phi_out = (T *)c->phi;
     p.rho_p = c->part.n > 0 ? (const T *)c->part.rho_p : nullptr;
+    p.rho_flag = c->part.flag;
     p.rho_mean = (const T *)((const unsigned char *)c->rho_mean + 16);
     p.phi_ext = (const T *)c->phi_ext;
     return p;
@@ -474,7 +507,32 @@ template <typename T>
 static int particles_deposit(wdm_ctx *c)
 {
     if (c->part.n == 0) return WDM_OK;
-    { Timed t(c, S_PART_CLEAR); CU(c, cudaMemsetAsync(c->part.rho_p, 0, c->n * sizeof(T), c->stream)); }
+    if (c->deposit_fixed) {
+        if (!c->deposit_acc) {
+            cudaError_t e = cudaMalloc(&c->deposit_acc, c->n * sizeof(unsigned long long));
+            if (e != cudaSuccess) { cudaGetLastError(); c->deposit_acc = nullptr; return fail(c, WDM_ENOMEM, "cudaMalloc of the fixed-point deposit mesh (%zu bytes): %s", c->n * 8, cudaGetErrorString(e)); }
+            CU(c, cudaMemsetAsync(c->deposit_acc, 0, c->n * sizeof(unsigned long long), c->stream));
+        }
+        if (c->deposit_mass == 0) {
+            // bound of the total mass, needed once per particle set for the fixed-point scale (host synchronisation)
+            if (!c->part.has_mass) c->deposit_mass = fabs(c->part.mass_scalar) * (double)c->part.n;
+            else {
+                double *acc = (double *)c->rho_mean, h[2];
+                const int nb = (int)std::min<long long>(148, (c->part.n + 255) / 256);
+                k_sum_mass<T><<<nb, 256, 0, c->stream>>>((const T *)c->part.mass, c->part.n, (double *)c->H);
+                k_sum_partials<<<1, 256, 0, c->stream>>>((const double *)c->H, nb, acc, 1);
+                CU(c, cudaMemcpyAsync(h, acc, 16, cudaMemcpyDeviceToHost, c->stream));
+                CU(c, cudaStreamSynchronize(c->stream));
+                c->deposit_mass = fabs(h[1]) * 1.001;          // the scale is a power of two: the last bits of this sum do not matter
+            }
+            if (!(c->deposit_mass > 0)) c->deposit_mass = 1.0;
+        }
+        Timed t(c, S_PART_DEPOSIT);
+        c->launches += 1;
+        CU(c, particle_deposit_fixed(c->part, c->N, c->L, c->dtype, c->deposit_acc, c->deposit_mass, c->stream));
+        return WDM_OK;
+    }
+    { Timed t(c, S_PART_CLEAR); CU(c, particle_mesh_clear(c->part, c->N, c->dtype, c->stream)); }
     Timed t(c, S_PART_DEPOSIT);
     CU(c, particle_deposit(c->part, c->N, c->L, c->dtype, c->stream));
     return WDM_OK;
@@ -486,15 +544,21 @@ static int refresh(wdm_ctx *c)
     if (!c->have_psi) return fail(c, WDM_ESTATE, "wdm_set_psi has not been called");
     if (!c->stale) return WDM_OK;
     if (c->G > 0) {
-        {   // <rho> of the current state (conserved afterwards): see the density sweep
-            double *acc = (double *)c->rho_mean;
+        {   // <rho> of the current state (conserved afterwards): see the density sweep.  Block partials go to the head
+            // of H, which is dead until the density sweep writes it
+            double *acc = (double *)c->rho_mean, *partial = (double *)c->H;
             Timed t(c, S_MISC);
             CU(c, cudaMemsetAsync(acc, 0, 16, c->stream));
-            k_sum_density<T><<<148 * 4, 256, 0, c->stream>>>((const cx<T> *)c->psi, c->n, acc);
+            int nb = (int)std::min<size_t>(kSumBlocks, (c->n + 255) / 256);
+            k_sum_density<T><<<nb, 256, 0, c->stream>>>((const cx<T> *)c->psi, c->n, partial);
+            k_sum_partials<<<1, 256, 0, c->stream>>>(partial, nb, acc, 0);
             double extra = 0;
             if (c->part.n > 0) {
-                if (c->part.has_mass) k_sum_mass<T><<<148, 256, 0, c->stream>>>((const T *)c->part.mass, c->part.n, acc);
-                else extra = c->part.mass_scalar * (double)c->part.n;
+                if (c->part.has_mass) {
+                    nb = (int)std::min<long long>(148, (c->part.n + 255) / 256);
+                    k_sum_mass<T><<<nb, 256, 0, c->stream>>>((const T *)c->part.mass, c->part.n, partial);
+                    k_sum_partials<<<1, 256, 0, c->stream>>>(partial, nb, acc, 1);
+                } else extra = c->part.mass_scalar * (double)c->part.n;
             }
             k_finish_mean<T><<<1, 1, 0, c->stream>>>(acc, 1.0 / (double)c->n, extra, 1.0 / (c->L * c->L * c->L),
                                                       (T *)((unsigned char *)c->rho_mean + 16));
@@ -715,6 +779,7 @@ extern "C" int wdm_destroy(wdm_ctx *c)
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     for (void *p : c->owned) cudaFree(p);
     if (c->phi_ext_buf) cudaFree(c->phi_ext_buf);
+    if (c->deposit_acc) cudaFree(c->deposit_acc);
     delete c;
     return WDM_OK;
 }
@@ -772,6 +837,7 @@ static int set_particles(wdm_ctx *c, long long n, const void *pos, const void *v
         particle_bind(c->part, c->N, c->dtype, n, rho_p, pm);
     }
     c->launches += 3;
+    c->deposit_mass = 0;
     cudaError_t e = particle_set(c->part, c->N, c->L, c->dtype, n, pos, vel, mass, ms, kind == cudaMemcpyHostToDevice, c->stream);
     if (e != cudaSuccess) return fail(c, WDM_ECUDA, "particle_set: %s", cudaGetErrorString(e));
     c->stale = true;
@@ -892,6 +958,19 @@ extern "C" int wdm_set_assignment(wdm_ctx *c, int order)
     if (c->part.order != order) {
         c->part.order = order;
         c->stale = true;                     // the particles' share of the Poisson source changes
+    }
+    return WDM_OK;
+}
+
+extern "C" int wdm_set_deposit_mode(wdm_ctx *c, int deterministic)
+{
+    if (!c) return WDM_EINVAL;
+    if (deterministic != 0 && deterministic != 1) return fail(c, WDM_EINVAL, "deterministic must be 0 or 1");
+    int rcf = do_flush(c, true, true);
+    if (rcf) return rcf;
+    if (c->deposit_fixed != (deterministic != 0)) {
+        c->deposit_fixed = deterministic != 0;
+        c->stale = true;                     // the mesh is re-deposited with the other arithmetic
     }
     return WDM_OK;
 }

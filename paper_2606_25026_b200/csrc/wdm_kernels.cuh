@@ -140,6 +140,7 @@ struct SweepParams {
     const T *mask;             // 3 N reals, exp(-alpha b(x_axis) dt) along x, y, z; nullptr: no layer in this kick
     const T *phi_ext;          // C2R: static external potential added to Phi on its way out, or nullptr
     const T *rho_p;            // RHO: particle mesh density or nullptr
+    const unsigned char *rho_flag;   // RHO: one byte per (y, block of min(16, N) z-cells): 0 = rho_p is zero there, skip its loads
     const T *rho_mean;         // RHO: device scalar <rho>, subtracted before the transform (Eq. 23)
     cx<T> *H;                  // RHO / C2R: half spectrum
     T *phi_out;                // C2R: potential out

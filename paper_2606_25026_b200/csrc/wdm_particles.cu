@@ -1,9 +1,14 @@
 // wdm_particles.cu -- particle kernels (see wdm_particles.hpp).
 //
-// Particles are kept sorted by mesh tile (TS^3 cells, tile-major) with a counting sort, redone every
+// Particles are kept sorted by mesh tile (TS^3 cells, tile-major) and, inside a tile, by cell: a counting sort over
+// the tiles, then one CTA per tile sorting its segment by the 512 local cells in shared memory.  Redone every
 // kResortInterval pushes: a disc particle moves 1e-3..1e-2 cells per step, so the order stays useful for
-// hundreds of steps.  Correctness never depends on the order: the deposit falls back to global atomics
-// for any node outside the CTA's shared-memory box.
+// hundreds of steps.  With neighbouring lanes in the same or adjacent cells the 32 scattered Phi loads of a gather
+// fall into one or two sectors per instruction (the gather was bound by L1 wavefronts: 48 loads x ~32 sectors per
+// warp), and the lanes of a warp that share a stencil combine their weights before touching shared memory.
+// Correctness never depends on the order: the deposit falls back to global atomics for any node outside the
+// CTA's shared-memory box.
+#include <cmath>
 #include <cstdint>
 
 #include "wdm_particles.hpp"
@@ -171,6 +176,61 @@ __global__ void k_scatter(const T *pos, const T *vel, const T *mass, const int *
     orig2[d] = orig[i];
 }
 
+// Second level of the sort: CTA t orders the particles of tile t (the segment [bin[t], bin[t+1]) of the tile-sorted
+// arrays) by their cell inside the tile -- histogram of the TS^3 local cells in shared memory, exclusive scan,
+// scatter into the other buffer set.  Empty tiles exit at once.
+template <typename T>
+__global__ void __launch_bounds__(256) k_cellsort(const T *pos, const T *vel, const T *mass, const int *orig, const int *bin,
+                                                  T *pos2, T *vel2, T *mass2, int *orig2, int N, T L)
+{
+    constexpr int NC = TS * TS * TS;
+    __shared__ int hist[NC];
+    __shared__ int wsum[8];
+    const int t = blockIdx.x;
+    const int beg = bin[t], end = bin[t + 1];
+    if (end <= beg) return;
+    const T half_L = (T)0.5 * L, inv_dx = (T)N / L;
+    auto local_cell = [&](int i) {
+        T x[3] = {pos[3 * (long long)i], pos[3 * (long long)i + 1], pos[3 * (long long)i + 2]};
+        Cic<T> c = cic_of<T>(x, half_L, inv_dx, N);
+        return ((c.i0[0] % TS) * TS + (c.i0[1] % TS)) * TS + (c.i0[2] % TS);
+    };
+    if (end - beg == 1) {                       // the common case in the outskirts: nothing to order
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { pos2[3 * (long long)beg + a] = pos[3 * (long long)beg + a]; vel2[3 * (long long)beg + a] = vel[3 * (long long)beg + a]; }
+            if (mass) mass2[beg] = mass[beg];
+            orig2[beg] = orig[beg];
+        }
+        return;
+    }
+    for (int j = threadIdx.x; j < NC; j += blockDim.x) hist[j] = 0;
+    __syncthreads();
+    for (int i = beg + threadIdx.x; i < end; i += blockDim.x) atomicAdd(&hist[local_cell(i)], 1);
+    __syncthreads();
+    {   // exclusive scan of hist[0..512): two entries per thread
+        const int j = 2 * threadIdx.x, a0 = hist[j], a1 = hist[j + 1];
+        int x = a0 + a1;
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+        for (int d = 1; d < 32; d <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
+        if (lane == 31) wsum[w] = x;
+        __syncthreads();
+        int base = 0;
+        for (int k = 0; k < w; ++k) base += wsum[k];
+        const int excl = base + x - (a0 + a1);
+        hist[j] = excl;
+        hist[j + 1] = excl + a0;
+    }
+    __syncthreads();
+    for (int i = beg + threadIdx.x; i < end; i += blockDim.x) {
+        const long long d = beg + atomicAdd(&hist[local_cell(i)], 1);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { pos2[3 * d + a] = pos[3 * (long long)i + a]; vel2[3 * d + a] = vel[3 * (long long)i + a]; }
+        if (mass) mass2[d] = mass[i];
+        orig2[d] = orig[i];
+    }
+}
+
 // a = sum_nodes w * (phi[node+e] - phi[node-e]) per axis (the caller scales by -1/(2 dx)): gather of the
 // central-difference gradient (Eq. 21) with the deposit's weights (G13, G30)
 template <typename T, int ORDER>
@@ -249,8 +309,10 @@ __global__ void k_push(T *pos, T *vel, const T *__restrict__ phi, long long n, i
 // Particles of a warp with the same stencil are combined first (warp-aggregated atomics).
 template <typename T, int ORDER>
 __global__ void __launch_bounds__(256) k_deposit(const T *__restrict__ pos, const T *__restrict__ mass, T mass_scalar,
-                                                 T *rho, long long n, int N, T L)
+                                                 T *rho, unsigned char *flag, long long n, int N, T L)
 {
+    // flag[y * (N / FB) + z / FB] = 1 for every block of FB z-cells of a y-row that receives mass (see mesh_flag_block)
+    const int fb = mesh_flag_block(N), nfb = N / fb;
     constexpr int NW = ORDER * ORDER * ORDER;
     __shared__ T box[BOX * BOX * BOX];
     __shared__ int org[3];
@@ -278,28 +340,31 @@ __global__ void __launch_bounds__(256) k_deposit(const T *__restrict__ pos, cons
             m = (mass ? mass[i] : mass_scalar) * inv_vol;
             cell = (c.base[0] * N + c.base[1]) * N + c.base[2];
         }
-        // combine the lanes whose stencils coincide: the group leader deposits the summed weights
-        unsigned peers = __match_any_sync(0xffffffffu, cell);
-        int leader = __ffs(peers) - 1;
-        int lane = threadIdx.x & 31;
+        // Combine the lanes whose stencils coincide.  The particles are sorted by cell, so lanes with the same stencil
+        // form RUNS of consecutive lanes: a segmented reduction (5 shuffle steps per weight) leaves the run's sum in its
+        // first lane, which deposits it.  (A cell that shows up in two separate runs -- particles that drifted since the
+        // last sort -- is simply deposited twice.)
+        const int lane = threadIdx.x & 31;
+        const int prev = __shfl_up_sync(0xffffffffu, cell, 1);
+        const bool head = lane == 0 || prev != cell;
+        const unsigned heads = __ballot_sync(0xffffffffu, head);
+        const unsigned above = lane == 31 ? 0u : heads & ~((2u << lane) - 1u);       // run heads in the lanes after this one
+        const int run_end = above ? __ffs(above) - 1 : 32;                         // first lane of the next run
+        const int leader = head ? lane : -1;
         T w[NW];
 #pragma unroll
         for (int q = 0; q < NW; ++q) {
             int bx = q / (ORDER * ORDER), by = (q / ORDER) % ORDER, bz = q % ORDER;
             w[q] = active ? m * c.w[0][bx] * c.w[1][by] * c.w[2][bz] : (T)0;
         }
-        if (peers != (1u << lane)) {
-            // tree-free reduction inside each peer group: walk the group mask
+        if (heads != 0xffffffffu) {
 #pragma unroll
             for (int q = 0; q < NW; ++q) {
-                T acc = (T)0;
-                unsigned rem = peers;
-                while (rem) {
-                    int src = __ffs(rem) - 1;
-                    rem &= rem - 1;
-                    acc += __shfl_sync(peers, w[q], src);
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const T v = __shfl_down_sync(0xffffffffu, w[q], d);
+                    if (lane + d < run_end) w[q] += v;
                 }
-                w[q] = acc;
             }
         }
         if (active && lane == leader) {
@@ -309,7 +374,11 @@ __global__ void __launch_bounds__(256) k_deposit(const T *__restrict__ pos, cons
             for (int q = 0; q < NW; ++q) {
                 int bx = q / (ORDER * ORDER), by = (q / ORDER) % ORDER, bz = q % ORDER;
                 if (inside) atomicAdd(&box[((rx + bx) * BOX + ry + by) * BOX + rz + bz], w[q]);
-                else atomicAdd(rho + ((size_t)((c.base[0] + bx) & M) * N + ((c.base[1] + by) & M)) * N + ((c.base[2] + bz) & M), w[q]);
+                else {
+                    const int gy = (c.base[1] + by) & M, gz = (c.base[2] + bz) & M;
+                    atomicAdd(rho + ((size_t)((c.base[0] + bx) & M) * N + gy) * N + gz, w[q]);
+                    flag[gy * nfb + gz / fb] = 1;
+                }
             }
         }
     }
@@ -318,9 +387,67 @@ __global__ void __launch_bounds__(256) k_deposit(const T *__restrict__ pos, cons
         T v = box[j];
         if (v != (T)0) {
             int rz = j % BOX, ry = (j / BOX) % BOX, rx = j / (BOX * BOX);
-            atomicAdd(rho + ((size_t)((org[0] + rx) & M) * N + ((org[1] + ry) & M)) * N + ((org[2] + rz) & M), v);
+            const int gy = (org[1] + ry) & M, gz = (org[2] + rz) & M;
+            atomicAdd(rho + ((size_t)((org[0] + rx) & M) * N + gy) * N + gz, v);
+            flag[gy * nfb + gz / fb] = 1;
         }
     }
+}
+
+// Deterministic deposit (debugging mode, SURVEY.md "Determinism"): every weight is rounded ONCE to a 64-bit fixed-point
+// number (scale = a power of two chosen from the total mass, so that the sum of everything fits) and accumulated with
+// integer atomics -- integer addition is associative, so the mesh is bit-identical from run to run whatever the order
+// of the particles, the warps or the sort.  Costs 8 bytes per cell of extra memory and a conversion pass.
+template <typename T, int ORDER>
+__global__ void __launch_bounds__(256) k_deposit_fixed(const T *__restrict__ pos, const T *__restrict__ mass, T mass_scalar,
+                                                       unsigned long long *acc, long long n, int N, T L, double scale)
+{
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const T inv_dx = (T)N / L, inv_vol = inv_dx * inv_dx * inv_dx;
+    const T x[3] = {pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+    const Asg<T, ORDER> c = asg_of<T, ORDER>(x, (T)0.5 * L, inv_dx, N);
+    const T m = (mass ? mass[i] : mass_scalar) * inv_vol;
+    const int M = N - 1;
+#pragma unroll
+    for (int bx = 0; bx < ORDER; ++bx)
+#pragma unroll
+        for (int by = 0; by < ORDER; ++by)
+#pragma unroll
+            for (int bz = 0; bz < ORDER; ++bz) {
+                const T w = m * c.w[0][bx] * c.w[1][by] * c.w[2][bz];          // the same product as k_deposit
+                const long long q = __double2ll_rn((double)w * scale);
+                atomicAdd(acc + ((size_t)((c.base[0] + bx) & M) * N + ((c.base[1] + by) & M)) * N + ((c.base[2] + bz) & M),
+                          (unsigned long long)q);
+            }
+}
+
+// rho = acc / scale, acc = 0 (whole mesh)
+template <typename T>
+__global__ void k_fixed_to_mesh(unsigned long long *acc, T *rho, size_t n, double inv_scale)
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const long long v = (long long)acc[i];
+        rho[i] = (T)((double)v * inv_scale);
+        if (v) acc[i] = 0;
+    }
+}
+
+// Zero the flagged parts of the particle mesh and the flags: block b = (y, z-block) covers rho[x][y][zb*FB .. +FB) for
+// every x.  One CTA per flag; unflagged blocks (a thin disc flags ~10 % of them) cost one byte load.
+template <typename T>
+__global__ void __launch_bounds__(128) k_mesh_clear(T *rho, unsigned char *flag, int N, int fb)
+{
+    const int b = blockIdx.x, nfb = N / fb;
+    if (!flag[b]) return;
+    const int y = b / nfb, z0 = (b - y * nfb) * fb;
+    // fb reals per x-row: threads cover (x, z) pairs, fb consecutive threads on one row
+    for (int i = threadIdx.x; i < N * fb; i += blockDim.x) {
+        const int x = i / fb, z = z0 + i % fb;
+        rho[((size_t)x * N + y) * N + z] = (T)0;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) flag[b] = 0;
 }
 
 template <typename T>
@@ -352,10 +479,16 @@ cudaError_t resort(ParticleState &ps, int N, double L, cudaStream_t s)
     k_scatter<T><<<blocks(n, 256), 256, 0, s>>>((const T *)ps.pos, (const T *)ps.vel, ps.has_mass ? (const T *)ps.mass : nullptr,
                                                 ps.orig, ps.key, ps.bin + nb + 1, (T *)ps.pos2, (T *)ps.vel2,
                                                 (T *)ps.mass2, ps.orig2, n);
-    std::swap(ps.pos, ps.pos2);
-    std::swap(ps.vel, ps.vel2);
-    std::swap(ps.mass, ps.mass2);
-    std::swap(ps.orig, ps.orig2);
+    if (N >= TS) {
+        // tile-sorted set 2 -> tile- and cell-sorted set 1
+        k_cellsort<T><<<nb, 256, 0, s>>>((const T *)ps.pos2, (const T *)ps.vel2, ps.has_mass ? (const T *)ps.mass2 : nullptr, ps.orig2,
+                                         ps.bin, (T *)ps.pos, (T *)ps.vel, (T *)ps.mass, ps.orig, N, (T)L);
+    } else {
+        std::swap(ps.pos, ps.pos2);
+        std::swap(ps.vel, ps.vel2);
+        std::swap(ps.mass, ps.mass2);
+        std::swap(ps.orig, ps.orig2);
+    }
     ps.steps_since_sort = 0;
     return cudaGetLastError();
 }
@@ -364,10 +497,9 @@ template <typename T>
 cudaError_t set_impl(ParticleState &ps, int N, double L, long long n, const void *pos, const void *vel, const void *mass,
                      double mass_scalar, bool from_host, cudaStream_t s)
 {
-    ps.n = n;
-    ps.has_mass = mass != nullptr;
-    ps.mass_scalar = mass_scalar;
-    if (n == 0) return cudaSuccess;
+    // the particle set is committed only when every copy and launch has been accepted; a failure leaves none
+    ps.n = 0;
+    if (n == 0) { ps.has_mass = false; ps.mass_scalar = mass_scalar; return cudaSuccess; }
     cudaMemcpyKind kind = from_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
     cudaError_t e;
     // stage the caller's arrays in the second buffers, then wrap + index into the first
@@ -376,7 +508,11 @@ cudaError_t set_impl(ParticleState &ps, int N, double L, long long n, const void
     if (mass && (e = cudaMemcpyAsync(ps.mass, mass, sizeof(T) * n, kind, s)) != cudaSuccess) return e;
     k_ingest<T><<<blocks(n, 256), 256, 0, s>>>((const T *)ps.pos2, (const T *)ps.vel2, (T *)ps.pos, (T *)ps.vel, ps.orig, n, (T)L);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    return resort<T>(ps, N, L, s);
+    ps.n = n;
+    ps.has_mass = mass != nullptr;
+    ps.mass_scalar = mass_scalar;
+    if ((e = resort<T>(ps, N, L, s)) != cudaSuccess) ps.n = 0;
+    return e;
 }
 
 }  // namespace
@@ -384,7 +520,7 @@ cudaError_t set_impl(ParticleState &ps, int N, double L, long long n, const void
 size_t particle_bytes(int N, int dtype, long long cap)
 {
     size_t r = dtype == 0 ? 4 : 8, c = (size_t)(cap > 0 ? cap : 1);
-    return 4 * al(3 * c * r) + 2 * al(c * r) + 3 * al(c * 4) + al(sizeof(int) * (2 * (size_t)nbins(N) + 2)) + 256;
+    return 4 * al(3 * c * r) + 2 * al(c * r) + 3 * al(c * 4) + al(sizeof(int) * (2 * (size_t)nbins(N) + 2)) + al((size_t)N * N) + 256;
 }
 
 void particle_bind(ParticleState &ps, int N, int dtype, long long cap, void *rho_p, void *pool)
@@ -397,6 +533,8 @@ void particle_bind(ParticleState &ps, int N, int dtype, long long cap, void *rho
     ps.mass = take(c * r); ps.mass2 = take(c * r);
     ps.orig = (int *)take(c * 4); ps.orig2 = (int *)take(c * 4); ps.key = (int *)take(c * 4);
     ps.bin = (int *)take(sizeof(int) * (2 * (size_t)nbins(N) + 2));
+    ps.flag = (unsigned char *)take((size_t)N * N);
+    ps.mesh_clean = false;
     ps.capacity = cap;
     ps.n = 0;
 }
@@ -436,10 +574,51 @@ cudaError_t particle_deposit(ParticleState &ps, int N, double L, int dtype, cuda
     unsigned g = blocks(ps.n, CHUNK);
     const float *mf = ps.has_mass ? (const float *)ps.mass : nullptr;
     const double *md = ps.has_mass ? (const double *)ps.mass : nullptr;
-    if (dtype == 0 && ps.order == 2) k_deposit<float, 2><<<g, 256, 0, s>>>((const float *)ps.pos, mf, (float)ps.mass_scalar, (float *)ps.rho_p, ps.n, N, (float)L);
-    else if (dtype == 0) k_deposit<float, 3><<<g, 256, 0, s>>>((const float *)ps.pos, mf, (float)ps.mass_scalar, (float *)ps.rho_p, ps.n, N, (float)L);
-    else if (ps.order == 2) k_deposit<double, 2><<<g, 256, 0, s>>>((const double *)ps.pos, md, ps.mass_scalar, (double *)ps.rho_p, ps.n, N, L);
-    else k_deposit<double, 3><<<g, 256, 0, s>>>((const double *)ps.pos, md, ps.mass_scalar, (double *)ps.rho_p, ps.n, N, L);
+    if (dtype == 0 && ps.order == 2) k_deposit<float, 2><<<g, 256, 0, s>>>((const float *)ps.pos, mf, (float)ps.mass_scalar, (float *)ps.rho_p, ps.flag, ps.n, N, (float)L);
+    else if (dtype == 0) k_deposit<float, 3><<<g, 256, 0, s>>>((const float *)ps.pos, mf, (float)ps.mass_scalar, (float *)ps.rho_p, ps.flag, ps.n, N, (float)L);
+    else if (ps.order == 2) k_deposit<double, 2><<<g, 256, 0, s>>>((const double *)ps.pos, md, ps.mass_scalar, (double *)ps.rho_p, ps.flag, ps.n, N, L);
+    else k_deposit<double, 3><<<g, 256, 0, s>>>((const double *)ps.pos, md, ps.mass_scalar, (double *)ps.rho_p, ps.flag, ps.n, N, L);
+    return cudaGetLastError();
+}
+
+cudaError_t particle_deposit_fixed(ParticleState &ps, int N, double L, int dtype, unsigned long long *acc, double total_mass,
+                                   cudaStream_t s)
+{
+    if (ps.n == 0) return cudaSuccess;
+    // the largest possible cell value is total_mass / dx^3; leave two bits of head room below 2^62
+    const double dx = L / N, top = total_mass / (dx * dx * dx);
+    int ex = 0;
+    frexp(top > 0 ? top : 1.0, &ex);
+    const double scale = ldexp(1.0, 60 - ex);
+    const unsigned g = blocks(ps.n, 256);
+    const float *mf = ps.has_mass ? (const float *)ps.mass : nullptr;
+    const double *md = ps.has_mass ? (const double *)ps.mass : nullptr;
+    if (dtype == 0 && ps.order == 2) k_deposit_fixed<float, 2><<<g, 256, 0, s>>>((const float *)ps.pos, mf, (float)ps.mass_scalar, acc, ps.n, N, (float)L, scale);
+    else if (dtype == 0) k_deposit_fixed<float, 3><<<g, 256, 0, s>>>((const float *)ps.pos, mf, (float)ps.mass_scalar, acc, ps.n, N, (float)L, scale);
+    else if (ps.order == 2) k_deposit_fixed<double, 2><<<g, 256, 0, s>>>((const double *)ps.pos, md, ps.mass_scalar, acc, ps.n, N, L, scale);
+    else k_deposit_fixed<double, 3><<<g, 256, 0, s>>>((const double *)ps.pos, md, ps.mass_scalar, acc, ps.n, N, L, scale);
+    const size_t n3 = (size_t)N * N * N;
+    if (dtype == 0) k_fixed_to_mesh<float><<<148 * 8, 256, 0, s>>>(acc, (float *)ps.rho_p, n3, 1.0 / scale);
+    else k_fixed_to_mesh<double><<<148 * 8, 256, 0, s>>>(acc, (double *)ps.rho_p, n3, 1.0 / scale);
+    // the whole mesh was rewritten: every block counts as touched (a later sparse clear then zeroes all of it)
+    cudaError_t e = cudaMemsetAsync(ps.flag, 1, (size_t)N * (N / mesh_flag_block(N)), s);
+    if (e != cudaSuccess) return e;
+    ps.mesh_clean = true;
+    return cudaGetLastError();
+}
+
+cudaError_t particle_mesh_clear(ParticleState &ps, int N, int dtype, cudaStream_t s)
+{
+    const int fb = mesh_flag_block(N), nflag = N * (N / fb);
+    if (!ps.mesh_clean) {
+        // first use (or a mesh of unknown content): everything, once
+        cudaError_t e = cudaMemsetAsync(ps.rho_p, 0, (size_t)N * N * N * (dtype == 0 ? 4 : 8), s);
+        if (e == cudaSuccess) e = cudaMemsetAsync(ps.flag, 0, (size_t)nflag, s);
+        if (e == cudaSuccess) ps.mesh_clean = true;
+        return e;
+    }
+    if (dtype == 0) k_mesh_clear<float><<<nflag, 128, 0, s>>>((float *)ps.rho_p, ps.flag, N, fb);
+    else k_mesh_clear<double><<<nflag, 128, 0, s>>>((double *)ps.rho_p, ps.flag, N, fb);
     return cudaGetLastError();
 }
 

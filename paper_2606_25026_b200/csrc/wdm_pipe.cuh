@@ -585,10 +585,14 @@ struct PsiK {
             // single-precision partial sums of the low-k modes.
             const T mean = ldg(p.rho_mean);
             cx<T> *Sp = reinterpret_cast<cx<T> *>(buf);
+            // particle mass reaches only a small part of the mesh (a thin disc: ~10 % of the tiles); the deposit flags the
+            // (y, z-block) columns it touched and every other tile skips the loads (rho_p is zero there)
+            constexpr int FB = N < 16 ? N : 16;
+            const bool has_rho_p = p.rho_p != nullptr && p.rho_flag[(t / TL::INNER) * (N / FB) + ((t % TL::INNER) * W) / FB] != 0;
             if constexpr (PAIR) {
                 // the pair (pl, pl + 1) at rows pq + mA r IS packed line pl / 2 at the rows of this thread's own
                 // level-A butterfly of the real-to-complex transform: straight from registers
-                const T *gp = p.rho_p ? p.rho_p + tile.at(pq, pl) : nullptr;
+                const T *gp = has_rho_p ? p.rho_p + tile.at(pq, pl) : nullptr;
                 cx<T> v[RA];
                 static_for<0, RA>([&](auto r_) {
                     constexpr int r = decltype(r_)::value;
@@ -608,7 +612,7 @@ struct PsiK {
                     constexpr int it = decltype(it_)::value;
                     int q, l;
                     split<AX, mA, W>(gt + it * NTG, q, l);
-                    const T *gp = p.rho_p ? p.rho_p + tile.at(q, l) : nullptr;
+                    const T *gp = has_rho_p ? p.rho_p + tile.at(q, l) : nullptr;
                     static_for<0, RA>([&](auto r_) {
                         constexpr int r = decltype(r_)::value;
                         int row = q + mA * r;

@@ -244,6 +244,44 @@ def test_config5_full(wdm):
     check_particles(sim, o, w.L, w.nsteps, "c64")
 
 
+@pytest.mark.parametrize("order", [2, 3])
+def test_deterministic_deposit_is_bit_stable_and_matches_oracle(wdm, order):
+    """wdm_set_deposit_mode(1): fixed-point accumulation (SURVEY.md "Determinism").  The thin-disc workload at reduced
+    size, sorted twice on the way (more pushes than the re-sort interval): two runs agree bit for bit in psi, Phi, rho and
+    the particles, and the result matches the oracle like the floating-point deposit does."""
+    import torch
+    w = wl.config5(N=64, n_particles=1 << 14, nsteps=70)
+    outs = []
+    for rep in range(2):
+        sim, o = pair(wdm, w, len(w.pos))
+        sim.set_deposit_mode(True)
+        sim.set_assignment(order)
+        if rep == 0:
+            o.set_assignment(order)
+            check_fields(sim, o, "c64", 0, "fixed-point deposit, initial")
+            dt = wl.cfl_dt(w, float(np.abs(o.potential()).max()))
+        sim.step(70, dt)
+        p, v = sim.particles()
+        outs.append((sim.psi().clone(), sim.potential().clone(), sim.density().clone(), p.clone(), v.clone()))
+        if rep == 0:
+            o.step(70, dt)
+            check_fields(sim, o, "c64", 70, "fixed-point deposit")
+            check_particles(sim, o, w.L, 70, "c64")
+        sim.close()
+    for a, b in zip(*outs):
+        assert torch.equal(a, b)
+    # back and forth between the two arithmetics in one context
+    sim, o = pair(wdm, w, len(w.pos))
+    sim.step(2, dt); o.step(2, dt)
+    sim.set_deposit_mode(True)
+    sim.step(2, dt); o.step(2, dt)
+    sim.set_deposit_mode(False)
+    sim.step(2, dt); o.step(2, dt)
+    check_fields(sim, o, "c64", 6, "mode switches")
+    check_particles(sim, o, w.L, 6, "c64")
+    sim.close()
+
+
 def test_resort_keeps_results(wdm):
     """More pushes than the re-sort interval: sorting must not change what is computed."""
     w = wl.small_coupled(16, dtype="c128", n_particles=300)
