@@ -321,18 +321,27 @@ struct Packed {
     using T = typename C::T;
     static constexpr int RSP = C::W / 2;
     static constexpr bool SWZ = ON && RSP * sizeof(cx<T>) == 64 && C::RB == 1;
+    // 32-byte rows (W = 8 complex64 / W = 4 complex128: the 1024-point tiles).  The middle level reads rows a multiple of
+    // RM apart from neighbouring lanes: RM * 32 bytes apart, i.e. in the same 8 banks -- an 8-way conflict (ncu at 1024^3:
+    // 2.4e8 conflicts in 6.4e8 instructions of the complex-to-real sweep, short-scoreboard stalls 9 per issue).  One
+    // empty row after every RM rows shifts consecutive blocks by 32 bytes: four blocks cover all banks.
+    static constexpr bool PADROW = ON && RSP * sizeof(cx<T>) == 32 && C::RB == 1;
+    static constexpr int BLK = (C::RM + (PADROW ? 1 : 0)) * RSP;          // elements from row r to row r + RM
+    static constexpr size_t ELEMS = (size_t)(C::N + (PADROW ? C::N / C::RM : 0)) * RSP;
     static __device__ __forceinline__ int idx(int row, int l)
     {
         if constexpr (SWZ) row ^= (row / C::RM) & 1;
+        if constexpr (PADROW) row += row / C::RM;
         return row * RSP + l;
     }
-    // The same index for the two access patterns of the stages, written so that the swizzle costs nothing per
+    // The same index for the two access patterns of the stages, written so that the swizzle / padding costs nothing per
     // access once the stage is unrolled (d a compile-time constant): two base addresses per thread, the rest
     // immediates.  idxA: row q + d of a level-A butterfly (q < RM, d a multiple of RM; RB == 1 so mA == RM).
     // idxM: row row0 + d of a middle-level butterfly (row0 a multiple of RM, d < RM).
     static __device__ __forceinline__ int idxA(int q, int d, int l)
     {
         if constexpr (SWZ) return ((q ^ ((d / C::RM) & 1)) + d) * RSP + l;
+        else if constexpr (PADROW) return (q + d + d / C::RM) * RSP + l;
         else return (q + d) * RSP + l;
     }
     static __device__ __forceinline__ int idxM(int row0, int d, int l)
@@ -340,7 +349,8 @@ struct Packed {
         if constexpr (SWZ) {
             const int b = ((row0 / C::RM) & 1) * RSP;
             return (row0 + d) * RSP + l + ((d & 1) ? -b : b);
-        } else return (row0 + d) * RSP + l;
+        } else if constexpr (PADROW) return (row0 + row0 / C::RM + d) * RSP + l;
+        else return (row0 + d) * RSP + l;
     }
 };
 
@@ -357,7 +367,7 @@ __device__ __forceinline__ void half_spectrum_items(int gt, F &&f)
     constexpr int NT = C::NT, HM = C::RM / 2, ITEMS = (C::N / 2) * WP;
     constexpr bool FAST = C::RB == 1 && NT % WP == 0 && (NT / WP) % (2 * HM) == 0 && ITEMS % NT == 0 && ITEMS / NT <= 16;
     if constexpr (FAST) {
-        constexpr int DA = NT / WP / HM, ITERS = ITEMS / NT, STEP = DA * C::RM * WP;
+        constexpr int DA = NT / WP / HM, ITERS = ITEMS / NT, STEP = DA * PK::BLK;
         static_assert(ITERS * DA == C::RA && PK::RSP == WP, "item i of a thread is frequency k0 + DA i");
         const int l = gt % WP, kk0 = gt / WP, sM = kk0 % HM, sA0 = kk0 / HM;
         const int k0 = sA0 + C::RA * sM;
@@ -765,7 +775,7 @@ struct C2RK {
     static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA;
     static constexpr int WP = W / 2, RSP = W / 2;
     using PK = Packed<C, true>;
-    static constexpr size_t PACKED_BYTES = align128((size_t)N * RSP * sizeof(cx<T>));
+    static constexpr size_t PACKED_BYTES = align128(PK::ELEMS * sizeof(cx<T>));
     static constexpr size_t TILE_BYTES = PACKED_BYTES + align128((size_t)(N / 2 + 1) * W * sizeof(cx<T>));
     static constexpr int AUX = AUX_NONE;
     using Pre = NoPre;
