@@ -134,15 +134,35 @@ int wdm_get_assignment(wdm_ctx *ctx, int *order);
  * cloud-in-cell / triangular-shaped-cloud sum of PAPER.md:314 (readings G12, G30).  Marks the potential stale. */
 int wdm_set_deposit_mode(wdm_ctx *ctx, int deterministic);
 
-/* Diagnostics of the current state (Sect. 3.5-3.6) by one reduction pass on the device; the
- * gradients are the second-order central differences of Eq. 21.  Synchronises the stream.
- * out_host[0] M = sum |psi|^2 dx^3       [1] max |psi|^2       [2] max |Phi_total|
- *         [3] V = sum |psi|^2 Phi dx^3 (as printed: no factor 1/2)
- *         [4] K = 1/2 sum |rho v|^2/rho dx^3, rho v = (hbar/m) Im(psi* grad psi)
- *         [5] Q = (hbar/m)^2/2 sum |grad sqrt(rho)|^2 dx^3
- *         [6] dt_max of Eq. 26, without the safety factor      [7] reserved (0)
+/* Diagnostics of the current (time-level) state (Sect. 3.5-3.6), on demand: one reduction pass over
+ * (psi, Phi) with the second-order central differences of Eq. 21 for K and Q, and three forward-only
+ * axis sweeps (psi is read, nothing is written) for the spectral kinetic energy.  Synchronises the stream.
+ * out_host must hold 12 doubles:
+ *   [0] M = sum |psi|^2 dx^3       [1] max |psi|^2       [2] max |Phi_total|
+ *   [3] V = sum |psi|^2 Phi dx^3 (as printed: no factor 1/2)
+ *   [4] K = 1/2 sum |rho v|^2/rho dx^3, rho v = (hbar/m) Im(psi* grad psi)
+ *   [5] Q = (hbar/m)^2/2 sum |grad sqrt(rho)|^2 dx^3   (Eq. 12 with its hbar^2/2m; reading G31)
+ *   [6] dt_max of Eq. 26, without the safety factor
+ *   [7] T = (hbar/m)^2/2 sum_k k^2 |psi~_k|^2 dx^3/N^3  (spectral kinetic energy; K + Q in the continuum limit)
+ *   [8] W = V/2       [9] E = T + W, the energy the pure SPE conserves       [10], [11] reserved (0)
  * The potential is recomputed first if stale.  Particles do not enter (rho is the wave density). */
 int wdm_get_diagnostics(wdm_ctx *ctx, double *out_host);
+
+/* Diagnostics accumulated INSIDE the sweeps of a step, at no extra pass over the grid and no extra kernel launch
+ * (SURVEY 8(f) rank 2): while switched on, wdm_step uses instantiations of its sweeps that also reduce what they have
+ * in registers (the L2-chained forms are not used meanwhile).  wdm_get_step_diagnostics returns, for the LAST step run,
+ * the state between Eq. 18(c) and (d) -- psi_2 after the drift, before the closing half kick, the
+ * Poisson source rho = |psi_2|^2 + particles and the potential just solved from it; synchronises the stream.
+ * out_host must hold 8 doubles:
+ *   [0] M = sum |psi_2|^2 dx^3, [1] max |psi_2|^2                      (density sweep; G > 0 only)
+ *   [2] max |Phi_total|                                                 (complex-to-real sweep; G > 0 only)
+ *   [3] T = T_x + T_y + T_z of psi_2, spectral: each axis sweep sums k_a^2 |F_a psi|^2 in its middle level (the other
+ *       axes' drift factors have unit modulus, so T is the same before and after Eq. 18(b))
+ *   [4] W = 1/2 sum rho Phi_grav dx^3 over the whole source, summed spectrally in the Green's-function sweep
+ *   [5] T_x, [6] T_y, [7] T_z
+ * E = T + W is the conserved energy of the pure SPE.  WDM_ESTATE until a step has run. */
+int wdm_set_step_diagnostics(wdm_ctx *ctx, int on);
+int wdm_get_step_diagnostics(wdm_ctx *ctx, double *out_host);
 
 /* Execution mode of the plane-local sweeps (no effect on results beyond rounding order).
  * mode is a bit mask.  Bit 0 (1): the z and y sweeps of psi (Eq. 18(b)) run as one

@@ -213,6 +213,11 @@ struct wdm_ctx {
     int absorb_nb = 50;
     const void *phi_ext = nullptr;            // library-owned copy of the caller's N^3 reals (phi_ext_buf) or nullptr
     void *phi_ext_buf = nullptr;              // cudaMalloc'ed on the first wdm_set_kick_terms with an external potential
+    // per-step diagnostics accumulated inside the sweeps (wdm_set_step_diagnostics): three sets of DIAG_COUNT doubles on the
+    // device -- two used by alternate steps (a step's z sweep zeroes the other set), one for the on-demand measurement
+    bool step_diag = false, step_diag_valid = false;
+    double *diag_dev = nullptr;
+    int diag_set = 0, diag_last = 0;
     // deterministic deposit (wdm_set_deposit_mode): N^3 64-bit accumulators, cudaMalloc'ed on first use; upper bound of
     // the total particle mass (0 = not measured for the current particle set)
     bool deposit_fixed = false;
@@ -272,7 +277,7 @@ static size_t grid_bytes(int N, int dtype, long long max_particles)
     size_t n = (size_t)N * N * N, nH = (size_t)(N / 2 + 1) * N * N, c = csize(dtype), r = rsize(dtype);
     size_t b = align_up(n * c) + align_up(n * r) + align_up(nH * c);
     b += 3 * align_up((size_t)N * c) + 2 * align_up((size_t)N * r) + align_up((size_t)N * 2) + 256;
-    b += align_up((size_t)(2 * N + 2 + 8) * sizeof(unsigned int)) + align_up((size_t)3 * N * r);
+    b += align_up((size_t)(2 * N + 2 + 8) * sizeof(unsigned int)) + align_up((size_t)3 * N * r) + align_up(3 * DIAG_COUNT * sizeof(double));
     if (max_particles > 0) b += align_up(n * r) + particle_bytes(N, dtype, max_particles);
     return b + 4096;
 }
@@ -467,6 +472,8 @@ static SweepParams<T> base_params(wdm_ctx *c)
     p.rho_flag = c->part.flag;
     p.rho_mean = (const T *)((const unsigned char *)c->rho_mean + 16);
     p.phi_ext = (const T *)c->phi_ext;
+    p.diag = c->diag_dev + c->diag_set * DIAG_COUNT;
+    p.diag_zero = c->diag_dev + (c->diag_set ^ 1) * DIAG_COUNT;
     return p;
 }
 
@@ -474,7 +481,7 @@ static SweepParams<T> base_params(wdm_ctx *c)
 
 // rho (from the current psi and particle mesh) -> Phi.  drift: also do the x-axis part of Eq. 18(b).
 template <typename T>
-static int density_poisson(wdm_ctx *c, bool drift)
+static int density_poisson(wdm_ctx *c, bool drift, int dg = 0)
 {
     const long long N = c->N;
     {
@@ -483,23 +490,23 @@ static int density_poisson(wdm_ctx *c, bool drift)
         p.tmap = c->tm_psi_x;
         take_ticket(c, p);
         Timed t(c, S_PSI_X_RHO);
-        CU(c, c->tab->psi_x_rho(&p, drift ? 1 : 0, c->stream));
+        CU(c, c->tab->psi_x_rho(&p, drift ? 1 : 0, dg, c->stream));
     }
     SweepParams<T> p = base_params<T>(c);
     p.data = (cx<T> *)c->H;
     p.tmap = c->tm_h_y;
-    if (c->lag_h > 0) {
+    if (c->lag_h > 0 && !dg) {
         ChainCtl ctl{c->chain_done + N, ++c->epoch_h * (unsigned int)(N / c->tab->fact.W), c->lag_h};
         Timed t(c, S_H_YZY);
         CU(c, c->tab->h_yzy(&p, &p, &ctl, c->stream));
     } else {
         { take_ticket(c, p); Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
-        { take_ticket(c, p); Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, c->stream)); }
+        { take_ticket(c, p); Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, dg, c->stream)); }
         { take_ticket(c, p); Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
     }
     p.tmap = c->tm_h_x;
     p.tmap2 = c->tm_h_x1;
-    { take_ticket(c, p); Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, c->stream)); }
+    { take_ticket(c, p); Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, dg, c->stream)); }
     return WDM_OK;
 }
 
@@ -623,6 +630,8 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
     const bool have_phi = grav || c->phi_ext != nullptr;                 // particles and psi feel a potential
     const bool layer = c->alpha > 0;
     const bool kicks = have_phi || c->kappa != 0.0 || layer;
+    const int dg = c->step_diag ? 1 : 0;                  // the accumulating instantiations (separate sweeps only)
+    if (dg) CU(c, cudaMemsetAsync(c->diag_dev + c->diag_set * DIAG_COUNT, 0, DIAG_COUNT * sizeof(double), c->stream));
     for (int s = 0; s < nsteps; ++s) {
         // merged closing (h_d, of the previous step -- possibly of the previous call) + opening (h_a) half kicks
         // (G21); the absorbing layer sits between them
@@ -644,19 +653,19 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             pz.kick_extra = (c->kappa != 0.0 || pz.mask != nullptr) ? 1 : 0;
             py.data = (cx<T> *)c->psi;
             py.tmap = c->tm_psi_y;
-            if (c->lag_psi > 0 && !pz.kick_extra) {
+            if (c->lag_psi > 0 && !pz.kick_extra && !dg) {
                 ChainCtl ctl{c->chain_done, ++c->epoch_psi * (unsigned int)(N / c->tab->fact.W), c->lag_psi};
                 Timed t(c, S_PSI_ZY);
                 CU(c, c->tab->psi_zy(&pz, &py, kicks ? 1 : 0, &ctl, c->stream));
             } else {
-                { take_ticket(c, pz); Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? (pz.kick_extra ? 2 : 1) : 0, c->stream)); }
-                { take_ticket(c, py); Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, c->stream)); }
+                { take_ticket(c, pz); Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? (pz.kick_extra ? 2 : 1) : 0, dg, c->stream)); }
+                { take_ticket(c, py); Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, dg, c->stream)); }
             }
         }
         c->pend_psi = 0.0;
         c->pend_part = 0.0;
         if (grav) {
-            rc = density_poisson<T>(c, true);
+            rc = density_poisson<T>(c, true, dg);
             if (rc) return rc;
         } else {
             SweepParams<T> p = base_params<T>(c);
@@ -664,8 +673,9 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             p.tmap = c->tm_psi_x;
             take_ticket(c, p);
             Timed t(c, S_PSI_Y);
-            CU(c, c->tab->psi_strided(&p, 1, c->stream));
+            CU(c, c->tab->psi_strided(&p, 1, dg, c->stream));
         }
+        if (dg) { c->diag_last = c->diag_set; c->diag_set ^= 1; c->step_diag_valid = true; }
     }
     // the closing half kicks (and the last absorbing layer) stay pending: the next wdm_step merges them into its
     // opening kick; a read of the state or a change of parameters applies them first (flush_pending)
@@ -733,7 +743,7 @@ static int create_common(wdm_ctx **out, int N, double L, double mu, double G, in
         (rc = ctx_alloc(c, &c->ksq_pos, N * rs)) || (rc = ctx_alloc(c, &c->ksq_nat, N * rs)) ||
         (rc = ctx_alloc(c, &c->rho_mean, 64)) ||
         (rc = ctx_alloc(c, (void **)&c->chain_done, (size_t)(2 * N + 2 + 8) * sizeof(unsigned int))) ||
-        (rc = ctx_alloc(c, &c->mask, (size_t)3 * N * rs)))
+        (rc = ctx_alloc(c, &c->mask, (size_t)3 * N * rs)) || (rc = ctx_alloc(c, (void **)&c->diag_dev, 3 * DIAG_COUNT * sizeof(double))))
         return bail(rc);
     if (cudaMemset(c->chain_done, 0, (size_t)(2 * N + 2 + 8) * sizeof(unsigned int)) != cudaSuccess)
         return bail(fail(c, WDM_ECUDA, "cudaMemset of the chain counters failed"));
@@ -982,6 +992,23 @@ extern "C" int wdm_get_assignment(wdm_ctx *c, int *order)
     return WDM_OK;
 }
 
+// sum k_a^2 |F_a psi|^2 of the current psi for a = z, y, x into acc[0..2] (forward-only sweeps, psi untouched)
+template <typename T>
+static int measure_kinetic(wdm_ctx *c, double *acc)
+{
+    for (int a = 0; a < 3; ++a) {
+        SweepParams<T> p = base_params<T>(c);
+        p.data = (cx<T> *)c->psi;
+        p.diag = acc;
+        p.diag_zero = nullptr;
+        p.tmap = a == 1 ? c->tm_psi_y : c->tm_psi_x;
+        take_ticket(c, p);
+        Timed t(c, S_MISC);
+        CU(c, a == 0 ? c->tab->psi_z(&p, 0, 2, c->stream) : c->tab->psi_strided(&p, a == 2 ? 1 : 0, 2, c->stream));
+    }
+    return WDM_OK;
+}
+
 extern "C" int wdm_get_diagnostics(wdm_ctx *c, double *out_host)
 {
     if (!c) return WDM_EINVAL;
@@ -1014,7 +1041,47 @@ extern "C" int wdm_get_diagnostics(wdm_ctx *c, double *out_host)
     if (maxphi > 0 && 2.0 * M_PI * c->mu / maxphi < dtm) dtm = 2.0 * M_PI * c->mu / maxphi;
     if (c->kappa != 0 && maxrho > 0 && 2.0 * M_PI * c->mu / (fabs(c->kappa) * maxrho) < dtm) dtm = 2.0 * M_PI * c->mu / (fabs(c->kappa) * maxrho);
     out_host[6] = 0.5 * dtm;
-    out_host[7] = 0;
+    // spectral kinetic energy of the current psi: three forward-only sweeps (one per axis) that write nothing
+    {
+        double *m = c->diag_dev + 2 * DIAG_COUNT;
+        CU(c, cudaMemsetAsync(m, 0, DIAG_COUNT * sizeof(double), c->stream));
+        rc = c->dtype == WDM_C64 ? measure_kinetic<float>(c, m) : measure_kinetic<double>(c, m);
+        if (rc) return rc;
+        double t[3];
+        CU(c, cudaMemcpyAsync(t, m, sizeof t, cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        const double f = 0.5 * c->mu * c->mu * dV / c->N;
+        out_host[7] = f * (t[0] + t[1] + t[2]);
+    }
+    out_host[8] = 0.5 * out_host[3];
+    out_host[9] = out_host[7] + out_host[8];
+    out_host[10] = out_host[11] = 0;
+    return WDM_OK;
+}
+
+extern "C" int wdm_set_step_diagnostics(wdm_ctx *c, int on)
+{
+    if (!c) return WDM_EINVAL;
+    c->step_diag = on != 0;
+    c->step_diag_valid = false;
+    return WDM_OK;
+}
+
+extern "C" int wdm_get_step_diagnostics(wdm_ctx *c, double *out_host)
+{
+    if (!c) return WDM_EINVAL;
+    if (!out_host) return fail(c, WDM_EINVAL, "null output");
+    if (!c->step_diag_valid) return fail(c, WDM_ESTATE, "no step has run since wdm_set_step_diagnostics(ctx, 1)");
+    double d[DIAG_COUNT];
+    CU(c, cudaMemcpyAsync(d, c->diag_dev + c->diag_last * DIAG_COUNT, sizeof d, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    const double dx = c->L / c->N, dV = dx * dx * dx, f = 0.5 * c->mu * c->mu * dV / c->N;
+    out_host[0] = d[3] * dV;
+    out_host[1] = d[4];                      // maxima travel as bit patterns of non-negative doubles
+    out_host[2] = d[6];
+    out_host[5] = f * d[2]; out_host[6] = f * d[1]; out_host[7] = f * d[0];
+    out_host[3] = out_host[5] + out_host[6] + out_host[7];
+    out_host[4] = 0.5 * dV * d[5];
     return WDM_OK;
 }
 

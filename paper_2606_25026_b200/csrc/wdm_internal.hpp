@@ -19,13 +19,15 @@ struct SweepTable {
     Fact fact;
     int dtype;
     cudaError_t (*init)();                                               // opt in to > 48 KB dynamic shared memory
-    cudaError_t (*psi_z)(const void *params, int kick, cudaStream_t);    // contiguous axis, optional kick on load
-    cudaError_t (*psi_strided)(const void *params, int along_x, cudaStream_t);  // y axis (or x axis when G = 0)
-    cudaError_t (*psi_x_rho)(const void *params, int drift, cudaStream_t);  // x axis + density + R2C -> H
+    // diag: 0 plain; 1 the instantiation that also accumulates the per-step diagnostics into params->diag; 2 (psi sweeps,
+    // no kick) forward transform only, sum k^2 |F psi|^2 into params->diag, nothing written
+    cudaError_t (*psi_z)(const void *params, int kick, int diag, cudaStream_t);    // contiguous axis, optional kick on load
+    cudaError_t (*psi_strided)(const void *params, int along_x, int diag, cudaStream_t);  // y axis (or x axis when G = 0)
+    cudaError_t (*psi_x_rho)(const void *params, int drift, int diag, cudaStream_t);  // x axis + density + R2C -> H
     cudaError_t (*h_y_fwd)(const void *params, cudaStream_t);
-    cudaError_t (*h_z_green)(const void *params, cudaStream_t);
+    cudaError_t (*h_z_green)(const void *params, int diag, cudaStream_t);
     cudaError_t (*h_y_inv)(const void *params, cudaStream_t);
-    cudaError_t (*c2r)(const void *params, cudaStream_t);
+    cudaError_t (*c2r)(const void *params, int diag, cudaStream_t);
     // L2-chained forms (wdm_chain.cuh): z then y sweep of psi by x-planes; y forward, z Green, y inverse of H by
     // kx-planes.  chain_lag(stages, planes, requested) returns the lag to use (requested <= 0: automatic) or 0 when
     // no lag is both safe and meaningful for this size -- then the separate sweeps above must be used.

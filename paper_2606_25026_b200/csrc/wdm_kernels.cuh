@@ -150,6 +150,10 @@ struct SweepParams {
     // TMA descriptors of the array a strided sweep walks: boxes of (W elements along z) x (<= 256 rows along the
     // sweep axis); tmap2 is the one-row box that fetches row N/2 of the half spectrum in the complex-to-real sweep
     CUtensorMap tmap, tmap2;
+    // Per-step diagnostics (the DIAG instantiations only): accumulators of THIS step, and the set the
+    // next step will use, zeroed by this launch.  Layout (doubles): [0..2] sum k_a^2 |F_a psi|^2 from the z, y, x sweeps,
+    // [3] sum |psi_2|^2, [4] max |psi_2|^2 (bit pattern), [5] sum_k w_kx green(k) |rho~_k|^2, [6] max |Phi| (bit pattern)
+    double *diag, *diag_zero;
     unsigned int *ticket;      // tile tickets drawn in this launch (0 when the launch starts)
     unsigned int *ticket_next; // the next launch's counter: this launch zeroes it (launches alternate between two words)
 };
@@ -208,5 +212,31 @@ WDM_DEV void split(int b, int &g, int &l)
 }
 
 enum { H_Y_FWD = 0, H_Z_GREEN = 1, H_Y_INV = 2 };
+
+// per-thread accumulators of a DIAG sweep, kept for the whole kernel and reduced once per CTA at its end
+struct DiagAcc {
+    double s0 = 0.0, s1 = 0.0, mx = 0.0;
+};
+enum { DIAG_COUNT = 8 };
+// block reduction of (s0, s1, mx) over the CTA and one atomic each into d[i0], d[i1], d[imx] (an index < 0: nothing)
+__device__ __forceinline__ void diag_flush(double *d, const DiagAcc &a, int i0, int i1, int imx)
+{
+    __shared__ double r0[32], r1[32], rm[32];
+    double s0 = a.s0, s1 = a.s1, mx = a.mx;
+    for (int o = 16; o; o >>= 1) {
+        s0 += __shfl_down_sync(0xffffffffu, s0, o);
+        s1 += __shfl_down_sync(0xffffffffu, s1, o);
+        mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
+    }
+    const int w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if ((threadIdx.x & 31) == 0) { r0[w] = s0; r1[w] = s1; rm[w] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < nw; ++k) { s0 += r0[k]; s1 += r1[k]; mx = fmax(mx, rm[k]); }
+        if (i0 >= 0) atomicAdd(d + i0, s0);
+        if (i1 >= 0) atomicAdd(d + i1, s1);
+        if (imx >= 0) atomicMax(reinterpret_cast<unsigned long long *>(d + imx), (unsigned long long)__double_as_longlong(mx));
+    }
+}
 
 }  // namespace wdm

@@ -170,6 +170,8 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
     }
     asm volatile("griddepcontrol.wait;" ::: "memory");         // the previous kernel on the stream is complete and visible
     if (tid == 0 && bid == 0) *p.ticket_next = 0;               // the launch before this one has finished with it
+    if constexpr (K::DG == 1)
+        if (bid == 0 && tid < DIAG_COUNT && p.diag_zero && K::DIAG_ZEROES) p.diag_zero[tid] = 0.0;
     __syncthreads();
     for (int k = 0; k < NBUF; ++k)
         if (k % NG == grp && gt < 32 && tile_of[k] >= 0) K::issue(p, tile_of[k], smem + (size_t)k * K::TILE_BYTES, full + k, gt);
@@ -217,6 +219,10 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
             }
             if (tn >= 0) K::issue(p, tn, buf, full + b, gt);
         }
+    }
+    if constexpr (K::DG != 0) {
+        __syncthreads();
+        K::flush(p, pre);
     }
 }
 
@@ -389,7 +395,7 @@ __device__ __forceinline__ void half_spectrum_items(int gt, F &&f)
     }
 }
 
-struct NoPre {};
+struct NoPre { DiagAcc d; };
 
 constexpr size_t align128(size_t x) { return (x + 127) & ~(size_t)127; }
 
@@ -400,8 +406,15 @@ constexpr size_t align128(size_t x) { return (x + 127) & ~(size_t)127; }
 // formed from the outgoing registers, packed real-to-complex FFT along x in the same buffer -> H.
 // KICK: 0 none, 1 plain potential kick, 2 with the extra terms of SweepParams::kick_extra (a separate
 // instantiation, so the plain kernel carries none of their code or registers).
-template <class C_, int AX, int KICK, bool RHO, bool DRIFT>
+// DG_: 0 no diagnostics; 1 accumulate the per-step diagnostics on the way (sum k^2 |F psi|^2 of this axis in the middle
+// level -- the drift multiplies the spectrum by unit-modulus factors, so each axis sweep sees the kinetic energy of
+// its own axis; with RHO also sum and max of |psi_2|^2 from the outgoing registers); 2 measure only: forward transform,
+// accumulate, nothing written (the on-demand kinetic energy of wdm_get_diagnostics).
+template <class C_, int AX, int KICK, bool RHO, bool DRIFT, int DG_ = 0>
 struct PsiK {
+    static constexpr int DG = DG_;
+    static constexpr bool DIAG_ZEROES = AX == AX_CONTIG;        // the z sweep opens a step
+    static_assert(DG_ != 2 || (KICK == 0 && !RHO && DRIFT), "measure-only sweeps are plain forward transforms");
     using C = C_;
     using T = typename C::T;
     using TL = Tile<C, AX>;
@@ -416,7 +429,11 @@ struct PsiK {
     // the thread's FIRST level-A butterfly only.  The rest are loaded at the top of the tile's first phase and
     // arrive while the first butterfly computes -- half the registers held through the radix-32 middle level.
     static constexpr int PF = 1;
-    struct Pre { T th[KICK ? PF : 1][KICK ? RA : 1]; };
+    struct Pre { T th[KICK ? PF : 1][KICK ? RA : 1]; DiagAcc d; };
+    static __device__ __forceinline__ void flush(const SweepParams<T> &p, const Pre &pre)
+    {
+        diag_flush(p.diag, pre.d, AX == AX_CONTIG ? 0 : (AX == AX_Y ? 1 : 2), RHO ? 3 : -1, RHO ? 4 : -1);
+    }
     static constexpr bool PAIR = ax_strided(AX) && pair_ok<C>();
     // the density sweep is short of registers at the end of its last psi stage (two lines of outputs, their
     // |psi|^2 and the twiddles): it fetches the twiddles where it needs them instead of keeping them
@@ -514,9 +531,24 @@ struct PsiK {
             group_sync(grp, NTG);
             auto idx = [](int row, int l) { return L::idx(row, l); };
             g_fwd_B<C, W>(S, tb.twB, gt, grp, idx);
+            T tsum = (T)0;                                 // this tile's share of sum k^2 |F psi|^2 (DG)
+            if constexpr (DG == 2) {
+                for (int b = gt; b < (N / RM) * W; b += NTG) {
+                    int l = b % W, g = b / W;
+                    mid_fwd<RM, T>(g * RM, [&](int row) { return S[L::idx(row, l)]; },
+                                   [&](int row, cx<T> v) { tsum += ldg(p.ksq_pos + row) * (v.x * v.x + v.y * v.y); });
+                }
+                pre.d.s0 += (double)tsum;
+                return;
+            }
             for (int b = gt; b < (N / RM) * W; b += NTG) {
                 int l = b % W, g = b / W;
                 auto mul = [&](int pos, cx<T> &a, cx<T> &c) {
+                    if constexpr (DG == 1) {
+                        T ka, kc;
+                        ld2r(p.ksq_pos + pos, ka, kc);
+                        tsum += ka * (a.x * a.x + a.y * a.y) + kc * (c.x * c.x + c.y * c.y);
+                    }
                     cx<T> pa, pc;
                     ld2(tb.phase + pos, pa, pc);          // both kinetic factors in one 16-byte load
                     a = cmul(a, pa);
@@ -529,6 +561,7 @@ struct PsiK {
                     mid_both<RM, T>(g * RM, [&](int row) { return S[L::idx(row, l)]; },
                                     [&](int row, cx<T> v) { S[L::idx(row, l)] = v; }, mul);
             }
+            if constexpr (DG == 1) pre.d.s0 += (double)tsum;
             group_sync(grp, NTG);
             g_inv_B<C, W>(S, tb.twB, gt, grp, idx);
             hook();
@@ -584,6 +617,19 @@ struct PsiK {
                     });
                 });
             }
+        }
+        if constexpr (RHO && DG == 1) {
+            // mass and peak density of psi_2 (Alg. 1 l.12; the maxima feed Eq. 26) from the registers
+            T rs = (T)0, rm = (T)0;
+            static_for<0, (PAIR ? 2 : ITER)>([&](auto it_) {
+                static_for<0, RA>([&](auto r_) {
+                    const T v = rho[decltype(it_)::value][decltype(r_)::value];
+                    rs += v;
+                    rm = fmax(rm, v);
+                });
+            });
+            pre.d.s1 += (double)rs;
+            pre.d.mx = fmax(pre.d.mx, (double)rm);
         }
         if constexpr (RHO) {
             // rho tile as N rows x W reals == N rows x W/2 packed complex lines (lines 2l', 2l'+1)
@@ -664,8 +710,11 @@ struct PsiK {
 };
 
 // ---------------------------------------------------------------- Poisson sweeps on the half spectrum
-template <class C_, int MODE>
+template <class C_, int MODE, int DG_ = 0>
 struct HK {
+    static constexpr int DG = DG_;                              // 1 (Green sweep only): W = 1/2 sum rho Phi, spectrally
+    static constexpr bool DIAG_ZEROES = false;
+    static_assert(DG_ == 0 || MODE == H_Z_GREEN, "only the Green sweep accumulates");
     using C = C_;
     using T = typename C::T;
     static constexpr int AX = (MODE == H_Z_GREEN) ? AX_CONTIG : AX_Y;
@@ -675,6 +724,7 @@ struct HK {
     static constexpr size_t TILE_BYTES = align128(L::ELEMS * sizeof(cx<T>));
     static constexpr int AUX = MODE == H_Z_GREEN ? AUX_KSQ : AUX_NONE;
     using Pre = NoPre;
+    static __device__ __forceinline__ void flush(const SweepParams<T> &p, const Pre &pre) { diag_flush(p.diag, pre.d, 5, -1, -1); }
     static constexpr bool PAIR = ax_strided(AX) && pair_ok<C>();
     using Pers = PairTw<C, PAIR>;
     // (first warp of the group, lane = gt)
@@ -684,7 +734,7 @@ struct HK {
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
     template <class HOOK>
-    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &,
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &pre,
                                                    const Pers &pers, HOOK &&)
     {
         cx<T> *S = reinterpret_cast<cx<T> *>(buf);
@@ -722,18 +772,23 @@ struct HK {
                 int pen = t * W + l, kx = pen / N, ypos = pen - kx * N;
                 T kxy = ldg(p.ksq_nat + kx) + tb.ksq_pos[ypos];
                 bool zero_line = (kx == 0 && ypos == 0);
+                T wsum = (T)0;
                 auto mul = [&](int pos, cx<T> &a, cx<T> &c) {
                     T ka, kc;
                     ld2r(tb.ksq_pos + pos, ka, kc);
                     T ga = (zero_line && pos == 0) ? (T)0 : green_over(p.green, kxy + ka);
+                    const T gc = green_over(p.green, kxy + kc);
+                    if constexpr (DG == 1) wsum += ga * (a.x * a.x + a.y * a.y) + gc * (c.x * c.x + c.y * c.y);
                     a = cscale(a, ga);
-                    c = cscale(c, green_over(p.green, kxy + kc));
+                    c = cscale(c, gc);
                 };
                 if constexpr (L::VEC2)
                     mid_both2<RM, T>(g * RM, [&](int row, cx<T> &a, cx<T> &c) { ld2(S + L::idx(row, l), a, c); },
                                      [&](int row, cx<T> a, cx<T> c) { st2(S + L::idx(row, l), a, c); }, mul);
                 else
                     mid_both<RM, T>(g * RM, ldS(l), stS(l), mul);
+                // conj(rho~_k) Phi~_k over the FULL spectrum: rows 0 < kx < N/2 stand for their mirrors too
+                if constexpr (DG == 1) pre.d.s0 += (double)wsum * ((kx == 0 || kx == N / 2) ? 1.0 : 2.0);
             }
             group_sync(grp, NTG);
             g_inv_B<C, W>(S, tb.twB, gt, grp, idx);
@@ -767,8 +822,10 @@ struct HK {
 // complex-to-real inverse along x: H[kx <= N/2][y][z] -> Phi[x][y][z]; lines (2l', 2l'+1) share one FFT.
 // Buffer = [packed tile: N rows x W/2 complex][raw tile: N/2+1 rows x W complex, filled by the async copies].
 // EXT: add the static external potential on the way out (SweepParams::phi_ext != nullptr), a separate instantiation
-template <class C_, bool EXT = false>
+template <class C_, bool EXT = false, int DG_ = 0>
 struct C2RK {
+    static constexpr int DG = DG_;                              // 1: max |Phi_total| from the outgoing registers
+    static constexpr bool DIAG_ZEROES = false;
     using C = C_;
     using T = typename C::T;
     using TL = Tile<C, AX_X>;
@@ -779,6 +836,7 @@ struct C2RK {
     static constexpr size_t TILE_BYTES = PACKED_BYTES + align128((size_t)(N / 2 + 1) * W * sizeof(cx<T>));
     static constexpr int AUX = AUX_NONE;
     using Pre = NoPre;
+    static __device__ __forceinline__ void flush(const SweepParams<T> &p, const Pre &pre) { diag_flush(p.diag, pre.d, -1, -1, 6); }
     static constexpr bool PAIR = pair_ok<C>();          // packed line gt % (W/2), butterfly gt / (W/2): the PairTw twiddles
     using Pers = PairTw<C, PAIR>;
     static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar, int lane)
@@ -787,11 +845,12 @@ struct C2RK {
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
     template <class HOOK>
-    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &,
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &pre,
                                                    const Pers &pers, HOOK &&)
     {
         cx<T> *Sp = reinterpret_cast<cx<T> *>(buf);
         const cx<T> *R = reinterpret_cast<const cx<T> *>(buf + PACKED_BYTES);
+        T pmax = (T)0;
         const TL tile(p, t);
         // Z_k = A_k + i B_k,  Z_{N-k} = conj(A_k) + i conj(B_k)
         // Rows kx = 0 and kx = N/2 are the x-spectrum of REAL lines at a self-mirrored frequency: real in exact
@@ -830,11 +889,13 @@ struct C2RK {
                     v.x += e.x;
                     v.y += e.y;
                 }
+                if constexpr (DG == 1) pmax = fmax(pmax, fmax(fabs(v.x), fabs(v.y)));
                 stv(reinterpret_cast<cx<T> *>(gp + (long long)(row - q) * TL::RSTRIDE), v);
             };
             if constexpr (PAIR) inv_level_w<RA, T>(q, mA, pers.w, [&](int row) { return Sp[PK::idxA(q, row - q, l)]; }, out);
             else inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return Sp[PK::idxA(q, row - q, l)]; }, out);
         }
+        if constexpr (DG == 1) pre.d.mx = fmax(pre.d.mx, (double)pmax);
     }
 };
 

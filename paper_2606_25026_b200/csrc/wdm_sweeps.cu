@@ -113,6 +113,20 @@ using HZG = HK<C, H_Z_GREEN>;
 using HYI = HK<C, H_Y_INV>;
 using C2R = C2RK<C, false>;
 using C2RExt = C2RK<C, true>;
+// the same sweeps accumulating the per-step diagnostics (wdm_set_step_diagnostics), and the forward-only sweeps that
+// measure the spectral kinetic energy on demand (wdm_get_diagnostics)
+using PsiZKickD = PsiK<C, AX_CONTIG, 1, false, true, 1>;
+using PsiZKickXD = PsiK<C, AX_CONTIG, 2, false, true, 1>;
+using PsiZD = PsiK<C, AX_CONTIG, 0, false, true, 1>;
+using PsiSD = PsiK<C, AX_Y, 0, false, true, 1>;
+using PsiXD = PsiK<C, AX_X, 0, false, true, 1>;
+using PsiXRhoD = PsiK<C, AX_X, 0, true, true, 1>;
+using HZGD = HK<C, H_Z_GREEN, 1>;
+using C2RD = C2RK<C, false, 1>;
+using C2RExtD = C2RK<C, true, 1>;
+using PsiZM = PsiK<C, AX_CONTIG, 0, false, true, 2>;
+using PsiSM = PsiK<C, AX_Y, 0, false, true, 2>;
+using PsiXM = PsiK<C, AX_X, 0, false, true, 2>;
 
 cudaError_t init()
 {
@@ -123,6 +137,7 @@ cudaError_t init()
     g_ctas = sms * C::MINB;
 #define OPT(K) if ((e = optin<K>()) != cudaSuccess) return e;
     OPT(PsiZKick) OPT(PsiZKickX) OPT(C2RExt) OPT(PsiZ) OPT(PsiS) OPT(PsiX) OPT(PsiXRho) OPT(RhoOnly) OPT(HYF) OPT(HZG) OPT(HYI) OPT(C2R)
+    OPT(PsiZKickD) OPT(PsiZKickXD) OPT(PsiZD) OPT(PsiSD) OPT(PsiXD) OPT(PsiXRhoD) OPT(HZGD) OPT(C2RD) OPT(C2RExtD) OPT(PsiZM) OPT(PsiSM) OPT(PsiXM)
 #undef OPT
     g_chain_ctas = g_ctas;
     if ((e = chain_optin<PsiZKick, PsiS>(sms)) != cudaSuccess) return e;
@@ -167,24 +182,32 @@ cudaError_t h_yzy(const void *py, const void *pz, const ChainCtl *ctl, cudaStrea
     return chain_launch<HYF, HZG, HYI>(cp, C::N / 2 + 1, ctl, s);
 }
 
-cudaError_t psi_z(const void *pp, int kick, cudaStream_t s)
+// diag: 0 plain, 1 accumulate the per-step diagnostics, 2 (psi sweeps without kick only) measure, write nothing
+cudaError_t psi_z(const void *pp, int kick, int diag, cudaStream_t s)
 {
+    if (diag == 2) return launch<PsiZM>(pp, kTilesGrid, s);
+    if (diag == 1) return kick == 2 ? launch<PsiZKickXD>(pp, kTilesGrid, s) : (kick ? launch<PsiZKickD>(pp, kTilesGrid, s) : launch<PsiZD>(pp, kTilesGrid, s));
     return kick == 2 ? launch<PsiZKickX>(pp, kTilesGrid, s) : (kick ? launch<PsiZKick>(pp, kTilesGrid, s) : launch<PsiZ>(pp, kTilesGrid, s));
 }
-cudaError_t psi_strided(const void *pp, int along_x, cudaStream_t s)
+cudaError_t psi_strided(const void *pp, int along_x, int diag, cudaStream_t s)
 {
+    if (diag == 2) return along_x ? launch<PsiXM>(pp, kTilesGrid, s) : launch<PsiSM>(pp, kTilesGrid, s);
+    if (diag == 1) return along_x ? launch<PsiXD>(pp, kTilesGrid, s) : launch<PsiSD>(pp, kTilesGrid, s);
     return along_x ? launch<PsiX>(pp, kTilesGrid, s) : launch<PsiS>(pp, kTilesGrid, s);
 }
-cudaError_t psi_x_rho(const void *pp, int drift, cudaStream_t s)
+cudaError_t psi_x_rho(const void *pp, int drift, int diag, cudaStream_t s)
 {
+    if (diag == 1 && drift) return launch<PsiXRhoD>(pp, kTilesGrid, s);
     return drift ? launch<PsiXRho>(pp, kTilesGrid, s) : launch<RhoOnly>(pp, kTilesGrid, s);
 }
 cudaError_t h_y_fwd(const void *pp, cudaStream_t s) { return launch<HYF>(pp, kTilesHalf, s); }
-cudaError_t h_z_green(const void *pp, cudaStream_t s) { return launch<HZG>(pp, kTilesHalf, s); }
+cudaError_t h_z_green(const void *pp, int diag, cudaStream_t s) { return diag == 1 ? launch<HZGD>(pp, kTilesHalf, s) : launch<HZG>(pp, kTilesHalf, s); }
 cudaError_t h_y_inv(const void *pp, cudaStream_t s) { return launch<HYI>(pp, kTilesHalf, s); }
-cudaError_t c2r(const void *pp, cudaStream_t s)
+cudaError_t c2r(const void *pp, int diag, cudaStream_t s)
 {
-    return static_cast<const P *>(pp)->phi_ext ? launch<C2RExt>(pp, kTilesGrid, s) : launch<C2R>(pp, kTilesGrid, s);
+    const bool ext = static_cast<const P *>(pp)->phi_ext != nullptr;
+    if (diag == 1) return ext ? launch<C2RExtD>(pp, kTilesGrid, s) : launch<C2RD>(pp, kTilesGrid, s);
+    return ext ? launch<C2RExt>(pp, kTilesGrid, s) : launch<C2R>(pp, kTilesGrid, s);
 }
 
 const SweepTable kTable = {Fact{C::N, C::RA, C::RB, C::RM, C::W, C::NT, C::NG, C::MINB}, WDM_DTYPE, init, psi_z,

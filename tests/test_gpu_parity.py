@@ -765,7 +765,7 @@ def test_diagnostics_match_oracle(wdm, dtype, N, rtol):
     w = wl.Workload(f"diag{N}", N, dtype, 2, L=1.3, hbar_over_m=0.8, G=30.0, psi=psi0)
     dt = 0.2 * (w.L / N) ** 2
     sim, o = pair(wdm, w)
-    keys = ("M", "max_rho", "max_phi", "V", "K", "Q", "dt_max")
+    keys = ("M", "max_rho", "max_phi", "V", "K", "Q", "dt_max", "T", "W", "E")
     # Initial state: both sides hold the SAME psi (the cast array), and both evaluate M, max rho, K, Q in float64 from
     # it: only the summation order differs.  max|Phi|, V and dt_max depend on the potential, which the complex64 path
     # holds in float32: the field tolerance of north_star (rel-L2 2e-5; measured 1e-7..2e-7 here), no extra factor.
@@ -775,6 +775,7 @@ def test_diagnostics_match_oracle(wdm, dtype, N, rtol):
         o.set_kick_terms(kappa=kappa)
         a, b = sim.diagnostics(), o.diagnostics()
         for key in keys:
+            # (T is summed in the grid precision inside the measuring sweeps: the field tolerance, like the Phi-dependent ones)
             bound = (psi_only if key in ("M", "max_rho", "K", "Q") else max(rtol, psi_only)) * max(abs(b[key]), 1e-300)
             assert abs(a[key] - b[key]) <= bound, (key, a[key], b[key])
     sim.set_kick_terms(); o.set_kick_terms()
@@ -784,6 +785,70 @@ def test_diagnostics_match_oracle(wdm, dtype, N, rtol):
     a, b = sim.diagnostics(), o.diagnostics()
     for key in keys:
         assert abs(a[key] - b[key]) <= 2 * max(tol(dtype, 2), psi_only) * abs(b[key]), (key, a[key], b[key])
+    sim.close()
+
+
+@pytest.mark.parametrize("dtype,N,case", [("c128", 32, "plain"), ("c64", 64, "plain"), ("c64", 256, "plain"), ("c64", 512, "plain"),
+                                          ("c128", 64, "terms"), ("c64", 128, "terms"), ("c64", 16, "particles"), ("c128", 16, "particles"),
+                                          ("c64", 64, "free")])
+def test_step_diagnostics_fused_in_the_sweeps(wdm, dtype, N, case):
+    """wdm_set_step_diagnostics: M, max |psi_2|^2, max |Phi|, T per axis (spectral, middle level of each psi sweep) and
+    W (spectral, Green sweep) of the last step, reduced inside the sweeps -- against the oracle's record of the same state
+    (between Eq. 18(c) and (d)), with the launch count per step unchanged.  Every quantity is quadratic in fields that
+    agree to tol: twice the field tolerance."""
+    if case == "particles":
+        w = wl.small_coupled(N, dtype=dtype)
+        dt, nsteps = w.dt, 3
+    else:
+        psi0 = (0.3 * wl.random_field(N, dtype, 300 + N) + 1.0).astype(np.complex64 if dtype == "c64" else np.complex128)
+        w = wl.Workload(f"sdiag{N}", N, dtype, 3, L=1.3, hbar_over_m=0.8, G=0.0 if case == "free" else 30.0, psi=psi0)
+        dt, nsteps = 0.2 * (w.L / N) ** 2, 3
+    sim, o = pair(wdm, w, 0 if w.pos is None else len(w.pos))
+    if case == "terms":
+        ext = _ext_potential(N, w.L, 25.0).astype(np.float32 if dtype == "c64" else np.float64)
+        kw = dict(kappa=-40.0, phi_ext=ext, absorb_alpha=3.0 / dt / 8, absorb_nb=12)
+        sim.set_kick_terms(**kw); o.set_kick_terms(**kw)
+    with pytest.raises(wdm.WdmError) as e:
+        sim.step_diagnostics()
+    assert e.value.code == wdm.WDM_ESTATE
+    sim.set_step_diagnostics(True); o.set_step_diagnostics(True)
+    sim.step(1, dt); o.step(1, dt)                       # a first call, so that the second starts from a merged kick
+    n0 = wdm.wdm_launch_count(sim.h)
+    sim.step(nsteps, dt); o.step(nsteps, dt)
+    per_step = 7 if w.G > 0 else 3
+    extra = 0 if w.pos is None else 3 * nsteps           # push, clear, deposit
+    assert wdm.wdm_launch_count(sim.h) - n0 == per_step * nsteps + extra
+    a, b = sim.step_diagnostics(), o.step_diagnostics()
+    t = 2 * max(tol(dtype, nsteps + 1), 1e-11)
+    keys = ("T", "Tx", "Ty", "Tz") if w.G == 0 else ("M", "max_rho", "max_phi", "T", "W", "Tx", "Ty", "Tz")
+    for key in keys:
+        assert abs(a[key] - b[key]) <= t * abs(b[key]), (key, a[key], b[key])
+    # the fields themselves are what they are without the accumulation
+    check_fields(sim, o, dtype, nsteps + 1, "with step diagnostics")
+    # switching off returns to the plain instantiations; the record is gone
+    sim.set_step_diagnostics(False)
+    sim.step(1, dt); o.step(1, dt)
+    with pytest.raises(wdm.WdmError):
+        sim.step_diagnostics()
+    check_fields(sim, o, dtype, nsteps + 2, "after step diagnostics")
+    sim.close()
+
+
+def test_energy_conservation_from_step_diagnostics_c64(wdm):
+    """E = T + W from the fused record stays constant to O(dt^2) over a run ("total energy broadly
+    conserved"; pin P6/P17 on the oracle): 128^3 complex64, strong gravity, 40 steps, read every 10."""
+    N = 128
+    psi0 = (0.2 * wl.random_field(N, "c64", 5) + 1.0).astype(np.complex64)
+    sim = wdm.Sim(N, 1.0, 1.0, 50.0 / (4 * math.pi), "c64")
+    sim.set_psi(psi0)
+    sim.set_step_diagnostics(True)
+    dt = (1.0 / N) ** 2 / 6
+    E = []
+    for _ in range(4):
+        sim.step(10, dt)
+        d = sim.step_diagnostics()
+        E.append(d["T"] + d["W"])
+    assert max(abs(e - E[0]) for e in E) <= 2e-5 * abs(E[0]), E
     sim.close()
 
 
