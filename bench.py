@@ -39,10 +39,6 @@ UNIT = "cell-updates/s"
 ALG_BYTES_PER_CELL_C = {
     "psi_sweep_z_kick": 2.5, "psi_sweep_y": 2.0, "psi_sweep_x_rho_r2c": 2.5,
     "poisson_y_fwd": 1.0, "poisson_z_green": 1.0, "poisson_y_inv": 1.0, "poisson_x_c2r": 1.0,
-    # L2-chained kernels do the work of several sweeps of the SURVEY 8(d) table: their algorithmic bytes are the sum
-    # of those sweeps (what bench reports as `achieved`); HBM_MIN_* is what must cross HBM once the later stages
-    # read from L2 (first stage's read + last stage's write)
-    "psi_chain_z_kick_y": 4.5, "poisson_chain_y_zgreen_y": 3.0,
 }
 # The CPU oracle is timed on ONE sample, in the reference arm and in the cpu_baseline leg alike: the soliton + halo
 # recipe of the bench workload at 256^3 (float64, 0.3 s per KDK step on 16 host cores; 512^3 would need 6.5 GB and
@@ -51,7 +47,6 @@ REF_SAMPLE_N = 256
 # algorithmic HBM bytes per particle of the particle kernels (pos, vel read + write in the push,
 # pos read in the deposit; the gathered Phi nodes and the deposited rho_p nodes go through L2)
 PARTICLE_BYTES = {"particle_gather_kick_drift": 48, "particle_cic_deposit": 12}
-HBM_MIN_PER_CELL_C = dict(ALG_BYTES_PER_CELL_C, psi_chain_z_kick_y=2.5, poisson_chain_y_zgreen_y=1.0)
 
 
 def make_workload(name: str):
@@ -253,7 +248,6 @@ def main():
                    "particles": npart, "dt": dt, "timed_call": f"wdm_step({K}, dt)",
                    "l2": "inputs larger than L2 (psi alone is %.2f GB vs 126 MB L2), no flush" % (N ** 3 * 8 / 1e9)
                          if N >= 512 else "working set near/below L2: L2-resident, launch-bound regime",
-                   "chain_lag_planes": list(wdm.wdm_get_chain(sim.h)),
                    "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU"},
         "gpu_launches": launches, "clocks": clk.summary(),
     }
@@ -273,7 +267,6 @@ def main():
         dom = max((k for k in kern if k in ALG_BYTES_PER_CELL_C), key=lambda k: kern[k]["launches"] * kern[k]["avg_ms"])
         peak, how = peaks()
         alg = ALG_BYTES_PER_CELL_C[dom] * csize * N ** 3
-        step_min = sum(HBM_MIN_PER_CELL_C[k] for k in kern if k in HBM_MIN_PER_CELL_C and kern[k]["launches"] >= kp) * csize * N ** 3
         achieved = alg / (kern[dom]["avg_ms"] * 1e-3) / 1e9
         traffic = None
         tp = os.path.join(ROOT, "profiles", "traffic.json")
@@ -281,15 +274,12 @@ def main():
             traffic = json.load(open(tp)).get(w.name, {}).get(dom)
         out["roofline"] = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                            "frac": achieved / peak, "traffic": traffic, "peak_source": how,
-                           "alg_bytes_per_launch": alg, "hbm_min_bytes_per_launch": HBM_MIN_PER_CELL_C[dom] * csize * N ** 3,
+                           "alg_bytes_per_launch": alg,
                            "whole_step": {"alg_bytes_per_step": 11 * csize * N ** 3,
                                           "achieved": 11 * csize * N ** 3 / (ms / K * 1e-3) / 1e9,
                                           "frac": 11 * csize * N ** 3 / (ms / K * 1e-3) / 1e9 / peak,
                                           "frac_of_nominal_8TBs": 11 * csize * N ** 3 / (ms / K * 1e-3) / 1e9 / 8000.0,
-                                          "note": "11c per cell = SURVEY 8(d) count for seven separate sweeps; "
-                                                  "hbm_min_* counts what the launched (chained) kernels must move",
-                                          "hbm_min_bytes_per_step": step_min,
-                                          "hbm_min_frac": step_min / (ms / K * 1e-3) / 1e9 / peak}}
+                                          "note": "11c per cell = SURVEY 8(d) count for the seven sweeps of a step"}}
         out["kernels"] = kern
         if npart:
             # particle kernels against their own HBM count; the rho_p clear (one real per cell, "particle_mesh_clear")

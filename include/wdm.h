@@ -150,7 +150,7 @@ int wdm_get_diagnostics(wdm_ctx *ctx, double *out_host);
 
 /* Diagnostics accumulated INSIDE the sweeps of a step, at no extra pass over the grid and no extra kernel launch
  * (SURVEY 8(f) rank 2): while switched on, wdm_step uses instantiations of its sweeps that also reduce what they have
- * in registers (the L2-chained forms are not used meanwhile).  wdm_get_step_diagnostics returns, for the LAST step run,
+ * in registers.  wdm_get_step_diagnostics returns, for the LAST step run,
  * the state between Eq. 18(c) and (d) -- psi_2 after the drift, before the closing half kick, the
  * Poisson source rho = |psi_2|^2 + particles and the potential just solved from it; synchronises the stream.
  * out_host must hold 8 doubles:
@@ -163,18 +163,6 @@ int wdm_get_diagnostics(wdm_ctx *ctx, double *out_host);
  * E = T + W is the conserved energy of the pure SPE.  WDM_ESTATE until a step has run. */
 int wdm_set_step_diagnostics(wdm_ctx *ctx, int on);
 int wdm_get_step_diagnostics(wdm_ctx *ctx, double *out_host);
-
-/* Execution mode of the plane-local sweeps (no effect on results beyond rounding order).
- * mode is a bit mask.  Bit 0 (1): the z and y sweeps of psi (Eq. 18(b)) run as one
- * kernel.  Bit 1 (2): the y-forward, z-Green, y-inverse sweeps of the Poisson solve (Eq. 18(c)
- * PAPER.md:194, Eq. 23) run as one kernel.  In a chained kernel the later stage trails
- * the earlier one by `lag` x-planes and reads them from L2 instead of HBM.  mode 0: one launch per
- * sweep.  Default: 0.  lag <= 0 picks the lag automatically.  wdm_get_chain reports the lags in use
- * (0 = that chain runs as separate sweeps, e.g. because the grid is too small for it to be
- * meaningful).  The environment variables WDM_CHAIN=<mode> and WDM_CHAIN_LAG=<planes> set the
- * defaults of new contexts. */
-int wdm_set_chain(wdm_ctx *ctx, int mode, int lag);
-int wdm_get_chain(wdm_ctx *ctx, int *lag_psi_out, int *lag_poisson_out);
 
 /* Instrumentation.  wdm_launch_count: kernels launched by this context so far.  With profiling on,
  * every kernel launch is bracketed by CUDA events on the context's stream;

@@ -48,7 +48,7 @@ def lib():
             "wdm_get_psi_host": [vp, vp], "wdm_get_density_host": [vp, vp], "wdm_get_potential_host": [vp, vp],
             "wdm_get_particles_host": [vp, vp, vp],
             "wdm_launch_count": [vp, C.POINTER(ll)], "wdm_set_profiling": [vp, i],
-            "wdm_set_kick_terms": [vp, d, vp, d, i], "wdm_get_diagnostics": [vp, C.POINTER(d)], "wdm_set_step_diagnostics": [vp, i], "wdm_get_step_diagnostics": [vp, C.POINTER(d)], "wdm_set_particle_mode": [vp, i, i], "wdm_set_assignment": [vp, i], "wdm_set_deposit_mode": [vp, i], "wdm_get_assignment": [vp, C.POINTER(i)], "wdm_set_chain": [vp, i, i], "wdm_get_chain": [vp, C.POINTER(i), C.POINTER(i)],
+            "wdm_set_kick_terms": [vp, d, vp, d, i], "wdm_get_diagnostics": [vp, C.POINTER(d)], "wdm_set_step_diagnostics": [vp, i], "wdm_get_step_diagnostics": [vp, C.POINTER(d)], "wdm_set_particle_mode": [vp, i, i], "wdm_set_assignment": [vp, i], "wdm_set_deposit_mode": [vp, i], "wdm_get_assignment": [vp, C.POINTER(i)],
             "wdm_kernel_stats": [vp, C.POINTER(i), C.POINTER(C.c_char_p), C.POINTER(ll), C.POINTER(d)],
         }
         for name, args in sig.items():
@@ -65,7 +65,7 @@ EXPORTS = ["wdm_workspace_bytes", "wdm_create", "wdm_create_ws", "wdm_destroy", 
            "wdm_set_psi_host", "wdm_set_particles", "wdm_set_particles_host", "wdm_step", "wdm_run_host",
            "wdm_get_psi", "wdm_get_density", "wdm_get_potential", "wdm_get_particles", "wdm_get_psi_host",
            "wdm_get_density_host", "wdm_get_potential_host", "wdm_get_particles_host", "wdm_launch_count",
-           "wdm_set_profiling", "wdm_kernel_stats", "wdm_last_error", "wdm_set_chain", "wdm_get_chain", "wdm_set_kick_terms", "wdm_get_diagnostics", "wdm_set_particle_mode", "wdm_set_assignment", "wdm_get_assignment", "wdm_set_deposit_mode", "wdm_set_step_diagnostics", "wdm_get_step_diagnostics"]
+           "wdm_set_profiling", "wdm_kernel_stats", "wdm_last_error", "wdm_set_kick_terms", "wdm_get_diagnostics", "wdm_set_particle_mode", "wdm_set_assignment", "wdm_get_assignment", "wdm_set_deposit_mode", "wdm_set_step_diagnostics", "wdm_get_step_diagnostics"]
 
 
 def _chk(rc, h=None):
@@ -216,17 +216,6 @@ def wdm_get_step_diagnostics(h):
     out = (C.c_double * 8)()
     _chk(lib().wdm_get_step_diagnostics(h, out), h)
     return dict(zip(("M", "max_rho", "max_phi", "T", "W", "Tx", "Ty", "Tz"), list(out)))
-
-
-def wdm_set_chain(h, mode, lag=0):
-    _chk(lib().wdm_set_chain(h, int(mode), int(lag)), h)
-
-
-def wdm_get_chain(h):
-    """(lag of the psi z->y chain, lag of the Poisson y->z->y chain) in x-planes; 0 = separate sweeps."""
-    a, b = C.c_int(), C.c_int()
-    _chk(lib().wdm_get_chain(h, C.byref(a), C.byref(b)), h)
-    return a.value, b.value
 
 
 def wdm_set_profiling(h, on):

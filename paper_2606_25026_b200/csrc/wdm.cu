@@ -178,11 +178,11 @@ __global__ void __launch_bounds__(256) k_diag(const cx<T> *__restrict__ psi, con
 }
 
 enum Slot { S_PSI_Z, S_PSI_Y, S_PSI_X_RHO, S_H_Y_FWD, S_H_Z_GREEN, S_H_Y_INV, S_C2R, S_KICK, S_PART_PUSH,
-            S_PART_DEPOSIT, S_PART_SORT, S_MISC, S_PSI_ZY, S_H_YZY, S_PART_CLEAR, S_COUNT };
+            S_PART_DEPOSIT, S_PART_SORT, S_MISC, S_PART_CLEAR, S_COUNT };
 static const char *kSlotNames[S_COUNT] = {"psi_sweep_z_kick", "psi_sweep_y", "psi_sweep_x_rho_r2c", "poisson_y_fwd",
                                           "poisson_z_green", "poisson_y_inv", "poisson_x_c2r", "kick_elementwise",
                                           "particle_gather_kick_drift", "particle_cic_deposit", "particle_cell_sort",
-                                          "misc", "psi_chain_z_kick_y", "poisson_chain_y_zgreen_y", "particle_mesh_clear"};
+                                          "misc", "particle_mesh_clear"};
 
 }  // namespace wdm
 
@@ -204,7 +204,6 @@ struct wdm_ctx {
     void *twA = nullptr, *twB = nullptr, *phase = nullptr, *ksq_pos = nullptr, *ksq_nat = nullptr;
     double phase_dt = 0;
     bool phase_valid = false, have_psi = false, stale = true;
-    // L2-chained sweeps (wdm_chain.cuh): completion counters, launch epochs, lag per chain (0: separate sweeps)
     // particle variants (wdm_set_particle_mode; reading G29)
     int nsub = 1;
     bool pstatic = false;
@@ -228,10 +227,9 @@ struct wdm_ctx {
     bool mask_valid = false;
     // TMA descriptors (see SweepParams): psi along y / x, H along y / x, H single row along x
     CUtensorMap tm_psi_y, tm_psi_x, tm_h_y, tm_h_x, tm_h_x1;
-    unsigned int *chain_done = nullptr;       // [N] for psi z->y, then [2 (N/2+1)] for H y->z->y
-    unsigned int epoch_psi = 0, epoch_h = 0;
-    int lag_psi = 0, lag_h = 0;
+    unsigned int *tickets = nullptr;          // two tile-ticket words used by alternate sweep launches
     int ticket_parity = 0;
+    int l2_reverse = 1;                       // see SweepParams::reverse (WDM_L2_REVERSE=0 switches it off for A/B runs)
     // closing half kicks not applied yet (dt of the call that owes them; 0 = none): they merge with the opening
     // half kick of the next wdm_step, or are applied when the state is read or a parameter changes
     double pend_psi = 0, pend_part = 0;
@@ -448,7 +446,7 @@ static int ensure_mask(wdm_ctx *c, double dt)
 template <typename T>
 static void take_ticket(wdm_ctx *c, SweepParams<T> &p)
 {
-    unsigned int *base = c->chain_done + 2 * c->N + 2;
+    unsigned int *base = c->tickets;
     p.ticket = base + c->ticket_parity;
     p.ticket_next = base + (c->ticket_parity ^ 1);
     c->ticket_parity ^= 1;
@@ -495,15 +493,11 @@ static int density_poisson(wdm_ctx *c, bool drift, int dg = 0)
     SweepParams<T> p = base_params<T>(c);
     p.data = (cx<T> *)c->H;
     p.tmap = c->tm_h_y;
-    if (c->lag_h > 0 && !dg) {
-        ChainCtl ctl{c->chain_done + N, ++c->epoch_h * (unsigned int)(N / c->tab->fact.W), c->lag_h};
-        Timed t(c, S_H_YZY);
-        CU(c, c->tab->h_yzy(&p, &p, &ctl, c->stream));
-    } else {
-        { take_ticket(c, p); Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
-        { take_ticket(c, p); Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, dg, c->stream)); }
-        { take_ticket(c, p); Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
-    }
+    { take_ticket(c, p); Timed t(c, S_H_Y_FWD); CU(c, c->tab->h_y_fwd(&p, c->stream)); }
+    p.reverse = c->l2_reverse;
+    { take_ticket(c, p); Timed t(c, S_H_Z_GREEN); CU(c, c->tab->h_z_green(&p, dg, c->stream)); }
+    p.reverse = 0;
+    { take_ticket(c, p); Timed t(c, S_H_Y_INV); CU(c, c->tab->h_y_inv(&p, c->stream)); }
     p.tmap = c->tm_h_x;
     p.tmap2 = c->tm_h_x1;
     { take_ticket(c, p); Timed t(c, S_C2R); CU(c, c->tab->c2r(&p, dg, c->stream)); }
@@ -630,7 +624,7 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
     const bool have_phi = grav || c->phi_ext != nullptr;                 // particles and psi feel a potential
     const bool layer = c->alpha > 0;
     const bool kicks = have_phi || c->kappa != 0.0 || layer;
-    const int dg = c->step_diag ? 1 : 0;                  // the accumulating instantiations (separate sweeps only)
+    const int dg = c->step_diag ? 1 : 0;                  // the accumulating instantiations
     if (dg) CU(c, cudaMemsetAsync(c->diag_dev + c->diag_set * DIAG_COUNT, 0, DIAG_COUNT * sizeof(double), c->stream));
     for (int s = 0; s < nsteps; ++s) {
         // merged closing (h_d, of the previous step -- possibly of the previous call) + opening (h_a) half kicks
@@ -653,14 +647,9 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             pz.kick_extra = (c->kappa != 0.0 || pz.mask != nullptr) ? 1 : 0;
             py.data = (cx<T> *)c->psi;
             py.tmap = c->tm_psi_y;
-            if (c->lag_psi > 0 && !pz.kick_extra && !dg) {
-                ChainCtl ctl{c->chain_done, ++c->epoch_psi * (unsigned int)(N / c->tab->fact.W), c->lag_psi};
-                Timed t(c, S_PSI_ZY);
-                CU(c, c->tab->psi_zy(&pz, &py, kicks ? 1 : 0, &ctl, c->stream));
-            } else {
-                { take_ticket(c, pz); Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? (pz.kick_extra ? 2 : 1) : 0, dg, c->stream)); }
-                { take_ticket(c, py); Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, dg, c->stream)); }
-            }
+            py.reverse = c->l2_reverse;
+            { take_ticket(c, pz); Timed t(c, S_PSI_Z); CU(c, c->tab->psi_z(&pz, kicks ? (pz.kick_extra ? 2 : 1) : 0, dg, c->stream)); }
+            { take_ticket(c, py); Timed t(c, S_PSI_Y); CU(c, c->tab->psi_strided(&py, 0, dg, c->stream)); }
         }
         c->pend_psi = 0.0;
         c->pend_part = 0.0;
@@ -742,22 +731,12 @@ static int create_common(wdm_ctx **out, int N, double L, double mu, double G, in
         (rc = ctx_alloc(c, &c->twB, N * cs)) || (rc = ctx_alloc(c, &c->phase, N * cs)) ||
         (rc = ctx_alloc(c, &c->ksq_pos, N * rs)) || (rc = ctx_alloc(c, &c->ksq_nat, N * rs)) ||
         (rc = ctx_alloc(c, &c->rho_mean, 64)) ||
-        (rc = ctx_alloc(c, (void **)&c->chain_done, (size_t)(2 * N + 2 + 8) * sizeof(unsigned int))) ||
+        (rc = ctx_alloc(c, (void **)&c->tickets, 8 * sizeof(unsigned int))) ||
         (rc = ctx_alloc(c, &c->mask, (size_t)3 * N * rs)) || (rc = ctx_alloc(c, (void **)&c->diag_dev, 3 * DIAG_COUNT * sizeof(double))))
         return bail(rc);
-    if (cudaMemset(c->chain_done, 0, (size_t)(2 * N + 2 + 8) * sizeof(unsigned int)) != cudaSuccess)
-        return bail(fail(c, WDM_ECUDA, "cudaMemset of the chain counters failed"));
-    {
-        const char *env = getenv("WDM_CHAIN");             // bit mask as in wdm_set_chain
-        const char *lag = getenv("WDM_CHAIN_LAG");
-        int req = lag ? atoi(lag) : 0;
-        // default: separate sweeps.  Measured at 512^3 (end of round 1): the chained Poisson kernel moves a third of
-        // the DRAM bytes of its three sweeps but takes 0.59 ms against their 0.57 ms (the y sweeps run at 93-95 % of
-        // the HBM floor on their own; the chain pays for its dependency waits), the psi pair is clearly slower
-        int mode = env ? atoi(env) : 0;
-        if (mode & 1) c->lag_psi = c->tab->chain_lag(2, N, req);
-        if (mode & 2) c->lag_h = c->tab->chain_lag(3, N / 2 + 1, req);
-    }
+    if (cudaMemset(c->tickets, 0, 8 * sizeof(unsigned int)) != cudaSuccess)
+        return bail(fail(c, WDM_ECUDA, "cudaMemset of the ticket words failed"));
+    if (const char *env = getenv("WDM_L2_REVERSE")) c->l2_reverse = atoi(env) != 0;
     rc = dtype == WDM_C64 ? upload_tables<float>(c) : upload_tables<double>(c);
     if (rc) return bail(rc);
     if ((rc = make_tmaps(c))) return bail(rc);
@@ -1106,23 +1085,6 @@ extern "C" int wdm_set_kick_terms(wdm_ctx *c, double kappa, const void *phi_ext_
     c->absorb_nb = absorb_nb;
     c->mask_valid = false;
     c->stale = true;                 // Phi_total changes with the external term
-    return WDM_OK;
-}
-
-extern "C" int wdm_set_chain(wdm_ctx *c, int mode, int lag)
-{
-    if (!c) return WDM_EINVAL;
-    if (mode < 0 || mode > 3) return fail(c, WDM_EINVAL, "mode is a bit mask: 1 = chain the psi z/y sweeps, 2 = chain the Poisson y/z/y sweeps");
-    c->lag_psi = (mode & 1) ? c->tab->chain_lag(2, c->N, lag) : 0;
-    c->lag_h = (mode & 2) ? c->tab->chain_lag(3, c->N / 2 + 1, lag) : 0;
-    return WDM_OK;
-}
-
-extern "C" int wdm_get_chain(wdm_ctx *c, int *lag_psi_out, int *lag_poisson_out)
-{
-    if (!c) return WDM_EINVAL;
-    if (lag_psi_out) *lag_psi_out = c->lag_psi;
-    if (lag_poisson_out) *lag_poisson_out = c->lag_h;
     return WDM_OK;
 }
 

@@ -6,14 +6,6 @@
 
 namespace wdm {
 
-// completion counters of a chained launch: (stages - 1) x planes words, zeroed once, monotone across launches;
-// `target` is the value a finished plane's counter has reached in this launch (epoch x tiles per plane)
-struct ChainCtl {
-    unsigned int *done;
-    unsigned int target;
-    int lag;
-};
-
 // Launchers of one (dtype, N) instantiation; params is a SweepParams<T> of the matching T.
 struct SweepTable {
     Fact fact;
@@ -28,12 +20,6 @@ struct SweepTable {
     cudaError_t (*h_z_green)(const void *params, int diag, cudaStream_t);
     cudaError_t (*h_y_inv)(const void *params, cudaStream_t);
     cudaError_t (*c2r)(const void *params, int diag, cudaStream_t);
-    // L2-chained forms (wdm_chain.cuh): z then y sweep of psi by x-planes; y forward, z Green, y inverse of H by
-    // kx-planes.  chain_lag(stages, planes, requested) returns the lag to use (requested <= 0: automatic) or 0 when
-    // no lag is both safe and meaningful for this size -- then the separate sweeps above must be used.
-    int (*chain_lag)(int stages, int planes, int requested);
-    cudaError_t (*psi_zy)(const void *params_z, const void *params_y, int kick, const ChainCtl *, cudaStream_t);
-    cudaError_t (*h_yzy)(const void *params_y, const void *params_z, const ChainCtl *, cudaStream_t);
 };
 
 const SweepTable *sweep_table(int dtype, int N);

@@ -154,6 +154,10 @@ struct SweepParams {
     // next step will use, zeroed by this launch.  Layout (doubles): [0..2] sum k_a^2 |F_a psi|^2 from the z, y, x sweeps,
     // [3] sum |psi_2|^2, [4] max |psi_2|^2 (bit pattern), [5] sum_k w_kx green(k) |rho~_k|^2, [6] max |Phi| (bit pattern)
     double *diag, *diag_zero;
+    // Tiles are handed out in decreasing order.  The y sweep of psi and the z-Green sweep of H run against the direction
+    // of the sweep before them (and the y-inverse sweep with the direction of the y-forward one again): each starts on
+    // the planes its predecessor wrote last, which are still in the 126 MB L2.
+    int reverse;
     unsigned int *ticket;      // tile tickets drawn in this launch (0 when the launch starts)
     unsigned int *ticket_next; // the next launch's counter: this launch zeroes it (launches alternate between two words)
 };

@@ -142,7 +142,7 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
         for (int b = 0; b < NBUF; ++b) {
             mbar_init(full + b, 1);
             const int t0 = bid + b * stride;
-            tile_of[b] = t0 < ntiles ? t0 : -1;
+            tile_of[b] = t0 < ntiles ? (p.reverse ? ntiles - 1 - t0 : t0) : -1;
             issued[b] = 1;
         }
     using SM = PipeSmem<K>;
@@ -212,6 +212,7 @@ __device__ __forceinline__ void pipe_run(const SweepParams<typename K::C::T> &p,
         if (gt < 32) {
             int tn = (int)__shfl_sync(0xffffffffu, ticket, 0);
             if (tn >= ntiles) tn = -1;
+            else if (p.reverse) tn = ntiles - 1 - tn;
             if (gt == 0) {
                 tile_of[b] = tn;
                 __threadfence_block();

@@ -1,7 +1,7 @@
 // wdm_sweeps.cu -- __global__ wrappers of the pipelined sweeps for ONE (dtype, N), selected at compile time
 // with -DWDM_DTYPE={0,1} -DWDM_N=<N>.  build.py compiles this file once per supported size.
 #include "wdm_internal.hpp"
-#include "wdm_chain.cuh"
+#include "wdm_pipe.cuh"
 
 #ifndef WDM_DTYPE
 #error "compile with -DWDM_DTYPE=0|1 -DWDM_N=<N>"
@@ -41,13 +41,6 @@ __global__ void __launch_bounds__(kThreads, C::MINB) k_pipe(const __grid_constan
 
 template <class K> constexpr size_t smem_of() { return PipeSmem<K>::TOTAL; }
 
-template <class... KS>
-__global__ void __launch_bounds__(kThreads, C::MINB) k_chain(const __grid_constant__ ChainParams<Real, (int)sizeof...(KS)> cp)
-{
-    extern __shared__ __align__(128) unsigned char smem[];
-    chain_run<KS...>(cp, smem);
-}
-
 template <class K>
 cudaError_t optin()
 {
@@ -71,34 +64,6 @@ cudaError_t launch(const void *pp, int ntiles, cudaStream_t s)
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, k_pipe<K>, *static_cast<const P *>(pp), ntiles);
-}
-
-constexpr int kTilesPerPlane = C::N / C::W;                     // every chained stage: N / W tiles per x-plane
-int g_chain_ctas = 0;                                           // co-resident CTAs of the chained kernels
-
-template <class... KS>
-cudaError_t chain_optin(int sms)
-{
-    auto *f = k_chain<KS...>;
-    cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ChainSmem<KS...>::TOTAL);
-    if (e != cudaSuccess) return e;
-    int occ = 0;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f, kThreads, ChainSmem<KS...>::TOTAL)) != cudaSuccess) return e;
-    if (occ > C::MINB) occ = C::MINB;
-    if (occ * sms < g_chain_ctas) g_chain_ctas = occ * sms;
-    return cudaSuccess;
-}
-
-template <class... KS>
-cudaError_t chain_launch(ChainParams<Real, (int)sizeof...(KS)> &cp, int planes, const ChainCtl *ctl, cudaStream_t s)
-{
-    chain_plan(cp, planes, kTilesPerPlane, ctl->lag);
-    cp.done = ctl->done;
-    cp.target = ctl->target;
-    int grid = cp.total < g_chain_ctas ? cp.total : g_chain_ctas;
-    if (grid <= 0 || chain_min_distance(kTilesPerPlane, ctl->lag < planes ? ctl->lag : planes) <= grid) return cudaErrorInvalidConfiguration;
-    void *args[] = {&cp};
-    return cudaLaunchCooperativeKernel((void *)k_chain<KS...>, dim3(grid), dim3(kThreads), args, ChainSmem<KS...>::TOTAL, s);
 }
 
 using PsiZKick = PsiK<C, AX_CONTIG, 1, false, true>;
@@ -139,47 +104,7 @@ cudaError_t init()
     OPT(PsiZKick) OPT(PsiZKickX) OPT(C2RExt) OPT(PsiZ) OPT(PsiS) OPT(PsiX) OPT(PsiXRho) OPT(RhoOnly) OPT(HYF) OPT(HZG) OPT(HYI) OPT(C2R)
     OPT(PsiZKickD) OPT(PsiZKickXD) OPT(PsiZD) OPT(PsiSD) OPT(PsiXD) OPT(PsiXRhoD) OPT(HZGD) OPT(C2RD) OPT(C2RExtD) OPT(PsiZM) OPT(PsiSM) OPT(PsiXM)
 #undef OPT
-    g_chain_ctas = g_ctas;
-    if ((e = chain_optin<PsiZKick, PsiS>(sms)) != cudaSuccess) return e;
-    if ((e = chain_optin<PsiZ, PsiS>(sms)) != cudaSuccess) return e;
-    if ((e = chain_optin<HYF, HZG, HYI>(sms)) != cudaSuccess) return e;
     return cudaSuccess;
-}
-
-// lag (in planes) between consecutive stages: large enough that a tile's dependencies were stored before the
-// pipeline wants to request it (NBUF tiles per CTA are in flight), as small as possible beyond that so the
-// planes in transit stay in L2.  0: chaining is pointless or unsafe for this size.
-int chain_lag(int stages, int planes, int requested)
-{
-    const int tiles = planes * kTilesPerPlane * stages;
-    const int grid = tiles < g_chain_ctas ? tiles : g_chain_ctas;
-    if (g_chain_ctas <= 0 || planes < 4) return 0;
-    int safe = grid / kTilesPerPlane + 1;                                   // lag * tpu + 1 > grid
-    int lag = requested;
-    if (lag <= 0) {
-        int inflight = (C::NG + 1) * grid;                                  // measured optimum: about twice the tiles in flight
-        lag = 2 * inflight / (kTilesPerPlane * stages) + 1;
-        if (lag > planes / 2) lag = planes / 2;                             // small grids: keep the stages overlapped
-    }
-    if (lag < safe) lag = safe;
-    if (lag >= planes) return 0;
-    return lag;
-}
-
-cudaError_t psi_zy(const void *pz, const void *py, int kick, const ChainCtl *ctl, cudaStream_t s)
-{
-    ChainParams<Real, 2> cp;
-    cp.p[0] = *static_cast<const P *>(pz);
-    cp.p[1] = *static_cast<const P *>(py);
-    return kick ? chain_launch<PsiZKick, PsiS>(cp, C::N, ctl, s) : chain_launch<PsiZ, PsiS>(cp, C::N, ctl, s);
-}
-cudaError_t h_yzy(const void *py, const void *pz, const ChainCtl *ctl, cudaStream_t s)
-{
-    ChainParams<Real, 3> cp;
-    cp.p[0] = *static_cast<const P *>(py);
-    cp.p[1] = *static_cast<const P *>(pz);
-    cp.p[2] = *static_cast<const P *>(py);
-    return chain_launch<HYF, HZG, HYI>(cp, C::N / 2 + 1, ctl, s);
 }
 
 // diag: 0 plain, 1 accumulate the per-step diagnostics, 2 (psi sweeps without kick only) measure, write nothing
@@ -211,7 +136,7 @@ cudaError_t c2r(const void *pp, int diag, cudaStream_t s)
 }
 
 const SweepTable kTable = {Fact{C::N, C::RA, C::RB, C::RM, C::W, C::NT, C::NG, C::MINB}, WDM_DTYPE, init, psi_z,
-                           psi_strided, psi_x_rho, h_y_fwd, h_z_green, h_y_inv, c2r, chain_lag, psi_zy, h_yzy};
+                           psi_strided, psi_x_rho, h_y_fwd, h_z_green, h_y_inv, c2r};
 
 }  // namespace
 

@@ -651,45 +651,6 @@ def test_large_phase_kick_with_gravity_c64(wdm):
     sim.close()
 
 
-# ---------------------------------------------------------------- L2-chained sweeps: same arithmetic, different schedule
-
-@pytest.mark.parametrize("dtype,N,G", [("c64", 128, 1.0), ("c128", 128, 1.0), ("c64", 256, 1.0), ("c128", 256, 0.0),
-                                       ("c64", 512, 1.0)])
-def test_chained_sweeps_match_separate_sweeps(wdm, dtype, N, G):
-    """wdm_set_chain only changes WHEN a tile runs (stage s + 1 trails stage s by `lag` planes inside one
-    kernel); every tile does the arithmetic of the separate sweep, so psi and Phi agree to a few roundings
-    (the two instantiations may contract multiply-adds differently), for the automatic lag and for the
-    smallest and a large one (the ramps of the position sequence differ).  A tile that read a plane before
-    its producer stored it would be wrong at O(1) in that tile, i.e. >= 1e-3 in these norms."""
-    import torch
-    psi0 = (0.3 * wl.random_field(N, dtype, 11) + 1.0).astype(np.complex64 if dtype == "c64" else np.complex128)
-    dt = (1.0 / N) ** 2 / 6
-
-    def run(mode, lag):
-        sim = wdm.Sim(N, 1.0, 1.0, G / (4 * math.pi), dtype)
-        wdm.wdm_set_chain(sim.h, mode, lag)
-        lags = wdm.wdm_get_chain(sim.h)
-        sim.set_psi(psi0)
-        sim.step(3, dt)
-        out = sim.psi().clone(), sim.potential().clone()
-        torch.cuda.synchronize()
-        sim.close()
-        return out, lags
-
-    (psi_s, phi_s), lags0 = run(0, 0)
-    assert lags0 == (0, 0)
-    used = set()
-    for lag in (0, 1, N // 4):
-        (psi_c, phi_c), lags = run(3, lag)
-        assert lags[0] > 0 and lags[1] > 0, f"chain not enabled at N={N}: {lags}"
-        used.add(lags)
-        eps = 1e-6 if dtype == "c64" else 1e-14
-        e_psi = float((psi_c - psi_s).abs().max() / psi_s.abs().max())
-        e_phi = float((phi_c - phi_s).abs().max() / phi_s.abs().max()) if G > 0 else 0.0
-        assert e_psi <= eps and e_phi <= 10 * eps, f"lags {lags}: psi {e_psi}, Phi {e_phi}"
-    assert len(used) >= 2
-
-
 # ---------------------------------------------------------------- extra kick terms (SURVEY.md 8(f) rank 1)
 
 def _ext_potential(N, L, amp):

@@ -4,7 +4,6 @@ compute-sanitizer (memcheck, racecheck, synccheck; see profiles/r2_sanitizer.md 
   * two-level and three-level tiles, complex64 and complex128, with fewer tiles than CTAs (static assignment only);
   * 128^3: more tiles than the first static round, so the ticket path hands out tiles dynamically;
   * coupled particles (shared-memory atomics of the deposit, the sort, both assignment schemes);
-  * the L2-chained kernels (release / acquire counters between stages of one cooperative launch);
   * the extra kick terms and the external potential (separate instantiations of the z and complex-to-real sweeps).
 
 Each case is also a parity test against the CPU oracle, so a plain `pytest -m gpu` run checks the same code.
@@ -34,7 +33,7 @@ def wdm():
     return w
 
 
-def run_pair(wdm, w, nsteps, chain=0, kick=None, order=2, substeps=1):
+def run_pair(wdm, w, nsteps, kick=None, order=2, substeps=1):
     npart = 0 if w.pos is None else len(w.pos)
     sim = wdm.Sim(w.N, w.L, w.hbar_over_m, w.G, w.dtype, max_particles=npart)
     o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
@@ -46,8 +45,6 @@ def run_pair(wdm, w, nsteps, chain=0, kick=None, order=2, substeps=1):
             x.set_particle_mode(substeps=substeps)
     if kick:
         sim.set_kick_terms(**kick); o.set_kick_terms(**kick)
-    if chain:
-        wdm.wdm_set_chain(sim.h, chain, 0)
     sim.step(nsteps, w.dt); o.step(nsteps, w.dt)
     t = (1e-12 if w.dtype == "c128" else 2e-5)
     assert rel(sim.psi().cpu().numpy(), o.psi()) <= t
@@ -88,11 +85,6 @@ def test_san_16_coupled(wdm, dtype, order):
     run_pair(wdm, wl.small_coupled(16, dtype=dtype), 3, order=order, substeps=2 if order == 3 else 1)
 
 
-@pytest.mark.parametrize("dtype,N", [("c64", 32), ("c128", 32), ("c64", 128)])
-def test_san_chained(wdm, dtype, N):
-    run_pair(wdm, noise(N, dtype), 2, chain=3)
-
-
 def test_san_kick_terms(wdm):
     N = 32
     w = noise(N, "c64")
@@ -106,18 +98,16 @@ def test_san_kick_terms(wdm):
 # compute-sanitizer is closed on the GPU pool this repository is measured on (profiles/r2_sanitizer.md).  Two properties
 # that a race or an out-of-bounds store would break are checked directly instead.
 
-@pytest.mark.parametrize("dtype,N,chain", [("c64", 128, 0), ("c64", 128, 3), ("c128", 64, 0), ("c64", 256, 0)])
-def test_runs_are_bitwise_reproducible(wdm, dtype, N, chain):
-    """Pure SPE steps use no atomics: whichever CTA draws a tile (dynamic tickets, chained stages waiting on counters),
-    the tile's arithmetic is the same, so repeated runs from the same input must agree BIT FOR BIT.  A tile read before
-    its producer finished, or a buffer refilled before its last reader left, shows up as a run-to-run difference."""
+@pytest.mark.parametrize("dtype,N", [("c64", 128), ("c128", 64), ("c64", 256), ("c128", 128)])
+def test_runs_are_bitwise_reproducible(wdm, dtype, N):
+    """Pure SPE steps use no atomics: whichever CTA draws a tile (dynamic tickets), the tile's arithmetic is the same, so
+    repeated runs from the same input must agree BIT FOR BIT.  A buffer refilled before its last reader left, or read
+    before its copy landed, shows up as a run-to-run difference."""
     import torch
     w = noise(N, dtype)
     outs = []
     for rep in range(3):
         sim = wdm.Sim(w.N, w.L, w.hbar_over_m, w.G, w.dtype)
-        if chain:
-            wdm.wdm_set_chain(sim.h, chain, 0)
         sim.set_psi(w.psi)
         sim.step(6, w.dt)
         outs.append((sim.psi().clone(), sim.potential().clone()))
