@@ -176,6 +176,41 @@ def run_reference(args, rank, world):
     }))
 
 
+def coupled_record(wdm, torch, K, W):
+    """cfg5: ONE wdm_step(K, dt) between CUDA events after W warm-up steps; cell- and particle-updates/s, per-kernel means."""
+    w = wl.config5()
+    N, npart = w.N, len(w.pos)
+    sim = wdm.Sim(N, w.L, w.hbar_over_m, w.G, w.dtype, max_particles=npart)
+    sim.set_psi(torch.from_numpy(w.psi).pin_memory())
+    sim.set_particles(w.pos, w.vel, w.mass)
+    sim.step(0, 0.0)
+    dt = wl.cfl_dt(w, float(sim.potential().abs().max()))
+    stream = torch.cuda.current_stream()
+    sim.step(W, dt)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    sim.step(K, dt)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    wdm.wdm_set_profiling(sim.h, True)
+    kp = min(K, 64)
+    sim.step(kp, dt)
+    stats = wdm.wdm_kernel_stats(sim.h)
+    wdm.wdm_set_profiling(sim.h, False)
+    sim.close()
+    peak, _ = peaks()
+    rec = {"workload": w.name, "N": N, "particles": npart, "steps": K, "ms_per_step": ms / K,
+           "cell_updates_per_s": N ** 3 * K / (ms * 1e-3), "particle_updates_per_s": npart * K / (ms * 1e-3),
+           "alg_bytes_per_step": 12 * 8 * N ** 3 + 60 * npart,
+           "frac_of_hbm_peak": (12 * 8 * N ** 3 + 60 * npart) / (ms / K * 1e-3) / 1e9 / peak,
+           "note": "12c per cell (rho_p cleared and read) + 60 B per particle, SURVEY 8(d); 256^3 sits near the 126 MB L2",
+           "kernels_avg_ms": {k: t / c for k, (c, t) in stats.items() if c},
+           "kernel_launches_per_step": {k: c / kp for k, (c, t) in stats.items() if c}}
+    return rec
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -321,6 +356,12 @@ def main():
             out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": thr, "kind": "oracle",
                                    "sample": f"float64 CPU oracle, soliton+halo at {n_ref}^3, {CPU_STEPS} timed KDK steps ({el:.1f} s)"}
     sim.close()
+    # ---- the coupled run of BASELINE.json's metric ("+ particle updates/s"): config 5 (256^3 complex64 soliton + halo,
+    # 2^20 disc particles), same timing rules, as a sub-record of the default line (rank 0, N = 1)
+    if rank == 0 and world == 1 and not args.no_extras and args.workload == "t512":
+        del sim
+        torch.cuda.empty_cache()
+        out["coupled"] = coupled_record(wdm, torch, K, W)
     if rank == 0:
         print(json.dumps(out))
     if dist is not None:
