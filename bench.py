@@ -176,6 +176,55 @@ def run_reference(args, rank, world):
     }))
 
 
+def run_dist(args, rank, world, local, dist, torch):
+    """One box sharded over the ranks.  NOT the north_star path: a separate line, scaling "strong"."""
+    import paper_2606_25026_b200.dist as wd
+    K, W = args.steps, max(3, args.warmup)
+    w = make_workload(args.workload)
+    N, xl = w.N, w.N // world
+    sim = wd.DistSim(N, w.L, w.hbar_over_m, w.G, w.dtype, rank, world)
+    slab = torch.from_numpy(w.psi[rank * xl:(rank + 1) * xl])
+    dt = w.dt if w.dt is not None else (w.L / N) ** 2 / 6.0
+
+    def run(prog):
+        if world > 1:
+            sim.run(prog)
+        else:
+            wd.run_emulated([sim], [prog])
+
+    run(sim.prog_set_psi(slab))
+    run(sim.prog_step(W, dt))
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+        torch.cuda.synchronize()
+    stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        e0.record(stream)
+        run(sim.prog_step(K, dt))
+        e1.record(stream)
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
+    csize = 8 if w.dtype == "c64" else 16
+    xbytes = (2 * xl * xl * N + 2 * xl * (-(-(N // 2 + 1) // world)) * N) * csize * (world - 1)     # sent per rank per step
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": N ** 3 * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f32" if w.dtype == "c64" else "f64", "data": "synthetic",
+            "config": {"workload": w.name, "N": N, "mode": "slab-decomposed (wdm_dist.h), pure SPE",
+                       "parallelism": f"x-slabs over {world} rank(s), 4 all-to-all exchanges per step",
+                       "exchange_bytes_sent_per_rank_per_step": xbytes,
+                       "note": "with one rank the exchanges are local copies: this is the cost of the decomposition "
+                               "machinery (pack / unpack passes), not a scaling measurement"},
+            "gpu_launches": sim.launched_phases, "clocks": clk.summary()}))
+    sim.close()
+
+
 def coupled_record(wdm, torch, K, W):
     """cfg5: ONE wdm_step(K, dt) between CUDA events after W warm-up steps; cell- and particle-updates/s, per-kernel means."""
     w = wl.config5()
@@ -220,6 +269,9 @@ def main():
     ap.add_argument("--impl", default="wdm")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e / per-kernel / particle legs (used under ncu)")
+    ap.add_argument("--dist", action="store_true",
+                    help="slab-decomposed step (include/wdm_dist.h): ONE box sharded over the ranks, NCCL all-to-all "
+                         "between phases (strong scaling); with one rank the exchange is a local copy")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -237,6 +289,11 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if args.dist:
+        run_dist(args, rank, world, local, dist, torch)
+        if dist is not None:
+            dist.destroy_process_group()
+        return
 
     K, W = args.steps, max(3, args.warmup)
     w = make_workload(args.workload)

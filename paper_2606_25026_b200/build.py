@@ -28,7 +28,8 @@ def _sizes():
 
 
 def _newest_source() -> float:
-    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "wdm.h")]
+    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "wdm.h"),
+                                                              os.path.join(HERE, "..", "include", "wdm_dist.h")]
     return max(os.path.getmtime(f) for f in files)
 
 
@@ -36,7 +37,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     newest = _newest_source()
     jobs = [("wdm.o", ["-c", os.path.join(CSRC, "wdm.cu")]),
-            ("wdm_particles.o", ["-c", os.path.join(CSRC, "wdm_particles.cu")])]
+            ("wdm_particles.o", ["-c", os.path.join(CSRC, "wdm_particles.cu")]),
+            ("wdm_dist.o", ["-c", os.path.join(CSRC, "wdm_dist.cu")])]
     for dtype, n in _sizes():
         jobs.append((f"sweeps_{dtype}_{n}.o", [f"-DWDM_DTYPE={dtype}", f"-DWDM_N={n}", "-c", os.path.join(CSRC, "wdm_sweeps.cu")]))
 

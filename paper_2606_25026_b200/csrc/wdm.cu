@@ -351,33 +351,12 @@ struct Timed {
 
 // ---------------------------------------------------------------- TMA descriptors
 
-// Box of W complex elements along z by `rows` points along axis (1 = y, 2 = x) of a [nx][N][N] complex array.
-// Encoded in units of one real (float / double), no swizzle, no interleave: the box lands in shared memory as
-// dense [row][W] -- the strided tile layout.
+// (the encoder itself is in wdm_internal.hpp: encode_tmap)
 static int make_tmap(wdm_ctx *c, CUtensorMap *out, void *base, int nx, int axis, int rows)
 {
-    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
-                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-    static encode_fn encode = nullptr;
-    if (!encode) {
-        void *fn = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q);
-        if (e != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn)
-            return fail(c, WDM_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
-        encode = (encode_fn)fn;
-    }
-    const size_t r = rsize(c->dtype);
-    const cuuint64_t N = (cuuint64_t)c->N;
-    cuuint64_t dims[3] = {2 * N, N, (cuuint64_t)nx};
-    cuuint64_t strides[2] = {2 * N * r, 2 * N * N * r};
-    cuuint32_t box[3] = {(cuuint32_t)(2 * c->tab->fact.W), axis == 1 ? (cuuint32_t)rows : 1u, axis == 2 ? (cuuint32_t)rows : 1u};
-    cuuint32_t estr[3] = {1, 1, 1};
-    CUresult res = encode(out, c->dtype == WDM_C64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims,
-                          strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (res != CUDA_SUCCESS) return fail(c, WDM_ECUDA, "cuTensorMapEncodeTiled failed (%d) for N = %d axis %d rows %d", (int)res, c->N, axis, rows);
+    const int rc = encode_tmap(c->dtype, c->N, c->tab->fact.W, base, c->N, nx, axis, rows, out);
+    if (rc == -1) return fail(c, WDM_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
+    if (rc != 0) return fail(c, WDM_ECUDA, "cuTensorMapEncodeTiled failed (%d) for N = %d axis %d rows %d", rc, c->N, axis, rows);
     return WDM_OK;
 }
 

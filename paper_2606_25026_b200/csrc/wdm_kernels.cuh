@@ -147,6 +147,7 @@ struct SweepParams {
     const T *ksq_pos;          // Green: k^2 of the frequency held at a position
     const T *ksq_nat;          // Green: k^2 of frequency index k (natural)
     T green;                   // Green: -4 pi G / N^3
+    int kx0;                   // Green: global kx index of the first plane of the array (slab-decomposed runs; else 0)
     // TMA descriptors of the array a strided sweep walks: boxes of (W elements along z) x (<= 256 rows along the
     // sweep axis); tmap2 is the one-row box that fetches row N/2 of the half spectrum in the complex-to-real sweep
     CUtensorMap tmap, tmap2;

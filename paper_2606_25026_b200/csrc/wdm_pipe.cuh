@@ -257,8 +257,9 @@ __device__ __forceinline__ void tile_load(cx<typename C::T> *S, const cx<typenam
             else tma_load_3d(S + (size_t)k * RB * W, tm, c0, outer, k * RB, bar);
         }
         if constexpr (ROWS - FULL * RB > 0) {
-            static_assert(ROWS - FULL * RB == 1 && AX == AX_X, "only the half spectrum has an odd row");
-            tma_load_3d(S + (size_t)FULL * RB * W, tm1, c0, outer, FULL * RB, bar);
+            static_assert(ROWS - FULL * RB == 1, "only the half spectrum has an odd row");
+            if (AX == AX_Y) tma_load_3d(S + (size_t)FULL * RB * W, tm1, c0, FULL * RB, outer, bar);
+            else tma_load_3d(S + (size_t)FULL * RB * W, tm1, c0, outer, FULL * RB, bar);
         }
     } else {
         const TL tile(bid);
@@ -423,7 +424,10 @@ struct PsiK {
     static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA;
     static constexpr int ITER = (mA * W) / NTG;
     static_assert((mA * W) % NTG == 0, "whole number of level-A butterflies per thread");
-    static_assert(!RHO || AX == AX_X, "the density sweep runs along x");
+    // The density sweep runs along x: the outermost index of the single-GPU layout (AX_X), or the MIDDLE index of the
+    // transposed slab psi^T[y_loc][x][z] of a slab-decomposed run (AX_Y; the half spectrum is then H^T[y_loc][kx][z],
+    // (N/2 + 1) N elements per outer index -- see wdm_dist.cu)
+    static_assert(!RHO || ax_strided(AX), "the density sweep runs along a strided axis");
     static constexpr size_t TILE_BYTES = align128(L::ELEMS * sizeof(cx<T>));
     static constexpr int AUX = DRIFT ? AUX_PHASE : AUX_NONE;
     // Potential values prefetched across tiles (into registers, during the previous tile's last stage): those of
@@ -694,12 +698,14 @@ struct PsiK {
             }
             group_sync(grp, NTG);
             // Hermitian split of Z = FFT(a + i b):  A_k = (Z_k + conj Z_{N-k})/2,  B_k = (Z_k - conj Z_{N-k})/(2i)
+            // row k of the half spectrum, line 2l of this tile
+            const long long hbase = AX == AX_X ? tile.base : (long long)(t / TL::INNER) * ((long long)(N / 2 + 1) * N) + (long long)(t % TL::INNER) * W;
             auto emit = [&](int k, int e, int en, int l) {
                 cx<T> zk = Sp[e], zn = Sp[en];
                 const T h = (T)0.5;
                 cx<T> A = mk<T>((zk.x + zn.x) * h, (zk.y - zn.y) * h);
                 cx<T> B = mk<T>((zk.y + zn.y) * h, (zn.x - zk.x) * h);
-                st2(p.H + tile.at(k, 2 * l), A, B);
+                st2(p.H + hbase + (long long)k * TL::RSTRIDE + 2 * l, A, B);
             };
             half_spectrum_items<C, WP, Packed<C>>(gt, emit);
             if (gt < WP) {
@@ -771,6 +777,7 @@ struct HK {
             for (int b = gt; b < (N / RM) * W; b += NTG) {
                 int l = b % W, g = b / W;
                 int pen = t * W + l, kx = pen / N, ypos = pen - kx * N;
+                kx += p.kx0;                                   // first kx-plane of this rank's slab (0 on a single GPU)
                 T kxy = ldg(p.ksq_nat + kx) + tb.ksq_pos[ypos];
                 bool zero_line = (kx == 0 && ypos == 0);
                 T wsum = (T)0;
@@ -823,13 +830,15 @@ struct HK {
 // complex-to-real inverse along x: H[kx <= N/2][y][z] -> Phi[x][y][z]; lines (2l', 2l'+1) share one FFT.
 // Buffer = [packed tile: N rows x W/2 complex][raw tile: N/2+1 rows x W complex, filled by the async copies].
 // EXT: add the static external potential on the way out (SweepParams::phi_ext != nullptr), a separate instantiation
-template <class C_, bool EXT = false, int DG_ = 0>
+// AXR: the axis of the transform -- AX_X on a single GPU; AX_Y for the transposed slab H^T[y_loc][kx][z] ->
+// Phi^T[y_loc][x][z] of a slab-decomposed run.
+template <class C_, bool EXT = false, int DG_ = 0, int AXR = AX_X>
 struct C2RK {
     static constexpr int DG = DG_;                              // 1: max |Phi_total| from the outgoing registers
     static constexpr bool DIAG_ZEROES = false;
     using C = C_;
     using T = typename C::T;
-    using TL = Tile<C, AX_X>;
+    using TL = Tile<C, AXR>;
     static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA;
     static constexpr int WP = W / 2, RSP = W / 2;
     using PK = Packed<C, true>;
@@ -842,7 +851,7 @@ struct C2RK {
     using Pers = PairTw<C, PAIR>;
     static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar, int lane)
     {
-        tile_load<C, AX_X, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf + PACKED_BYTES), p.H, &p.tmap, &p.tmap2, t, bar, lane);
+        tile_load<C, AXR, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf + PACKED_BYTES), p.H, &p.tmap, &p.tmap2, t, bar, lane);
     }
     static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
     template <class HOOK>

@@ -135,8 +135,31 @@ cudaError_t c2r(const void *pp, int diag, cudaStream_t s)
     return ext ? launch<C2RExt>(pp, kTilesGrid, s) : launch<C2R>(pp, kTilesGrid, s);
 }
 
+// ---- slab-decomposed runs (wdm_dist.cu): the same sweeps on slab-shaped arrays, tile count given by the caller; the
+// distributed axis x is the middle index of the transposed slabs, so its sweeps are AX_Y instantiations
+using PsiTRho = PsiK<C, AX_Y, 0, true, true>;
+using RhoOnlyT = PsiK<C, AX_Y, 0, true, false>;
+using C2RT = C2RK<C, false, 0, AX_Y>;
+cudaError_t dist_init()
+{
+    cudaError_t e;
+    if ((e = optin<PsiTRho>()) != cudaSuccess) return e;
+    if ((e = optin<RhoOnlyT>()) != cudaSuccess) return e;
+    return optin<C2RT>();
+}
+cudaError_t dist_psi_z(const void *pp, int kick, int ntiles, cudaStream_t s) { return kick ? launch<PsiZKick>(pp, ntiles, s) : launch<PsiZ>(pp, ntiles, s); }
+cudaError_t dist_psi_y(const void *pp, int ntiles, cudaStream_t s) { return launch<PsiS>(pp, ntiles, s); }
+cudaError_t dist_psi_x_rho(const void *pp, int drift, int ntiles, cudaStream_t s)
+{
+    return drift ? launch<PsiTRho>(pp, ntiles, s) : launch<RhoOnlyT>(pp, ntiles, s);
+}
+cudaError_t dist_h_y(const void *pp, int inverse, int ntiles, cudaStream_t s) { return inverse ? launch<HYI>(pp, ntiles, s) : launch<HYF>(pp, ntiles, s); }
+cudaError_t dist_h_z_green(const void *pp, int ntiles, cudaStream_t s) { return launch<HZG>(pp, ntiles, s); }
+cudaError_t dist_c2r(const void *pp, int ntiles, cudaStream_t s) { return launch<C2RT>(pp, ntiles, s); }
+
 const SweepTable kTable = {Fact{C::N, C::RA, C::RB, C::RM, C::W, C::NT, C::NG, C::MINB}, WDM_DTYPE, init, psi_z,
-                           psi_strided, psi_x_rho, h_y_fwd, h_z_green, h_y_inv, c2r};
+                           psi_strided, psi_x_rho, h_y_fwd, h_z_green, h_y_inv, c2r,
+                           dist_init, dist_psi_z, dist_psi_y, dist_psi_x_rho, dist_h_y, dist_h_z_green, dist_c2r};
 
 }  // namespace
 
