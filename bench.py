@@ -187,7 +187,7 @@ def run_dist(args, rank, world, local, dist, torch):
     dt = w.dt if w.dt is not None else (w.L / N) ** 2 / 6.0
 
     def run(prog):
-        if world > 1:
+        if dist is not None:
             sim.run(prog)
         else:
             wd.run_emulated([sim], [prog])
@@ -218,6 +218,7 @@ def run_dist(args, rank, world, local, dist, torch):
             "dtype": "f32" if w.dtype == "c64" else "f64", "data": "synthetic",
             "config": {"workload": w.name, "N": N, "mode": "slab-decomposed (wdm_dist.h), pure SPE",
                        "parallelism": f"x-slabs over {world} rank(s), 4 all-to-all exchanges per step",
+                       "exchange": "NCCL all_to_all_single" if dist is not None else "local copy (single process)",
                        "exchange_bytes_sent_per_rank_per_step": xbytes,
                        "note": "with one rank the exchanges are local copies: this is the cost of the decomposition "
                                "machinery (pack / unpack passes), not a scaling measurement"},
@@ -286,7 +287,7 @@ def main():
 
     torch.cuda.set_device(local)
     dist = None
-    if world > 1:
+    if world > 1 or (args.dist and "RANK" in os.environ):      # (--dist under torchrun: NCCL also with a single rank)
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if args.dist:
