@@ -234,6 +234,7 @@ struct wdm_ctx {
     // half kick of the next wdm_step, or are applied when the state is read or a parameter changes
     double pend_psi = 0, pend_part = 0;
     ParticleState part;
+    void *part_pool = nullptr;      // owned contexts: the current particle pool (replaced by a larger one on demand)
     long long max_particles = -1;   // -1: unbounded (cudaMalloc on demand)
     // instrumentation
     long long launches = 0;
@@ -801,8 +802,16 @@ static int set_particles(wdm_ctx *c, long long n, const void *pos, const void *v
         void *rho_p = c->part.rho_p, *pm = nullptr;
         int rc;
         if (!rho_p && (rc = ctx_alloc(c, &rho_p, c->n * rs))) return rc;
-        if ((rc = ctx_alloc(c, &pm, particle_bytes(c->N, c->dtype, n)))) return rc;   // older pool stays until destroy
+        if ((rc = ctx_alloc(c, &pm, particle_bytes(c->N, c->dtype, n)))) return rc;
         particle_bind(c->part, c->N, c->dtype, n, rho_p, pm);
+        if (c->part_pool) {
+            // the smaller pool is not needed any more: release it once the stream has passed everything that used it
+            CU(c, cudaStreamSynchronize(c->stream));
+            for (size_t i = 0; i < c->owned.size(); ++i)
+                if (c->owned[i] == c->part_pool) { c->owned.erase(c->owned.begin() + i); break; }
+            cudaFree(c->part_pool);
+        }
+        c->part_pool = pm;
     }
     c->launches += 3;
     c->deposit_mass = 0;

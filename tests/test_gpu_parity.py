@@ -282,6 +282,33 @@ def test_deterministic_deposit_is_bit_stable_and_matches_oracle(wdm, order):
     sim.close()
 
 
+def test_particle_pool_grows_in_an_owned_context(wdm):
+    """wdm_create (library-owned memory): a second, larger particle set replaces the pool (the smaller one is released);
+    results match the oracle before and after."""
+    import torch
+    w = wl.small_coupled(16, dtype="c64", n_particles=100)
+    w2 = wl.small_coupled(16, dtype="c64", n_particles=3000, seed=78)
+    h = wdm.wdm_create(w.N, w.L, w.hbar_over_m, w.G, wdm.WDM_C64)
+    o = oracle.Oracle(w.N, w.L, w.hbar_over_m, w.G)
+    psi = torch.as_tensor(w.psi).cuda()
+    wdm.wdm_set_psi(h, psi); o.set_psi(w.psi)
+    for ww in (w, w2, w):                                   # grow, then shrink back (the larger pool is kept)
+        n = len(ww.pos)
+        wdm.wdm_set_particles(h, n, torch.as_tensor(ww.pos).cuda(), torch.as_tensor(ww.vel).cuda(), None, float(ww.mass))
+        o.set_particles(ww.pos, ww.vel, ww.mass)
+        wdm.wdm_step(h, 3, w.dt); o.step(3, w.dt)
+        pos = torch.empty((n, 3), dtype=torch.float32, device="cuda"); vel = torch.empty_like(pos)
+        wdm.wdm_get_particles(h, pos, vel)
+        out = torch.empty_like(psi); wdm.wdm_get_psi(h, out)
+        torch.cuda.synchronize()
+        po, _ = o.particles()
+        d = pos.cpu().numpy().astype(np.float64) - po
+        d -= w.L * np.round(d / w.L)
+        assert np.abs(d).max() <= POS_TOL * w.L
+        assert rel(out.cpu().numpy(), o.psi()) <= tol("c64", 9)
+    wdm.wdm_destroy(h)
+
+
 def test_resort_keeps_results(wdm):
     """More pushes than the re-sort interval: sorting must not change what is computed."""
     w = wl.small_coupled(16, dtype="c128", n_particles=300)
