@@ -25,8 +25,14 @@
  * Pins (tests/test_oracle_pins.py): P1 norm, P2 free Gaussian closed form, P3 plane wave,
  * P4 single-mode Poisson, P5 direct DFT, P6 O(dt^2) energy error, P7 time reversal, P8 CIC
  * momentum / mass / zero self force, P9 gather in a known field, P10 numpy.fft cross-check.
+ * P11 self-interaction plane wave, P12 external potential (harmonic ground state, particles feel it), P13 absorbing-layer
+ * values at face / edge / corner, P14 diagnostics closed forms (plane wave, real Gaussian, cosine density, Eq. 26),
+ * P15 sub-stepped leapfrog in a harmonic potential / static particles.
  * P16 triangular-shaped cloud: hand-computed weights, mass / centre / second moment, exact gradient of a
  * quadratic-free (single-mode) field, momentum conservation.
+ * P17 spectral kinetic energy (plane-wave closed forms incl. a Nyquist component, T -> K + Q at second order in dx, the
+ * moving-Gaussian closed form), E = T + W against numpy.fft and its O(dt^2) drift, the per-step record against a
+ * hand-undone closing kick; the density getter with an absorbing layer (reading G22).
  * The coupled psi+particle trajectory over many steps has no closed form: "parity unpinned"
  * beyond P1, P7, P8 and second-order self-convergence.
  *
