@@ -513,7 +513,8 @@ static int particles_deposit(wdm_ctx *c)
         CU(c, particle_deposit_fixed(c->part, c->N, c->L, c->dtype, c->deposit_acc, c->deposit_mass, c->stream));
         return WDM_OK;
     }
-    { Timed t(c, S_PART_CLEAR); CU(c, particle_mesh_clear(c->part, c->N, c->dtype, c->stream)); }
+    if (c->part.mesh_cleared) c->part.mesh_cleared = false;          // the push kernel before this cleared the flagged columns
+    else { Timed t(c, S_PART_CLEAR); CU(c, particle_mesh_clear(c->part, c->N, c->dtype, c->stream)); }
     Timed t(c, S_PART_DEPOSIT);
     CU(c, particle_deposit(c->part, c->N, c->L, c->dtype, c->stream));
     return WDM_OK;
@@ -580,7 +581,7 @@ static int flush_pending(wdm_ctx *c, bool psi, bool part)
     }
     if (part && c->pend_part != 0.0) {
         Timed t(c, S_PART_PUSH);
-        CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, 0.5 * c->pend_part / c->nsub, 0.0, 1, c->stream));
+        CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, 0.5 * c->pend_part / c->nsub, 0.0, 1, false, c->stream));
         c->pend_part = 0.0;
     }
     return WDM_OK;
@@ -613,7 +614,7 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
         const double hd_p = s == 0 ? 0.5 * c->pend_part : 0.5 * dt;
         if (c->part.n > 0 && !c->pstatic) {
             // v += a(Phi^n, x^n) kdt/nsub ; nsub x { x += v dt/nsub ; wrap ; [kick] } ; then deposit x^{n+1}  (G14-G16, G29)
-            { Timed t(c, S_PART_PUSH); CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, have_phi ? (hd_p + ha) / c->nsub : 0.0, dt, c->nsub, c->stream)); }
+            { Timed t(c, S_PART_PUSH); CU(c, particle_push(c->part, c->N, c->L, c->dtype, c->phi, have_phi ? (hd_p + ha) / c->nsub : 0.0, dt, c->nsub, grav && !c->deposit_fixed, c->stream)); }
             if (particle_sort_due(c->part)) { Timed t(c, S_PART_SORT); c->launches += 2; CU(c, particle_resort(c->part, c->N, c->L, c->dtype, c->stream)); }
             if (grav) { rc = particles_deposit<T>(c); if (rc) return rc; }
         }

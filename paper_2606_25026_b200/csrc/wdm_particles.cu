@@ -266,8 +266,17 @@ __device__ __forceinline__ void gather_grad(const T *__restrict__ phi, const T (
 // v += a(x) kick_dt ; then nsub drifts of drift_dt / nsub, wrapped, with a full kick of that size (gathered at the
 // new position, in the same potential) between two drifts (several N-body sub-steps per SPE step)
 template <typename T, int ORDER>
-__global__ void k_push(T *pos, T *vel, const T *__restrict__ phi, long long n, int N, T L, T kick_dt, T drift_dt, int nsub)
+__global__ void k_push(T *pos, T *vel, const T *__restrict__ phi, long long n, int N, T L, T kick_dt, T drift_dt, int nsub,
+                       T *mesh, unsigned char *flag, int nflag, int fb)
 {
+    // Clear duty (mesh != nullptr): the particle mesh must be zero before the deposit that follows this kernel, and
+    // nothing here reads it -- CTA b < nflag zeroes flagged column b (see k_mesh_clear) on its way, which saves a launch.
+    if (mesh && (int)blockIdx.x < nflag && flag[blockIdx.x]) {
+        const int b = blockIdx.x, nfb = N / fb, y = b / nfb, z0 = (b - y * nfb) * fb;
+        for (int i = threadIdx.x; i < N * fb; i += blockDim.x) mesh[((size_t)(i / fb) * N + y) * N + z0 + i % fb] = (T)0;
+        __syncthreads();
+        if (threadIdx.x == 0) flag[b] = 0;
+    }
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= n) return;
     T x[3] = {pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
@@ -547,16 +556,22 @@ cudaError_t particle_set(ParticleState &ps, int N, double L, int dtype, long lon
 }
 
 cudaError_t particle_push(ParticleState &ps, int N, double L, int dtype, const void *phi, double kick_dt, double drift_dt,
-                          int nsub, cudaStream_t s)
+                          int nsub, bool clear_mesh, cudaStream_t s)
 {
     if (ps.n == 0) return cudaSuccess;
     if (nsub < 1) nsub = 1;
-    const unsigned g = blocks(ps.n, 128);
-    if (dtype == 0 && ps.order == 2) k_push<float, 2><<<g, 128, 0, s>>>((float *)ps.pos, (float *)ps.vel, (const float *)phi, ps.n, N, (float)L, (float)kick_dt, (float)drift_dt, nsub);
-    else if (dtype == 0) k_push<float, 3><<<g, 128, 0, s>>>((float *)ps.pos, (float *)ps.vel, (const float *)phi, ps.n, N, (float)L, (float)kick_dt, (float)drift_dt, nsub);
-    else if (ps.order == 2) k_push<double, 2><<<g, 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt, nsub);
-    else k_push<double, 3><<<g, 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt, nsub);
+    const int fb = mesh_flag_block(N), nflag = N * (N / fb);
+    unsigned g = blocks(ps.n, 128);
+    // the sparse clear rides along only when the mesh is known to be clean outside the flagged columns
+    const bool clr = clear_mesh && ps.mesh_clean && ps.rho_p != nullptr;
+    if (clr && g < (unsigned)nflag) g = (unsigned)nflag;
+    void *mesh = clr ? ps.rho_p : nullptr;
+    if (dtype == 0 && ps.order == 2) k_push<float, 2><<<g, 128, 0, s>>>((float *)ps.pos, (float *)ps.vel, (const float *)phi, ps.n, N, (float)L, (float)kick_dt, (float)drift_dt, nsub, (float *)mesh, ps.flag, nflag, fb);
+    else if (dtype == 0) k_push<float, 3><<<g, 128, 0, s>>>((float *)ps.pos, (float *)ps.vel, (const float *)phi, ps.n, N, (float)L, (float)kick_dt, (float)drift_dt, nsub, (float *)mesh, ps.flag, nflag, fb);
+    else if (ps.order == 2) k_push<double, 2><<<g, 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt, nsub, (double *)mesh, ps.flag, nflag, fb);
+    else k_push<double, 3><<<g, 128, 0, s>>>((double *)ps.pos, (double *)ps.vel, (const double *)phi, ps.n, N, L, kick_dt, drift_dt, nsub, (double *)mesh, ps.flag, nflag, fb);
     if (drift_dt != 0.0) ++ps.steps_since_sort;
+    ps.mesh_cleared = clr;
     return cudaGetLastError();
 }
 
@@ -610,6 +625,7 @@ cudaError_t particle_deposit_fixed(ParticleState &ps, int N, double L, int dtype
 cudaError_t particle_mesh_clear(ParticleState &ps, int N, int dtype, cudaStream_t s)
 {
     const int fb = mesh_flag_block(N), nflag = N * (N / fb);
+    if (ps.mesh_cleared) { ps.mesh_cleared = false; return cudaSuccess; }      // the preceding push did it
     if (!ps.mesh_clean) {
         // first use (or a mesh of unknown content): everything, once
         cudaError_t e = cudaMemsetAsync(ps.rho_p, 0, (size_t)N * N * N * (dtype == 0 ? 4 : 8), s);

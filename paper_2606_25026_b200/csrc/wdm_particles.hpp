@@ -21,6 +21,7 @@ struct ParticleState {
     // and the density sweep reads rho_p only for flagged tiles.
     unsigned char *flag = nullptr;
     bool mesh_clean = false;                 // false: content unknown, the next clear zeroes the whole mesh
+    bool mesh_cleared = false;               // the last push also cleared the flagged columns: the next clear is a no-op
     bool has_mass = false;
     double mass_scalar = 0.0;
     int steps_since_sort = 0;
@@ -33,8 +34,9 @@ cudaError_t particle_set(ParticleState &ps, int N, double L, int dtype, long lon
                          const void *mass, double mass_scalar, bool from_host, cudaStream_t s);
 // v += a(phi, x) * kick_dt ; then nsub drifts of drift_dt / nsub (wrapped into [-L/2, L/2)) with a kick of that
 // size, gathered at the new position, between two drifts
+// clear_mesh: also zero the flagged columns of rho_p (the caller deposits next; see particle_mesh_clear)
 cudaError_t particle_push(ParticleState &ps, int N, double L, int dtype, const void *phi, double kick_dt,
-                          double drift_dt, int nsub, cudaStream_t s);
+                          double drift_dt, int nsub, bool clear_mesh, cudaStream_t s);
 // the tile order is kResortInterval drifts old: re-sort (counting sort by mesh tile) before the next deposit
 bool particle_sort_due(const ParticleState &ps);
 cudaError_t particle_resort(ParticleState &ps, int N, double L, int dtype, cudaStream_t s);

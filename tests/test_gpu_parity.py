@@ -804,7 +804,7 @@ def test_step_diagnostics_fused_in_the_sweeps(wdm, dtype, N, case):
     n0 = wdm.wdm_launch_count(sim.h)
     sim.step(nsteps, dt); o.step(nsteps, dt)
     per_step = 7 if w.G > 0 else 3
-    extra = 0 if w.pos is None else 3 * nsteps           # push, clear, deposit
+    extra = 0 if w.pos is None else 2 * nsteps           # push (which also clears the flagged mesh columns), deposit
     assert wdm.wdm_launch_count(sim.h) - n0 == per_step * nsteps + extra
     a, b = sim.step_diagnostics(), o.step_diagnostics()
     t = 2 * max(tol(dtype, nsteps + 1), 1e-11)
