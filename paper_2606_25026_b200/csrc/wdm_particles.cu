@@ -10,6 +10,7 @@
 // CTA's shared-memory box.
 #include <cmath>
 #include <cstdint>
+#include <type_traits>
 
 #include "wdm_particles.hpp"
 
@@ -323,12 +324,36 @@ __global__ void __launch_bounds__(256) k_deposit(const T *__restrict__ pos, cons
     // flag[y * (N / FB) + z / FB] = 1 for every block of FB z-cells of a y-row that receives mass (see mesh_flag_block)
     const int fb = mesh_flag_block(N), nfb = N / fb;
     constexpr int NW = ORDER * ORDER * ORDER;
-    __shared__ T box[BOX * BOX * BOX];
+    // Single precision: the box holds 32-bit FIXED-POINT sums.  Shared-memory atomics are native only for 32-bit integers
+    // (ATOMS.ADD); a float atomicAdd compiles to a compare-and-swap spin loop (ATOMS.CAST.SPIN), which retries whenever
+    // the leaders of several warps hit the same node of a dense cell.  The scale maps the largest sum the chunk can
+    // produce -- all its particles on one node -- onto 2^31; one unit is 5e-7 of a single particle's m / dx^3, below the
+    // float rounding of the sums it replaces.  Double precision keeps the (compare-and-swap) double sums.
+    constexpr bool FIXED = sizeof(T) == 4;
+    using BoxT = typename std::conditional<FIXED, int, T>::type;
+    __shared__ BoxT box[BOX * BOX * BOX];
     __shared__ int org[3];
+    __shared__ T smax[8];
     const long long start = (long long)blockIdx.x * CHUNK;
     const long long end = start + CHUNK < n ? start + CHUNK : n;
     const T inv_dx = (T)N / L, inv_vol = inv_dx * inv_dx * inv_dx, half_L = (T)0.5 * L;
-    for (int j = threadIdx.x; j < BOX * BOX * BOX; j += blockDim.x) box[j] = (T)0;
+    for (int j = threadIdx.x; j < BOX * BOX * BOX; j += blockDim.x) box[j] = (BoxT)0;
+    T scale = (T)1, inv_scale = (T)1;
+    if constexpr (FIXED) {
+        T mmax = fabs(mass_scalar);
+        if (mass) {                                            // largest |mass| of the chunk
+            mmax = (T)0;
+            for (long long i = start + threadIdx.x; i < end; i += blockDim.x) mmax = fmax(mmax, fabs(mass[i]));
+            for (int d = 16; d; d >>= 1) mmax = fmax(mmax, __shfl_down_sync(0xffffffffu, mmax, d));
+            if ((threadIdx.x & 31) == 0) smax[threadIdx.x >> 5] = mmax;
+            __syncthreads();
+            mmax = smax[0];
+            for (int w = 1; w < (int)(blockDim.x >> 5); ++w) mmax = fmax(mmax, smax[w]);
+        }
+        const T bound = (T)CHUNK * mmax * inv_vol;
+        scale = bound > (T)0 ? (T)2147480000.0 / bound : (T)0;
+        inv_scale = bound > (T)0 ? bound / (T)2147480000.0 : (T)0;
+    }
     if (threadIdx.x == 0) {
         T x[3] = {pos[3 * start], pos[3 * start + 1], pos[3 * start + 2]};
         Cic<T> c = cic_of<T>(x, half_L, inv_dx, N);
@@ -382,8 +407,10 @@ __global__ void __launch_bounds__(256) k_deposit(const T *__restrict__ pos, cons
 #pragma unroll
             for (int q = 0; q < NW; ++q) {
                 int bx = q / (ORDER * ORDER), by = (q / ORDER) % ORDER, bz = q % ORDER;
-                if (inside) atomicAdd(&box[((rx + bx) * BOX + ry + by) * BOX + rz + bz], w[q]);
-                else {
+                if (inside) {
+                    if constexpr (FIXED) atomicAdd(&box[((rx + bx) * BOX + ry + by) * BOX + rz + bz], __float2int_rn(w[q] * scale));
+                    else atomicAdd(&box[((rx + bx) * BOX + ry + by) * BOX + rz + bz], w[q]);
+                } else {
                     const int gy = (c.base[1] + by) & M, gz = (c.base[2] + bz) & M;
                     atomicAdd(rho + ((size_t)((c.base[0] + bx) & M) * N + gy) * N + gz, w[q]);
                     flag[gy * nfb + gz / fb] = 1;
@@ -393,8 +420,9 @@ __global__ void __launch_bounds__(256) k_deposit(const T *__restrict__ pos, cons
     }
     __syncthreads();
     for (int j = threadIdx.x; j < BOX * BOX * BOX; j += blockDim.x) {
-        T v = box[j];
-        if (v != (T)0) {
+        const BoxT vb = box[j];
+        if (vb != (BoxT)0) {
+            const T v = FIXED ? (T)vb * inv_scale : (T)vb;
             int rz = j % BOX, ry = (j / BOX) % BOX, rx = j / (BOX * BOX);
             const int gy = (org[1] + ry) & M, gz = (org[2] + rz) & M;
             atomicAdd(rho + ((size_t)((org[0] + rx) & M) * N + gy) * N + gz, v);
