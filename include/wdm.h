@@ -125,9 +125,10 @@ int wdm_set_particle_mode(wdm_ctx *ctx, int substeps, int is_static);
 int wdm_set_assignment(wdm_ctx *ctx, int order);
 int wdm_get_assignment(wdm_ctx *ctx, int *order);
 
-/* Arithmetic of the particle deposit.  0 (default): floating-point atomics in shared and global memory -- the sum over
- * the particles of a node depends on their order, so the coupled result is reproducible only to rounding (1e-7
- * relative in complex64).  1: every weight is rounded once to 64-bit fixed point (a power-of-two scale chosen from the
+/* Arithmetic of the particle deposit.  0 (default): partial sums per chunk of 1024 sorted particles in shared memory
+ * (complex64: 32-bit fixed point, one unit = 5e-7 of the chunk's largest particle mass / dx^3; complex128: double),
+ * added to the mesh with floating-point atomics -- the sum over the particles of a node depends on their order, so the
+ * coupled result is reproducible only to rounding (1e-7 relative in complex64).  1: every weight is rounded once to 64-bit fixed point (a power-of-two scale chosen from the
  * total particle mass) and accumulated with integer atomics: the mesh, hence the whole coupled run, is bit-identical from
  * run to run (a debugging mode: 8 bytes per cell of extra device memory, cudaMalloc'ed on first use -- WDM_ENOMEM if that
  * fails -- a conversion pass per step, and one host synchronisation per particle set).  Either way the deposit is the
