@@ -249,6 +249,30 @@ __device__ __forceinline__ void gather_grad(const T *__restrict__ phi, const T (
         iz[d] = (c.base[2] + d - 1) & M;
     }
     a[0] = a[1] = a[2] = (T)0;
+    if constexpr (ORDER == 2) {
+        // cloud-in-cell: the 48 central-difference operands are 32 distinct nodes of the 4^3 neighbourhood (those with at
+        // most one coordinate outside the cell); load each once, 32-bit offsets (N^3 <= 2^30)
+        int ox[4], oy[4];
+#pragma unroll
+        for (int d = 0; d < 4; ++d) { ox[d] = ix[d] * N * N; oy[d] = iy[d] * N; }
+        T f[4][4][4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if ((i == 0 || i == 3) + (j == 0 || j == 3) + (k == 0 || k == 3) <= 1) f[i][j][k] = __ldg(phi + (ox[i] + oy[j] + iz[k]));
+#pragma unroll
+        for (int p = 1; p <= 2; ++p)
+#pragma unroll
+            for (int q = 1; q <= 2; ++q) {
+                a[0] += c.w[1][p - 1] * c.w[2][q - 1] * (c.w[0][0] * (f[2][p][q] - f[0][p][q]) + c.w[0][1] * (f[3][p][q] - f[1][p][q]));
+                a[1] += c.w[0][p - 1] * c.w[2][q - 1] * (c.w[1][0] * (f[p][2][q] - f[p][0][q]) + c.w[1][1] * (f[p][3][q] - f[p][1][q]));
+                a[2] += c.w[0][p - 1] * c.w[1][q - 1] * (c.w[2][0] * (f[p][q][2] - f[p][q][0]) + c.w[2][1] * (f[p][q][3] - f[p][q][1]));
+            }
+        return;
+    }
 #pragma unroll
     for (int bx = 0; bx < ORDER; ++bx)
 #pragma unroll
