@@ -28,8 +28,8 @@ def _sizes():
 
 
 def _newest_source() -> float:
-    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "wdm.h"),
-                                                              os.path.join(HERE, "..", "include", "wdm_dist.h")]
+    inc = os.path.join(HERE, "..", "include")
+    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(inc, f) for f in os.listdir(inc)]
     return max(os.path.getmtime(f) for f in files)
 
 

@@ -9,9 +9,13 @@
 // Correctness never depends on the order: the deposit falls back to global atomics for any node outside the
 // CTA's shared-memory box.
 #include <cmath>
+#include <cstdarg>
 #include <cstdint>
+#include <cstdio>
+#include <mutex>
 #include <type_traits>
 
+#include "../../include/wdm_static.h"
 #include "wdm_particles.hpp"
 
 namespace wdm {
@@ -710,3 +714,98 @@ cudaError_t particle_get(ParticleState &ps, int dtype, void *pos_out, void *vel_
 }
 
 }  // namespace wdm
+
+// ---------------------------------------------------------------- wdm_deposit_static (include/wdm_static.h)
+// The deterministic deposit with its accumulator mesh in a file-scope array instead of allocated memory: for
+// callers that must not allocate.  Every GPU that loads the library holds these 2 MiB until the process exits; every
+// call on a GPU shares them (overlapping calls race, see the header).
+//
+// In HOST code `g_static_acc` is only a stand-in for the symbol, not a device address: the address the kernels get is
+// looked up with cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned long long g_static_acc[WDM_STATIC_MAX_CELLS];
+
+namespace {
+
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+unsigned long long *g_static_ptr[kMaxDevices] = {};      // device address of g_static_acc on device d, once looked up
+thread_local char g_static_err[512] = "";               // fixed buffer: not even the error path allocates
+
+int sfail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_static_err, sizeof g_static_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+// set-up: the scratch address on the CURRENT device (cached per device)
+int static_scratch(unsigned long long **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return sfail(WDM_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= kMaxDevices) return sfail(WDM_EUNSUPPORTED, "device ordinal %d outside [0, %d)", dev, kMaxDevices);
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        unsigned long long *p = nullptr;
+        e = cudaGetSymbolAddress((void **)&p, g_static_acc);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return sfail(WDM_ECUDA, "cudaGetSymbolAddress of the static deposit scratch on device %d: %s", dev, cudaGetErrorString(e));
+        }
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return WDM_OK;
+}
+
+}  // namespace
+
+extern "C" size_t wdm_static_scratch_bytes(void) { return sizeof(unsigned long long) * WDM_STATIC_MAX_CELLS; }
+
+extern "C" const char *wdm_static_last_error(void) { return g_static_err; }
+
+extern "C" int wdm_deposit_static(const void *pos_dev, const void *mass_dev, double mass_scalar, long long n, int N, double L,
+                                  int dtype, int order, double total_mass, void *rho_out_dev, void *cuda_stream)
+{
+    using namespace wdm;
+    if (dtype != WDM_C64 && dtype != WDM_C128) return sfail(WDM_EINVAL, "dtype must be WDM_C64 or WDM_C128, got %d", dtype);
+    if (order != 2 && order != 3) return sfail(WDM_EINVAL, "assignment order must be 2 (cloud-in-cell) or 3 (triangular-shaped cloud), got %d", order);
+    if (n < 0 || n > 0x7fffffffll * 256) return sfail(WDM_EINVAL, "particle count %lld out of range", n);
+    if (!(L > 0) || !std::isfinite(L)) return sfail(WDM_EINVAL, "L must be positive and finite");
+    if (!(total_mass > 0) || !std::isfinite(total_mass)) return sfail(WDM_EINVAL, "total_mass must be positive and finite (an upper bound of sum |m_i|)");
+    if (!std::isfinite(mass_scalar)) return sfail(WDM_EINVAL, "mass_scalar must be finite");
+    if (N < 8 || (N & (N - 1)) != 0) return sfail(WDM_EUNSUPPORTED, "N must be a power of two >= 8, got %d", N);
+    if (N > WDM_STATIC_MAX_N)
+        return sfail(WDM_EUNSUPPORTED, "N = %d: N^3 cells exceed the static scratch (%llu cells, N <= %d); use a wdm_ctx with wdm_set_deposit_mode",
+                     N, (unsigned long long)WDM_STATIC_MAX_CELLS, WDM_STATIC_MAX_N);
+    if (!rho_out_dev || (n > 0 && !pos_dev)) return sfail(WDM_EINVAL, "null pointer");
+
+    unsigned long long *acc = nullptr;
+    if (int rc = static_scratch(&acc)) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t n3 = (size_t)N * N * N;
+    // the array keeps whatever the last call (possibly a failed or a differently sized one) left in it
+    cudaError_t e = cudaMemsetAsync(acc, 0, n3 * sizeof(unsigned long long), s);
+    if (e != cudaSuccess) return sfail(WDM_ECUDA, "cudaMemsetAsync of the static scratch: %s", cudaGetErrorString(e));
+    // the same scale as particle_deposit_fixed: the largest possible cell value is total_mass / dx^3, two bits of head room
+    const double dx = L / N, top = total_mass / (dx * dx * dx);
+    int ex = 0;
+    frexp(top, &ex);
+    const double scale = ldexp(1.0, 60 - ex);
+    if (n > 0) {
+        const unsigned g = blocks(n, 256);
+        if (dtype == WDM_C64 && order == 2) k_deposit_fixed<float, 2><<<g, 256, 0, s>>>((const float *)pos_dev, (const float *)mass_dev, (float)mass_scalar, acc, n, N, (float)L, scale);
+        else if (dtype == WDM_C64) k_deposit_fixed<float, 3><<<g, 256, 0, s>>>((const float *)pos_dev, (const float *)mass_dev, (float)mass_scalar, acc, n, N, (float)L, scale);
+        else if (order == 2) k_deposit_fixed<double, 2><<<g, 256, 0, s>>>((const double *)pos_dev, (const double *)mass_dev, mass_scalar, acc, n, N, L, scale);
+        else k_deposit_fixed<double, 3><<<g, 256, 0, s>>>((const double *)pos_dev, (const double *)mass_dev, mass_scalar, acc, n, N, L, scale);
+        if ((e = cudaGetLastError()) != cudaSuccess) return sfail(WDM_ECUDA, "deposit kernel launch: %s", cudaGetErrorString(e));
+    }
+    const unsigned gc = blocks((long long)n3, 256);
+    if (dtype == WDM_C64) k_fixed_to_mesh<float><<<gc, 256, 0, s>>>(acc, (float *)rho_out_dev, n3, 1.0 / scale);
+    else k_fixed_to_mesh<double><<<gc, 256, 0, s>>>(acc, (double *)rho_out_dev, n3, 1.0 / scale);
+    if ((e = cudaGetLastError()) != cudaSuccess) return sfail(WDM_ECUDA, "conversion kernel launch: %s", cudaGetErrorString(e));
+    return WDM_OK;
+}
