@@ -168,7 +168,9 @@ int wdm_get_step_diagnostics(wdm_ctx *ctx, double *out_host);
 /* Instrumentation.  wdm_launch_count: kernels launched by this context so far.  With profiling on,
  * every kernel launch is bracketed by CUDA events on the context's stream;
  * wdm_kernel_stats synchronises and returns, for slot i < *n_inout, the kernel name, the number of
- * timed launches and their summed duration in ms, then resets the accumulators. */
+ * timed launches and their summed duration in ms, then resets the accumulators.
+ * With WDM_NVTX=1 in the environment every launch is also wrapped in an NVTX range named like its slot
+ * ("psi_sweep_z_kick", "poisson_z_green", "particle_cic_deposit", ...) for timeline tools. */
 int wdm_launch_count(wdm_ctx *ctx, long long *count_out);
 int wdm_set_profiling(wdm_ctx *ctx, int on);
 int wdm_kernel_stats(wdm_ctx *ctx, int *n_inout, const char **names_out, long long *launches_out,

@@ -17,7 +17,10 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "../../include/wdm.h"
+
 #include "wdm_internal.hpp"
 #include "wdm_kernels.cuh"
 #include "wdm_particles.hpp"
@@ -314,6 +317,14 @@ static int prof_flush(wdm_ctx *c)
     return WDM_OK;
 }
 
+// NVTX range per launch, named like the kernel-statistics slot ("NVTX ranges per sweep"): switched on
+// by WDM_NVTX=1 in the environment; the header-only NVTX v3 costs one predictable branch when no tool is attached.
+static bool nvtx_on()
+{
+    static const bool on = [] { const char *e = getenv("WDM_NVTX"); return e && atoi(e) != 0; }();
+    return on;
+}
+
 // Brackets one launch with events when profiling is on.  A failing event call switches profiling off for the
 // context and leaves the text in wdm_last_error (the launch itself is unaffected; its own status is checked by CU).
 struct Timed {
@@ -332,6 +343,7 @@ struct Timed {
     Timed(wdm_ctx *c_, int slot_) : c(c_), slot(slot_), on(c_->profiling)
     {
         c->launches++;
+        if (nvtx_on()) nvtxRangePushA(kSlotNames[slot]);
         if (!on) return;
         if (c->ev_used * 2 >= c->ev.size()) {
             if (c->ev.size() >= 2 * 8192) {
@@ -347,7 +359,11 @@ struct Timed {
         c->ev_slot[idx] = slot;
         if (!ok(c, cudaEventRecord(c->ev[2 * idx], c->stream), "cudaEventRecord")) on = false;
     }
-    ~Timed() { if (on) ok(c, cudaEventRecord(c->ev[2 * idx + 1], c->stream), "cudaEventRecord"); }
+    ~Timed()
+    {
+        if (on) ok(c, cudaEventRecord(c->ev[2 * idx + 1], c->stream), "cudaEventRecord");
+        if (nvtx_on()) nvtxRangePop();
+    }
 };
 
 // ---------------------------------------------------------------- TMA descriptors
