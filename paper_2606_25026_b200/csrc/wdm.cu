@@ -369,9 +369,9 @@ struct Timed {
 // ---------------------------------------------------------------- TMA descriptors
 
 // (the encoder itself is in wdm_internal.hpp: encode_tmap)
-static int make_tmap(wdm_ctx *c, CUtensorMap *out, void *base, int nx, int axis, int rows)
+static int make_tmap(wdm_ctx *c, CUtensorMap *out, void *base, int nx, int axis, int rows, int W = 0)
 {
-    const int rc = encode_tmap(c->dtype, c->N, c->tab->fact.W, base, c->N, nx, axis, rows, out);
+    const int rc = encode_tmap(c->dtype, c->N, W ? W : c->tab->fact.W, base, c->N, nx, axis, rows, out);
     if (rc == -1) return fail(c, WDM_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
     if (rc != 0) return fail(c, WDM_ECUDA, "cuTensorMapEncodeTiled failed (%d) for N = %d axis %d rows %d", rc, c->N, axis, rows);
     return WDM_OK;
@@ -385,7 +385,8 @@ static int make_tmaps(wdm_ctx *c)
     int rc;
     if ((rc = make_tmap(c, &c->tm_psi_y, c->psi, N, 1, box_rows(N))) || (rc = make_tmap(c, &c->tm_psi_x, c->psi, N, 2, box_rows(N))) ||
         (rc = make_tmap(c, &c->tm_h_y, c->H, N / 2 + 1, 1, box_rows(N))) ||
-        (rc = make_tmap(c, &c->tm_h_x, c->H, N / 2 + 1, 2, box_rows(N / 2))) || (rc = make_tmap(c, &c->tm_h_x1, c->H, N / 2 + 1, 2, 1)))
+        (rc = make_tmap(c, &c->tm_h_x, c->H, N / 2 + 1, 2, box_rows(N / 2), c->tab->c2r_w)) ||          // the complex-to-real sweep's tiles
+        (rc = make_tmap(c, &c->tm_h_x1, c->H, N / 2 + 1, 2, 1, c->tab->c2r_w)))
         return rc;
     return WDM_OK;
 }

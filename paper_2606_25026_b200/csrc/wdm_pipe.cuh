@@ -909,4 +909,90 @@ struct C2RK {
     }
 };
 
+// Complex-to-real sweep IN PLACE, for tiles too large to hold a packed copy beside the half spectrum (1024-point lines:
+// with the copy only W = 8 fits three times in shared memory -- 32-byte rows of Phi, 64-byte rows of H, and half of a
+// group idle in every stage).  Here the tile buffer is the half spectrum alone, W = 16, and every stage has one
+// butterfly per thread.  Two facts make it work (N = RA RM, RA = RM, two real lines 2l, 2l+1 per complex line l):
+//   * frequency k = g + RA sM sits at position (g, sM) of the inverse transform, and its mirror N - k at position
+//     (RA - g, RM - 1 - sM).  The first stage of thread (l, g) needs Z_k of block g: sM < RM/2 from the rows k <= N/2 of
+//     its own block (Z_k = A_k + i B_k), the others from the rows of block RA - g (Z_{N-k} = conj A_k + i conj B_k): the
+//     Hermitian unsplit happens in the registers that feed the butterfly, 32 conflict-free 16-byte loads per thread.
+//   * its RM outputs (g, r) go back as 16-byte pairs (r, r + RM/2) over the rows g + RA r of its own block -- rows the
+//     thread of block RA - g has read as well, hence one group barrier between the loads and the stores.  The last
+//     stage of thread (l, q) then finds (s, q), s < RA, in RA consecutive rows, in half q / (RM/2) of the pair; a warp
+//     holds q and q + RM/2 together, so its 8-byte loads cover whole 128-byte rows.
+// Rows k = 0 and k = N/2 drop their imaginary parts as in C2RK (reading G33).
+template <class C_, bool EXT, int DG_ = 0, int AXR = AX_X>
+struct C2RI {
+    static constexpr int DG = DG_;
+    static constexpr bool DIAG_ZEROES = false;
+    using C = C_;
+    using T = typename C::T;
+    using TL = Tile<C, AXR>;
+    static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA, WP = W / 2, HM = RM / 2;
+    static_assert(C::RB == 1 && RA == RM && NTG == WP * RA, "one butterfly per thread in both stages");
+    static constexpr size_t TILE_BYTES = align128((size_t)(N / 2 + 1) * W * sizeof(cx<T>));
+    static constexpr int AUX = AUX_NONE;
+    using Pre = NoPre;
+    struct Pers {
+        __device__ __forceinline__ void setup(const Tabs<T> &, int) {}
+    };
+    static __device__ __forceinline__ void flush(const SweepParams<T> &p, const Pre &pre) { diag_flush(p.diag, pre.d, -1, -1, 6); }
+    static __device__ __forceinline__ void issue(const SweepParams<T> &p, int t, unsigned char *buf, uint64_t *bar, int lane)
+    {
+        tile_load<C, AXR, N / 2 + 1>(reinterpret_cast<cx<T> *>(buf), p.H, &p.tmap, &p.tmap2, t, bar, lane);
+    }
+    static __device__ __forceinline__ void prefetch(const SweepParams<T> &, int, int, Pre &) {}
+    template <class HOOK>
+    static __device__ __forceinline__ void compute(const SweepParams<T> &p, const Tabs<T> &tb, int t, unsigned char *buf, int gt, int grp, Pre &pre,
+                                                   const Pers &, HOOK &&)
+    {
+        cx<T> *R = reinterpret_cast<cx<T> *>(buf);
+        const int l = gt % WP;
+        const TL tile(p, t);
+        {
+            const int g = gt / WP;
+            cx<T> *ra = R + g * W + 2 * l;
+            const cx<T> *rb = R + (RA - g) * W + 2 * l;
+            cx<T> v[RM];
+            static_for<0, HM>([&](auto i_) {
+                constexpr int i = decltype(i_)::value;
+                cx<T> A, B;
+                ld2(ra + i * RA * W, A, B);                                  // k = g + RA i
+                if (i == 0 && g == 0) A.y = B.y = (T)0;                      // k = 0
+                v[brev(i, RM)] = mk<T>(A.x - B.y, A.y + B.x);
+                ld2(rb + i * RA * W, A, B);                                  // k' = RA - g + RA i, for N - k' = g + RA (RM - 1 - i)
+                if (i == HM - 1 && g == 0) A.y = B.y = (T)0;                 // k' = N/2
+                v[brev(RM - 1 - i, RM)] = mk<T>(A.x + B.y, B.x - A.y);
+            });
+            dit_inv<RM>(v);
+            group_sync(grp, NTG);                                            // every thread has read its rows
+            static_for<0, HM>([&](auto r_) {
+                constexpr int r = decltype(r_)::value;
+                st2(ra + r * RA * W, v[r], v[r + HM]);
+            });
+        }
+        group_sync(grp, NTG);
+        {
+            const int t2 = gt / WP, q = (t2 & 1) * HM + (t2 >> 1);
+            const cx<T> *src = R + (RA * (q % HM)) * W + 2 * l + q / HM;
+            T pmax = (T)0;
+            T *gp = p.phi_out + tile.at(q, 2 * l);
+            const T *ge = EXT ? p.phi_ext + tile.at(q, 2 * l) : nullptr;           // Phi_total = Phi_DM + Phi_ext (Alg. 1 l.15)
+            auto out = [&](int row, cx<T> v) {
+                // Re -> line 2l, Im -> line 2l+1: one (re, im) pair is two adjacent reals of Phi
+                if constexpr (EXT) {
+                    cx<T> e = ldg(reinterpret_cast<const cx<T> *>(ge + (long long)(row - q) * TL::RSTRIDE));
+                    v.x += e.x;
+                    v.y += e.y;
+                }
+                if constexpr (DG == 1) pmax = fmax(pmax, fmax(fabs(v.x), fabs(v.y)));
+                stv(reinterpret_cast<cx<T> *>(gp + (long long)(row - q) * TL::RSTRIDE), v);
+            };
+            inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return src[((row - q) / mA) * W]; }, out);
+            if constexpr (DG == 1) pre.d.mx = fmax(pre.d.mx, (double)pmax);
+        }
+    }
+};
+
 }  // namespace wdm

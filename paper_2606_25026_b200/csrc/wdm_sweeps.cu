@@ -76,8 +76,18 @@ using RhoOnly = PsiK<C, AX_X, 0, true, false>;
 using HYF = HK<C, H_Y_FWD>;
 using HZG = HK<C, H_Z_GREEN>;
 using HYI = HK<C, H_Y_INV>;
-using C2R = C2RK<C, false>;
-using C2RExt = C2RK<C, true>;
+// complex-to-real sweep: in place with W = 16 tiles where the packed copy would force W = 8 (1024-point complex64 lines)
+#if WDM_DTYPE == 0 && WDM_N == 1024
+using CR = LineCfg<Real, 1024, 32, 1, 32, 16, 256, 2, 1>;
+template <bool EXT, int DG> using C2RSel = C2RI<CR, EXT, DG>;
+#else
+using CR = C;
+template <bool EXT, int DG> using C2RSel = C2RK<C, EXT, DG>;
+#endif
+static_assert(CR::NT * CR::NG == kThreads && CR::MINB == C::MINB, "one launch shape for every sweep of a size");
+constexpr int kTilesC2R = CR::N * CR::N / CR::W;
+using C2R = C2RSel<false, 0>;
+using C2RExt = C2RSel<true, 0>;
 // the same sweeps accumulating the per-step diagnostics (wdm_set_step_diagnostics), and the forward-only sweeps that
 // measure the spectral kinetic energy on demand (wdm_get_diagnostics)
 using PsiZKickD = PsiK<C, AX_CONTIG, 1, false, true, 1>;
@@ -87,8 +97,8 @@ using PsiSD = PsiK<C, AX_Y, 0, false, true, 1>;
 using PsiXD = PsiK<C, AX_X, 0, false, true, 1>;
 using PsiXRhoD = PsiK<C, AX_X, 0, true, true, 1>;
 using HZGD = HK<C, H_Z_GREEN, 1>;
-using C2RD = C2RK<C, false, 1>;
-using C2RExtD = C2RK<C, true, 1>;
+using C2RD = C2RSel<false, 1>;
+using C2RExtD = C2RSel<true, 1>;
 using PsiZM = PsiK<C, AX_CONTIG, 0, false, true, 2>;
 using PsiSM = PsiK<C, AX_Y, 0, false, true, 2>;
 using PsiXM = PsiK<C, AX_X, 0, false, true, 2>;
@@ -131,8 +141,8 @@ cudaError_t h_y_inv(const void *pp, cudaStream_t s) { return launch<HYI>(pp, kTi
 cudaError_t c2r(const void *pp, int diag, cudaStream_t s)
 {
     const bool ext = static_cast<const P *>(pp)->phi_ext != nullptr;
-    if (diag == 1) return ext ? launch<C2RExtD>(pp, kTilesGrid, s) : launch<C2RD>(pp, kTilesGrid, s);
-    return ext ? launch<C2RExt>(pp, kTilesGrid, s) : launch<C2R>(pp, kTilesGrid, s);
+    if (diag == 1) return ext ? launch<C2RExtD>(pp, kTilesC2R, s) : launch<C2RD>(pp, kTilesC2R, s);
+    return ext ? launch<C2RExt>(pp, kTilesC2R, s) : launch<C2R>(pp, kTilesC2R, s);
 }
 
 // ---- slab-decomposed runs (wdm_dist.cu): the same sweeps on slab-shaped arrays, tile count given by the caller; the
@@ -157,7 +167,7 @@ cudaError_t dist_h_y(const void *pp, int inverse, int ntiles, cudaStream_t s) { 
 cudaError_t dist_h_z_green(const void *pp, int ntiles, cudaStream_t s) { return launch<HZG>(pp, ntiles, s); }
 cudaError_t dist_c2r(const void *pp, int ntiles, cudaStream_t s) { return launch<C2RT>(pp, ntiles, s); }
 
-const SweepTable kTable = {Fact{C::N, C::RA, C::RB, C::RM, C::W, C::NT, C::NG, C::MINB}, WDM_DTYPE, init, psi_z,
+const SweepTable kTable = {Fact{C::N, C::RA, C::RB, C::RM, C::W, C::NT, C::NG, C::MINB}, WDM_DTYPE, CR::W, init, psi_z,
                            psi_strided, psi_x_rho, h_y_fwd, h_z_green, h_y_inv, c2r,
                            dist_init, dist_psi_z, dist_psi_y, dist_psi_x_rho, dist_h_y, dist_h_z_green, dist_c2r};
 

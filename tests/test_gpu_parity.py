@@ -629,6 +629,48 @@ def test_config4_1024_c64_against_c128(wdm):
         assert mx / mb <= MAXABS * t, (name, mx / mb)
 
 
+def test_1024_c64_external_potential_and_step_diagnostics_against_c128(wdm):
+    """The complex-to-real sweep of 1024^3 complex64 is an instantiation of its own (in place, 16-line tiles): its
+    external-potential and per-step-diagnostics forms against the complex128 library run (packed-copy sweep, three
+    levels), two steps of config 4 with a smooth Phi_ext of the size of the self-potential added on the way out
+    (Alg. 1 l.15).  Phi_total, psi and max |Phi_total| of the step diagnostics."""
+    import torch
+    w = wl.config4()
+    N = w.N
+    psi0 = torch.from_numpy(w.psi).cuda()
+    x = torch.arange(N, device="cuda", dtype=torch.float64) * (2 * math.pi / N)
+    out = {}
+    for dtype in ("c64", "c128"):
+        sim = wdm.Sim(N, w.L, w.hbar_over_m, w.G, dtype)
+        sim.set_psi(psi0)
+        scale = float(sim.potential().abs().max())
+        ext = (scale * (torch.cos(x)[:, None, None] * torch.sin(2 * x)[None, :, None] + 0.5 * torch.cos(3 * x + 0.3)[None, None, :]))
+        ext = ext.to(torch.float32 if dtype == "c64" else torch.float64).contiguous()
+        sim.set_kick_terms(phi_ext=ext)
+        sim.set_step_diagnostics(True)
+        sim.step(2, w.dt)
+        d = sim.step_diagnostics()
+        out[dtype] = (sim.psi(), sim.potential(), d["max_phi"])
+        sim.close()
+        del sim, ext
+        torch.cuda.empty_cache()
+    t = tol("c64", 2)
+    for i, name in enumerate(("psi", "Phi_total")):
+        a, b = out["c64"][i], out["c128"][i]
+        num = den = 0.0
+        mx = mb = 0.0
+        for x0 in range(0, N, 64):
+            bb = b[x0:x0 + 64]
+            dd = a[x0:x0 + 64].to(bb.dtype) - bb
+            num += float((dd.abs() ** 2).sum()); den += float((bb.abs() ** 2).sum())
+            mx = max(mx, float(dd.abs().max())); mb = max(mb, float(bb.abs().max()))
+        e = math.sqrt(num / den)
+        assert e <= t, (name, e)
+        assert mx / mb <= MAXABS * t, (name, mx / mb)
+    assert abs(out["c64"][2] / out["c128"][2] - 1) <= 10 * t
+    assert abs(out["c128"][2] / float(out["c128"][1].abs().max()) - 1) <= 1e-12      # the diagnostic is the maximum of what came out
+
+
 # ---------------------------------------------------------------- large kick phases (reading G25)
 
 @pytest.mark.parametrize("terms", ["plain", "kappa_layer"])
