@@ -930,7 +930,7 @@ struct C2RI {
     using T = typename C::T;
     using TL = Tile<C, AXR>;
     static constexpr int N = C::N, RA = C::RA, RM = C::RM, W = C::W, NTG = C::NT, mA = C::mA, WP = W / 2, HM = RM / 2;
-    static_assert(C::RB == 1 && RA == RM && NTG == WP * RA, "one butterfly per thread in both stages");
+    static_assert(C::RB == 1 && NTG == WP * RA && (mA * WP) % NTG == 0, "one first-stage butterfly per thread, whole rounds of the last stage");
     static constexpr size_t TILE_BYTES = align128((size_t)(N / 2 + 1) * W * sizeof(cx<T>));
     static constexpr int AUX = AUX_NONE;
     using Pre = NoPre;
@@ -973,10 +973,10 @@ struct C2RI {
             });
         }
         group_sync(grp, NTG);
-        {
-            const int t2 = gt / WP, q = (t2 & 1) * HM + (t2 >> 1);
+        T pmax = (T)0;
+        for (int b = gt; b < mA * WP; b += NTG) {
+            const int t2 = b / WP, q = (t2 & 1) * HM + (t2 >> 1);
             const cx<T> *src = R + (RA * (q % HM)) * W + 2 * l + q / HM;
-            T pmax = (T)0;
             T *gp = p.phi_out + tile.at(q, 2 * l);
             const T *ge = EXT ? p.phi_ext + tile.at(q, 2 * l) : nullptr;           // Phi_total = Phi_DM + Phi_ext (Alg. 1 l.15)
             auto out = [&](int row, cx<T> v) {
@@ -990,8 +990,8 @@ struct C2RI {
                 stv(reinterpret_cast<cx<T> *>(gp + (long long)(row - q) * TL::RSTRIDE), v);
             };
             inv_level<RA, T>(q, mA, tb.twA + q, [&](int row) { return src[((row - q) / mA) * W]; }, out);
-            if constexpr (DG == 1) pre.d.mx = fmax(pre.d.mx, (double)pmax);
         }
+        if constexpr (DG == 1) pre.d.mx = fmax(pre.d.mx, (double)pmax);
     }
 };
 

@@ -76,9 +76,13 @@ using RhoOnly = PsiK<C, AX_X, 0, true, false>;
 using HYF = HK<C, H_Y_FWD>;
 using HZG = HK<C, H_Z_GREEN>;
 using HYI = HK<C, H_Y_INV>;
-// complex-to-real sweep: in place with W = 16 tiles where the packed copy would force W = 8 (1024-point complex64 lines)
+// complex-to-real sweep: in place where the tile buffer then holds twice the lines of the packed-copy form (W = 16 instead
+// of 8 for 1024-point complex64 lines, 32 instead of 16 for 512-point ones)
 #if WDM_DTYPE == 0 && WDM_N == 1024
 using CR = LineCfg<Real, 1024, 32, 1, 32, 16, 256, 2, 1>;
+template <bool EXT, int DG> using C2RSel = C2RI<CR, EXT, DG>;
+#elif WDM_DTYPE == 0 && WDM_N == 512
+using CR = LineCfg<Real, 512, 16, 1, 32, 32, 256, 2, 1>;
 template <bool EXT, int DG> using C2RSel = C2RI<CR, EXT, DG>;
 #else
 using CR = C;
