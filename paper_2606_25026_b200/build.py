@@ -10,8 +10,9 @@ from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-OBJ = os.path.join(HERE, "build")
-LIB = os.path.join(HERE, "libwdm.so")
+# WDM_BUILD_DIR / WDM_LIB_OUT / WDM_NVCC_FLAGS: a second build beside the product's (developer A/B runs of a compile-time switch)
+OBJ = os.environ.get("WDM_BUILD_DIR", os.path.join(HERE, "build"))
+LIB = os.environ.get("WDM_LIB_OUT", os.path.join(HERE, "libwdm.so"))
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
          "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC"]
@@ -47,7 +48,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         out = os.path.join(OBJ, name)
         if not force and os.path.exists(out) and os.path.getmtime(out) >= newest:
             return out
-        cmd = [NVCC, *FLAGS, *(["-Xptxas", "-v"] if verbose else []), *args, "-o", out]
+        cmd = [NVCC, *FLAGS, *os.environ.get("WDM_NVCC_FLAGS", "").split(), *(["-Xptxas", "-v"] if verbose else []), *args, "-o", out]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed for {name}:\n{r.stdout}\n{r.stderr}")
