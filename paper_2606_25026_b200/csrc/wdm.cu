@@ -205,6 +205,7 @@ struct wdm_ctx {
     void *psi = nullptr, *phi = nullptr, *H = nullptr;
     void *rho_mean = nullptr;   // [0..1] double accumulators, then the mean as T at byte offset 16
     void *twA = nullptr, *twB = nullptr, *phase = nullptr, *ksq_pos = nullptr, *ksq_nat = nullptr;
+    void *x2tab = nullptr;                    // tables of the half-tile x sweeps (tab->x2_w != 0): 2 N complex, the second half follows dt
     double phase_dt = 0;
     bool phase_valid = false, have_psi = false, stale = true;
     // particle variants (wdm_set_particle_mode; reading G29)
@@ -229,7 +230,7 @@ struct wdm_ctx {
     double mask_dt = 0;
     bool mask_valid = false;
     // TMA descriptors (see SweepParams): psi along y / x, H along y / x, H single row along x
-    CUtensorMap tm_psi_y, tm_psi_x, tm_h_y, tm_h_x, tm_h_x1;
+    CUtensorMap tm_psi_y, tm_psi_x, tm_h_y, tm_h_x, tm_h_x1, tm_psi_x2;
     unsigned int *tickets = nullptr;          // two tile-ticket words used by alternate sweep launches
     int ticket_parity = 0;
     int l2_reverse = 1;                       // see SweepParams::reverse (WDM_L2_REVERSE=0 switches it off for A/B runs)
@@ -280,6 +281,7 @@ static size_t grid_bytes(int N, int dtype, long long max_particles)
     size_t b = align_up(n * c) + align_up(n * r) + align_up(nH * c);
     b += 3 * align_up((size_t)N * c) + 2 * align_up((size_t)N * r) + align_up((size_t)N * 2) + 256;
     b += align_up((size_t)(2 * N + 2 + 8) * sizeof(unsigned int)) + align_up((size_t)3 * N * r) + align_up(3 * DIAG_COUNT * sizeof(double));
+    b += align_up((size_t)2 * N * c);                                  // tables of the half-tile x sweeps (where built)
     if (max_particles > 0) b += align_up(n * r) + particle_bytes(N, dtype, max_particles);
     return b + 4096;
 }
@@ -388,6 +390,7 @@ static int make_tmaps(wdm_ctx *c)
         (rc = make_tmap(c, &c->tm_h_x, c->H, N / 2 + 1, 2, box_rows(N / 2), c->tab->c2r_w)) ||          // the complex-to-real sweep's tiles
         (rc = make_tmap(c, &c->tm_h_x1, c->H, N / 2 + 1, 2, 1, c->tab->c2r_w)))
         return rc;
+    if (c->tab->x2_w && (rc = make_tmap(c, &c->tm_psi_x2, c->psi, N, 2, 256, c->tab->x2_w))) return rc;
     return WDM_OK;
 }
 
@@ -399,6 +402,13 @@ static int upload_tables(wdm_ctx *c)
     Tables<T> t = build_tables<T>(c->tab->fact, c->L);
     CU(c, cudaMemcpyAsync(c->twA, t.twA.data(), t.twA.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(c->twB, t.twB.data(), t.twB.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, c->stream));
+    std::vector<cx<T>> x2;
+    if (c->tab->x2_w) {
+        Fact half;
+        if (!find_fact(c->N / 2, c->dtype, half)) return fail(c, WDM_EUNSUPPORTED, "no factorisation for the half line");
+        x2 = build_x2_static<T>(c->N, half);
+        CU(c, cudaMemcpyAsync(c->x2tab, x2.data(), x2.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, c->stream));
+    }
     CU(c, cudaMemcpyAsync(c->ksq_pos, t.ksq_pos.data(), t.ksq_pos.size() * sizeof(T), cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(c->ksq_nat, t.ksq_nat.data(), t.ksq_nat.size() * sizeof(T), cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));   // host vectors die here
@@ -411,6 +421,13 @@ static int ensure_phase(wdm_ctx *c, double dt)
     if (c->phase_valid && c->phase_dt == dt) return WDM_OK;
     std::vector<cx<T>> ph = build_phase<T>(c->tab->fact, c->L, c->mu, dt);
     CU(c, cudaMemcpyAsync(c->phase, ph.data(), ph.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, c->stream));
+    std::vector<cx<T>> x2;
+    if (c->tab->x2_w) {
+        Fact half;
+        if (!find_fact(c->N / 2, c->dtype, half)) return fail(c, WDM_EUNSUPPORTED, "no factorisation for the half line");
+        x2 = build_x2_phase<T>(c->N, half, c->L, c->mu, dt);
+        CU(c, cudaMemcpyAsync((cx<T> *)c->x2tab + c->N, x2.data(), x2.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, c->stream));
+    }
     CU(c, cudaStreamSynchronize(c->stream));
     c->phase_dt = dt;
     c->phase_valid = true;
@@ -456,6 +473,7 @@ static SweepParams<T> base_params(wdm_ctx *c)
     const int N = c->N;
     p.twA = (const cx<T> *)c->twA;
     p.twB = (const cx<T> *)c->twB;
+    p.x2tab = (const cx<T> *)c->x2tab;
     p.phase = (const cx<T> *)c->phase;
     p.ksq_pos = (const T *)c->ksq_pos;
     p.ksq_nat = (const T *)c->ksq_nat;
@@ -483,6 +501,7 @@ static int density_poisson(wdm_ctx *c, bool drift, int dg = 0)
         SweepParams<T> p = base_params<T>(c);
         p.data = (cx<T> *)c->psi;
         p.tmap = c->tm_psi_x;
+        p.tmap2 = c->tm_psi_x2;
         take_ticket(c, p);
         Timed t(c, S_PSI_X_RHO);
         CU(c, c->tab->psi_x_rho(&p, drift ? 1 : 0, dg, c->stream));
@@ -658,6 +677,7 @@ static int step_impl(wdm_ctx *c, int nsteps, double dt)
             SweepParams<T> p = base_params<T>(c);
             p.data = (cx<T> *)c->psi;
             p.tmap = c->tm_psi_x;
+            p.tmap2 = c->tm_psi_x2;
             take_ticket(c, p);
             Timed t(c, S_PSI_Y);
             CU(c, c->tab->psi_strided(&p, 1, dg, c->stream));
@@ -730,7 +750,7 @@ static int create_common(wdm_ctx **out, int N, double L, double mu, double G, in
         (rc = ctx_alloc(c, &c->ksq_pos, N * rs)) || (rc = ctx_alloc(c, &c->ksq_nat, N * rs)) ||
         (rc = ctx_alloc(c, &c->rho_mean, 64)) ||
         (rc = ctx_alloc(c, (void **)&c->tickets, 8 * sizeof(unsigned int))) ||
-        (rc = ctx_alloc(c, &c->mask, (size_t)3 * N * rs)) || (rc = ctx_alloc(c, (void **)&c->diag_dev, 3 * DIAG_COUNT * sizeof(double))))
+        (rc = ctx_alloc(c, &c->mask, (size_t)3 * N * rs)) || (c->tab->x2_w && (rc = ctx_alloc(c, &c->x2tab, (size_t)2 * N * cs))) || (rc = ctx_alloc(c, (void **)&c->diag_dev, 3 * DIAG_COUNT * sizeof(double))))
         return bail(rc);
     if (cudaMemset(c->tickets, 0, 8 * sizeof(unsigned int)) != cudaSuccess)
         return bail(fail(c, WDM_ECUDA, "cudaMemset of the ticket words failed"));

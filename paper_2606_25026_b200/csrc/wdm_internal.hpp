@@ -11,7 +11,8 @@ namespace wdm {
 struct SweepTable {
     Fact fact;
     int dtype;
-    int c2r_w;                                                           // lines per tile of the complex-to-real sweep (fact.W unless that sweep runs in place)
+    int c2r_w;
+    int x2_w;                                                            // 0, or the lines per tile of the half-tile x sweeps (wdm_x2.cuh): the host then supplies their tables and boxes                                                           // lines per tile of the complex-to-real sweep (fact.W unless that sweep runs in place)
     cudaError_t (*init)();                                               // opt in to > 48 KB dynamic shared memory
     // diag: 0 plain; 1 the instantiation that also accumulates the per-step diagnostics into params->diag; 2 (psi sweeps,
     // no kick) forward transform only, sum k^2 |F psi|^2 into params->diag, nothing written

@@ -129,6 +129,7 @@ struct SweepParams {
     cx<T> *data;               // psi (N^3) or H ((N/2+1) N^2), transformed in place
     const cx<T> *twA;          // level-A twiddles, s-major: twA[s*mA + q] = exp(-2 pi i q s / N)
     const cx<T> *twB;          // level-B twiddles, s-major over the sub-block
+    const cx<T> *x2tab;        // wdm_x2.cuh (x sweeps on half tiles; tmap2 = the 16-line boxes): 4 tables of N/2 entries, or nullptr
     const cx<T> *phase;        // psi sweeps: exp(-i mu k^2 dt/2)/N in position order
     const T *phi;              // KICK: potential, same shape as psi
     T kick;                    // KICK: theta = phi * kick   (dt/(2 mu) or dt/mu)

@@ -109,4 +109,34 @@ inline std::vector<cx<T>> build_phase(const Fact &f, double L, double mu, double
     return ph;
 }
 
+// Tables of the half-tile x sweeps (wdm_x2.cuh): a line of N points as two half lines one radix-2 stage apart.
+//   static part : [level-A twiddles of the N/2-point transform (s-major): N/2 | w^n = exp(-2 pi i n / N), n < N/2 : N/2]
+//   phase part  : the per-axis kinetic factor / N (build_phase) of frequency 2 k' and of 2 k' + 1 at the position of k' in
+//                 the N/2-point transform: [even: N/2 | odd: N/2]
+template <typename T>
+inline std::vector<cx<T>> build_x2_static(int N, const Fact &half)
+{
+    const int NH = N / 2, mA = NH / half.RA;
+    std::vector<cx<T>> t(2 * (size_t)NH);
+    for (int s = 0; s < half.RA; ++s)
+        for (int q = 0; q < mA; ++q) t[s * mA + q] = unit_root<T>((long long)q * s, NH);
+    for (int n = 0; n < NH; ++n) t[NH + n] = unit_root<T>(n, N);
+    return t;
+}
+
+template <typename T>
+inline std::vector<cx<T>> build_x2_phase(int N, const Fact &half, double L, double mu, double dt)
+{
+    const int NH = N / 2;
+    std::vector<cx<T>> t(2 * (size_t)NH);
+    for (int p = 0; p < NH; ++p) {
+        const int k5 = k_of_pos(p, half.RA, half.RB, half.RM);
+        for (int odd = 0; odd < 2; ++odd) {
+            const double kk = wavenumber(2 * k5 + odd, N, L), th = -0.5 * mu * kk * kk * dt;
+            t[odd * NH + p] = mk<T>((T)(std::cos(th) / N), (T)(std::sin(th) / N));
+        }
+    }
+    return t;
+}
+
 }  // namespace wdm

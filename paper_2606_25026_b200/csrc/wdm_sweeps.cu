@@ -2,6 +2,9 @@
 // with -DWDM_DTYPE={0,1} -DWDM_N=<N>.  build.py compiles this file once per supported size.
 #include "wdm_internal.hpp"
 #include "wdm_pipe.cuh"
+#if WDM_DTYPE == 0 && WDM_N == 1024
+#include "wdm_x2.cuh"
+#endif
 
 #ifndef WDM_DTYPE
 #error "compile with -DWDM_DTYPE=0|1 -DWDM_N=<N>"
@@ -66,6 +69,40 @@ cudaError_t launch(const void *pp, int ntiles, cudaStream_t s)
     return cudaLaunchKernelEx(&cfg, k_pipe<K>, *static_cast<const P *>(pp), ntiles);
 }
 
+// x-direction psi sweep and density sweep on half tiles (wdm_x2.cuh): 1024-point complex64 lines
+#if WDM_DTYPE == 0 && WDM_N == 1024
+#define WDM_HAVE_X2 1
+using C5 = LineCfg<Real, 512, 16, 1, 32, 16, 256, 2, 1>;
+constexpr int kX2W = C5::W, kTilesX2 = C::N * C::N / C5::W;
+static_assert(kThreads == 512 && C::MINB == 1, "launch shape of the half-tile sweeps");
+
+template <bool RHO>
+__global__ void __launch_bounds__(512, 1) k_x2(const __grid_constant__ P p, const int ntiles)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    X2<C5, RHO>::run(p, ntiles, smem);
+}
+
+template <bool RHO>
+cudaError_t launch_x2(const void *pp, cudaStream_t s)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(kTilesX2 < g_ctas ? kTilesX2 : g_ctas);
+    cfg.blockDim = dim3(512);
+    cfg.dynamicSmemBytes = X2<C5, RHO>::TOTAL;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_x2<RHO>, *static_cast<const P *>(pp), kTilesX2);
+}
+#else
+#define WDM_HAVE_X2 0
+constexpr int kX2W = 0;
+#endif
+
 using PsiZKick = PsiK<C, AX_CONTIG, 1, false, true>;
 using PsiZKickX = PsiK<C, AX_CONTIG, 2, false, true>;
 using PsiZ = PsiK<C, AX_CONTIG, 0, false, true>;
@@ -118,6 +155,10 @@ cudaError_t init()
     OPT(PsiZKick) OPT(PsiZKickX) OPT(C2RExt) OPT(PsiZ) OPT(PsiS) OPT(PsiX) OPT(PsiXRho) OPT(RhoOnly) OPT(HYF) OPT(HZG) OPT(HYI) OPT(C2R)
     OPT(PsiZKickD) OPT(PsiZKickXD) OPT(PsiZD) OPT(PsiSD) OPT(PsiXD) OPT(PsiXRhoD) OPT(HZGD) OPT(C2RD) OPT(C2RExtD) OPT(PsiZM) OPT(PsiSM) OPT(PsiXM)
 #undef OPT
+#if WDM_HAVE_X2
+    if ((e = cudaFuncSetAttribute(k_x2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)X2<C5, false>::TOTAL)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_x2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)X2<C5, true>::TOTAL)) != cudaSuccess) return e;
+#endif
     return cudaSuccess;
 }
 
@@ -130,12 +171,18 @@ cudaError_t psi_z(const void *pp, int kick, int diag, cudaStream_t s)
 }
 cudaError_t psi_strided(const void *pp, int along_x, int diag, cudaStream_t s)
 {
+#if WDM_HAVE_X2
+    if (along_x && diag == 0 && static_cast<const P *>(pp)->x2tab) return launch_x2<false>(pp, s);
+#endif
     if (diag == 2) return along_x ? launch<PsiXM>(pp, kTilesGrid, s) : launch<PsiSM>(pp, kTilesGrid, s);
     if (diag == 1) return along_x ? launch<PsiXD>(pp, kTilesGrid, s) : launch<PsiSD>(pp, kTilesGrid, s);
     return along_x ? launch<PsiX>(pp, kTilesGrid, s) : launch<PsiS>(pp, kTilesGrid, s);
 }
 cudaError_t psi_x_rho(const void *pp, int drift, int diag, cudaStream_t s)
 {
+#if WDM_HAVE_X2
+    if (drift && diag == 0 && static_cast<const P *>(pp)->x2tab) return launch_x2<true>(pp, s);
+#endif
     if (diag == 1 && drift) return launch<PsiXRhoD>(pp, kTilesGrid, s);
     return drift ? launch<PsiXRho>(pp, kTilesGrid, s) : launch<RhoOnly>(pp, kTilesGrid, s);
 }
@@ -171,7 +218,7 @@ cudaError_t dist_h_y(const void *pp, int inverse, int ntiles, cudaStream_t s) { 
 cudaError_t dist_h_z_green(const void *pp, int ntiles, cudaStream_t s) { return launch<HZG>(pp, ntiles, s); }
 cudaError_t dist_c2r(const void *pp, int ntiles, cudaStream_t s) { return launch<C2RT>(pp, ntiles, s); }
 
-const SweepTable kTable = {Fact{C::N, C::RA, C::RB, C::RM, C::W, C::NT, C::NG, C::MINB}, WDM_DTYPE, CR::W, init, psi_z,
+const SweepTable kTable = {Fact{C::N, C::RA, C::RB, C::RM, C::W, C::NT, C::NG, C::MINB}, WDM_DTYPE, CR::W, kX2W, init, psi_z,
                            psi_strided, psi_x_rho, h_y_fwd, h_z_green, h_y_inv, c2r,
                            dist_init, dist_psi_z, dist_psi_y, dist_psi_x_rho, dist_h_y, dist_h_z_green, dist_c2r};
 

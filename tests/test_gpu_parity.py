@@ -671,6 +671,52 @@ def test_1024_c64_external_potential_and_step_diagnostics_against_c128(wdm):
     assert abs(out["c128"][2] / float(out["c128"][1].abs().max()) - 1) <= 1e-12      # the diagnostic is the maximum of what came out
 
 
+def test_1024_c64_coupled_particles_against_c128(wdm):
+    """The density sweep of 1024^3 complex64 runs on half tiles (wdm_x2.cuh); its particle-mesh branch (flagged columns of
+    rho_p added to |psi|^2 before the real-to-complex transform) and the coupled step around it against the complex128
+    run, which uses the generic sweeps: config 4's field plus a clump and a sprinkling of particles carrying a tenth of
+    the mass, three steps."""
+    import torch
+    w = wl.config4()
+    N, nsteps = w.N, 3
+    rng = np.random.Generator(np.random.PCG64(wl.SEED_BASE + 4104))
+    n_p = 20000
+    pos = np.concatenate([rng.normal(0.0, 0.03 * w.L, size=(n_p - 2000, 3)) + np.array([0.11, -0.07, 0.05]) * w.L,
+                          rng.uniform(-0.5 * w.L, 0.5 * w.L, size=(2000, 3))])
+    pos = (pos + 0.5 * w.L) % w.L - 0.5 * w.L
+    vel = rng.normal(0.0, 0.05, size=(n_p, 3))
+    psi0 = torch.from_numpy(w.psi).cuda()
+    mass = 0.1 * float((psi0.abs().double() ** 2).sum()) * (w.L / N) ** 3 / n_p
+    out = {}
+    for dtype in ("c64", "c128"):
+        sim = wdm.Sim(N, w.L, w.hbar_over_m, w.G, dtype, max_particles=n_p)
+        sim.set_psi(psi0)
+        rdt = np.float32 if dtype == "c64" else np.float64
+        sim.set_particles(pos.astype(np.float32).astype(rdt), vel.astype(np.float32).astype(rdt), mass)
+        sim.step(nsteps, w.dt)
+        pp, _ = sim.particles()
+        out[dtype] = (sim.psi(), sim.potential(), pp.double().cpu().numpy())
+        sim.close()
+        del sim
+        torch.cuda.empty_cache()
+    t = tol("c64", nsteps)
+    for i, name in enumerate(("psi", "Phi")):
+        a, b = out["c64"][i], out["c128"][i]
+        num = den = 0.0
+        mx = mb = 0.0
+        for x0 in range(0, N, 64):
+            bb = b[x0:x0 + 64]
+            dd = a[x0:x0 + 64].to(bb.dtype) - bb
+            num += float((dd.abs() ** 2).sum()); den += float((bb.abs() ** 2).sum())
+            mx = max(mx, float(dd.abs().max())); mb = max(mb, float(bb.abs().max()))
+        e = math.sqrt(num / den)
+        assert e <= t, (name, e)
+        assert mx / mb <= MAXABS * t, (name, mx / mb)
+    d = out["c64"][2] - out["c128"][2]
+    d -= w.L * np.round(d / w.L)
+    assert np.abs(d).max() <= POS_TOL * w.L
+
+
 # ---------------------------------------------------------------- large kick phases (reading G25)
 
 @pytest.mark.parametrize("terms", ["plain", "kappa_layer"])
