@@ -87,12 +87,34 @@ WDM_DEV void rotate_neg_all(cx<float> (&v)[R], const float (&th)[R])
 #pragma unroll
     for (int r = 0; r < R; ++r) mx = fmaxf(mx, fabsf(th[r]));
     if (mx < 0.25f) {
+#if defined(__CUDA_ARCH__) && __CUDA_ARCH__ >= 1000 && !defined(WDM_NO_PACKED_ADD)
+        // the two polynomials of sincos_small for two phases at a time in packed single precision (the same operations
+        // in the same order per phase: identical results, half the issue slots)
+        static_assert(R % 2 == 0, "pairs of phases");
+        auto pk = [](float a, float b) { unsigned long long r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; };
+        auto mul2 = [](unsigned long long a, unsigned long long b) { unsigned long long r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; };
+        auto fma2 = [](unsigned long long a, unsigned long long b, unsigned long long c) { unsigned long long r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; };
+        const unsigned long long k120 = pk(1.0f / 120.0f, 1.0f / 120.0f), km6 = pk(-1.0f / 6.0f, -1.0f / 6.0f), k1 = pk(1.0f, 1.0f),
+                                 km720 = pk(-1.0f / 720.0f, -1.0f / 720.0f), k24 = pk(1.0f / 24.0f, 1.0f / 24.0f), kmh = pk(-0.5f, -0.5f);
+#pragma unroll
+        for (int r = 0; r < R; r += 2) {
+            const unsigned long long t = pk(th[r], th[r + 1]), t2 = mul2(t, t);
+            const unsigned long long sp = mul2(t, fma2(t2, fma2(t2, k120, km6), k1));
+            const unsigned long long cp = fma2(t2, fma2(t2, fma2(t2, km720, k24), kmh), k1);
+            float s0, s1, c0, c1;
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(s0), "=f"(s1) : "l"(sp));
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(c0), "=f"(c1) : "l"(cp));
+            v[r] = mk<float>(v[r].x * c0 + v[r].y * s0, v[r].y * c0 - v[r].x * s0);
+            v[r + 1] = mk<float>(v[r + 1].x * c1 + v[r + 1].y * s1, v[r + 1].y * c1 - v[r + 1].x * s1);
+        }
+#else
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             float s, c;
             sincos_small(th[r], s, c);
             v[r] = mk<float>(v[r].x * c + v[r].y * s, v[r].y * c - v[r].x * s);
         }
+#endif
     } else {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
