@@ -19,10 +19,11 @@
 // 2.2 k: 26 k against 30.6 k for the two 8-line tiles of the generic sweep.
 // The k-th half tile of a CTA goes to buffer k mod 3: tile i uses buffers 2i, 2i + 1 (mod 3); when its last reads are
 // done, half B of tile i + 1 and half A of tile i + 2 are requested into them (the density sweep, whose tail keeps the
-// second buffer, requests that half A at the first barrier of the next tile).  The density sweep forms rho - <rho> from the outgoing registers, splits the packed real lines the same way
-// (U = P_a + P_b, V = (P_a - P_b) w^n, both in the buffer of B so that A's can be refilled at once), and each group runs the
-// packed 512-point transform and the Hermitian split of its half of the spectrum: even rows of H from group 0, odd rows
-// (mirror of k' is N/2 - 1 - k') from group 1 -- 128-byte rows of H.
+// second buffer, requests that half A at the first barrier of the next tile).  The density sweep forms rho - <rho> from
+// the outgoing registers, splits the packed real lines the same way (U = P_a + P_b, V = (P_a - P_b) w^n, both in the
+// buffer of B so that A's can be refilled at once), and each group runs the packed 512-point transform and the Hermitian
+// split of its half of the spectrum: even rows of H from group 0, odd rows (mirror of k' is N/2 - 1 - k') from group 1 --
+// 128-byte rows of H.
 #pragma once
 
 #include "wdm_pipe.cuh"
